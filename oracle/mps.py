@@ -1,0 +1,290 @@
+"""T-1: boundary MPS by zipper + truncated SVD + one-site variational passes.
+Test infrastructure (see oracle/__init__.py).
+
+PAPER.md:137 (boundary MPS, row after row), Sec. III B 1 PAPER.md:149-163 + Fig. 7 (sparse
+diagrams: project the legs to the physical space of size d, batched matmul over the chi legs,
+apply the local Boltzmann factor, project out), Sec. III B 2 PAPER.md:165-179 + Fig. 8 (zipper
+right->left from a left-canonical MPS with the trivial 1x1x1 connector, SVD keeping chi values,
+then variational overlap maximisation).  Readings of silent points: DESIGN.md section 3
+(S1 converged truncated SVD = LAPACK dense SVD here; S2 schedule = whole zipper, then `sweeps`
+passes; S4 one sweep = one pass, alternating, first left->right; S5 gap guard; S6 rank cut).
+
+Conventions.  Row y is a chain of positions: Site_0 [, Med_0.5], Site_1, ...  (Med positions only
+for 3-sub-cluster cells; otherwise Bh is folded into the left leg of the next site).
+  MPS tensors      A[al, p, ar]          (p = lower physical leg of the row = R_{y+1}'s leg)
+  new MPS tensors  N[g, p', g2]          (p' = upper leg = R_y's leg)
+  environments     L[g, w, al], R[g2, w, ar]   (g: new bond, w: MPO bond, al/ar: old bond)
+  connector        C = right environment (the zipper's U*Sigma IS the overlap environment)
+Site MPO tensor (never built, except by `dense()` for the pins):
+  W[(l,i), p', p, (r,o)] = sum_x w(x) d(l,Pl x) d(i,Pi x) d(r,Pr x) d(o,Po x) Bv[p',Pu x] d(p,Pd x)
+Mediating tensor:  W[(r,o), q', q, (l',i')] = Bh[r,l'] d(q,o) Bd[q',i'].
+"""
+import numpy as np
+
+RANK_TOL = 1e-14      # S6: singular values <= RANK_TOL * sigma_1 count as zero
+GAP_GUARD = 1e-6      # S5: never cut between sigma_k, sigma_{k+1} closer than this (relative)
+
+
+def _seg(idx, n):
+    """stable grouping helper: order, segment starts and segment ids for scatter-add by idx."""
+    order = np.argsort(idx, kind="stable")
+    sidx = idx[order]
+    starts = np.flatnonzero(np.r_[True, sidx[1:] != sidx[:-1]])
+    return order, starts, sidx[starts]
+
+
+def _scatter_add(out, idx, vals, seg=None):
+    """out[idx[k]] += vals[k] (first axis)."""
+    order, starts, ids = seg if seg is not None else _seg(idx, out.shape[0])
+    out[ids] += np.add.reduceat(vals[order], starts, axis=0)
+    return out
+
+
+class SitePos:
+    def __init__(self, model, y, x):
+        c = model.cells[y][x]
+        self.kind = "site"
+        self.fold = not model.has_med
+        self.w = c.w
+        self.n_i, self.n_o = c.n["din"], c.n["dout"]
+        self.iL = c.P["left"] * self.n_i + c.P["din"]
+        self.iR = c.P["right"] * self.n_o + c.P["dout"]
+        self.Pu, self.Pd = c.P["up"], c.P["down"]
+        self.n_u = c.n["up"]
+        self.nL = c.n["left"] * self.n_i
+        self.Bv = model.Bv[(y, x)]                       # [p', u]
+        self.Bh = model.Bh[(y, x)] if self.fold else None  # [r_prev, l]
+        self.wl = self.Bh.shape[0] if self.fold else self.nL
+        self.wr = c.n["right"] * self.n_o
+        self.pu, self.pd = self.Bv.shape[0], c.n["down"]
+        self.d = c.d
+        self.chunk = 1 << 16
+
+    # -- helpers -----------------------------------------------------------------------------
+    def _left_in(self, L):
+        return np.einsum("gra,rl->gla", L, self.Bh) if self.fold else L
+
+    def _left_out(self, Ll):
+        return np.einsum("gla,rl->gra", Ll, self.Bh) if self.fold else Ll
+
+    def _chunks(self):
+        for s in range(0, self.d, self.chunk):
+            yield slice(s, min(self.d, s + self.chunk))
+
+    # -- Fig. 7(a,b) diagrams ---------------------------------------------------------------
+    def update(self, L, A, R):
+        """N[g,p',g2] = sum L[g,wl,al] W[wl,p',p,wr] A[al,p,ar] R[g2,wr,ar]."""
+        Ll = self._left_in(L)
+        N0 = np.zeros((self.n_u, L.shape[0], R.shape[0]))
+        for sl in self._chunks():
+            Lx = Ll[:, self.iL[sl], :].transpose(1, 0, 2)          # [x, g, al]
+            Ax = A[:, self.Pd[sl], :].transpose(1, 0, 2)           # [x, al, ar]
+            Rx = R[:, self.iR[sl], :].transpose(1, 2, 0)           # [x, ar, g2]
+            T = (Lx @ Ax @ Rx) * self.w[sl, None, None]
+            _scatter_add(N0, self.Pu[sl], T)
+        return np.einsum("pu,ugd->gpd", self.Bv, N0)
+
+    def env_left(self, L, A, N):
+        """L'[g2,wr,ar] = sum L[g,wl,al] N[g,p',g2] W[wl,p',p,wr] A[al,p,ar]."""
+        Ll = self._left_in(L)
+        Nb = np.einsum("pu,gpd->udg", self.Bv, N)                  # [u, g2, g]
+        out = np.zeros((self.wr, N.shape[2], A.shape[2]))
+        for sl in self._chunks():
+            T = Nb[self.Pu[sl]] @ Ll[:, self.iL[sl], :].transpose(1, 0, 2) @ A[:, self.Pd[sl], :].transpose(1, 0, 2)
+            _scatter_add(out, self.iR[sl], T * self.w[sl, None, None])
+        return out.transpose(1, 0, 2)
+
+    def env_right(self, R, A, N):
+        """R'[g,wl,al] = sum N[g,p',g2] W[wl,p',p,wr] A[al,p,ar] R[g2,wr,ar]."""
+        Nb = np.einsum("pu,gpd->ugd", self.Bv, N)                  # [u, g, g2]
+        out = np.zeros((self.nL, N.shape[0], A.shape[0]))
+        for sl in self._chunks():
+            T = Nb[self.Pu[sl]] @ R[:, self.iR[sl], :].transpose(1, 0, 2) @ A[:, self.Pd[sl], :].transpose(1, 2, 0)
+            _scatter_add(out, self.iL[sl], T * self.w[sl, None, None])
+        return self._left_out(out.transpose(1, 0, 2))
+
+    def theta(self, A, C):
+        """Theta[(al,wl),(p',g)] = sum A[al,p,ar] W[wl,p',p,wr] C[g,wr,ar]  (Fig. 8(c) dashed box)."""
+        out = np.zeros((self.nL * self.n_u, A.shape[0], C.shape[0]))
+        for sl in self._chunks():
+            T = A[:, self.Pd[sl], :].transpose(1, 0, 2) @ C[:, self.iR[sl], :].transpose(1, 2, 0)
+            _scatter_add(out, self.iL[sl] * self.n_u + self.Pu[sl], T * self.w[sl, None, None])
+        T0 = out.reshape(self.nL, self.n_u, A.shape[0], C.shape[0])
+        T1 = np.einsum("pu,luag->lpag", self.Bv, T0)
+        if self.fold:
+            T1 = np.einsum("rl,lpag->rpag", self.Bh, T1)
+        return T1.transpose(2, 0, 1, 3).reshape(A.shape[0] * self.wl, self.pu * C.shape[0])
+
+    def dense(self):
+        """Explicit W[wl, p', p, wr] (tiny cells only; used by the pins)."""
+        W0 = np.zeros((self.nL, self.n_u, self.pd, self.wr))
+        np.add.at(W0, (self.iL, self.Pu, self.Pd, self.iR), self.w)
+        W = np.einsum("pu,ludr->lpdr", self.Bv, W0)
+        return np.einsum("rl,lpdw->rpdw", self.Bh, W) if self.fold else W
+
+
+class MedPos:
+    def __init__(self, model, y, x):
+        """Mediating tensor between Site_x and Site_{x+1} of row y (Fig. 5)."""
+        cl, cr = model.cells[y][x], model.cells[y][x + 1]
+        self.kind = "med"
+        self.Bh = model.Bh[(y, x + 1)]        # [r, l']
+        self.Bd = model.Bd[(y, x + 1)]        # [q', i']
+        self.n_r, self.n_o = cl.n["right"], cl.n["dout"]
+        self.n_l, self.n_i = cr.n["left"], cr.n["din"]
+        self.wl, self.wr = self.n_r * self.n_o, self.n_l * self.n_i
+        self.pu, self.pd = self.Bd.shape[0], self.n_o
+
+    def _L4(self, L):
+        return L.reshape(L.shape[0], self.n_r, self.n_o, L.shape[2])
+
+    def _R4(self, R):
+        return R.reshape(R.shape[0], self.n_l, self.n_i, R.shape[2])
+
+    def update(self, L, A, R):
+        return np.einsum("groa,aob,rl,qi,dlib->gqd", self._L4(L), A, self.Bh, self.Bd, self._R4(R), optimize=True)
+
+    def env_left(self, L, A, N):
+        out = np.einsum("groa,gqd,aob,rl,qi->dlib", self._L4(L), N, A, self.Bh, self.Bd, optimize=True)
+        return out.reshape(out.shape[0], self.wr, out.shape[3])
+
+    def env_right(self, R, A, N):
+        out = np.einsum("gqd,aob,rl,qi,dlib->groa", N, A, self.Bh, self.Bd, self._R4(R), optimize=True)
+        return out.reshape(out.shape[0], self.wl, out.shape[3])
+
+    def theta(self, A, C):
+        T = np.einsum("aob,rl,qi,glib->aroqg", A, self.Bh, self.Bd, self._R4(C), optimize=True)
+        return T.reshape(A.shape[0] * self.wl, self.pu * C.shape[0])
+
+    def dense(self):
+        # W[(r,o), q', q, (l',i')] = Bh[r,l'] d(q,o) Bd[q',i']
+        W = np.einsum("rl,qi,ko->roqkli", self.Bh, self.Bd, np.eye(self.n_o))
+        return W.reshape(self.wl, self.pu, self.pd, self.wr)
+
+
+def row_positions(model, y):
+    pos = []
+    for x in range(model.Lx):
+        pos.append(SitePos(model, y, x))
+        if model.has_med and x + 1 < model.Lx:
+            pos.append(MedPos(model, y, x))
+    return pos
+
+
+def trivial_mps(model):
+    """R_{Ly} = 1: all legs of size 1."""
+    n = 2 * model.Lx - 1 if model.has_med else model.Lx
+    return [np.ones((1, 1, 1)) for _ in range(n)]
+
+
+def left_canonicalize(A):
+    """C-1: QR chain left->right (Fig. 8(c) 'initial MPS in the left canonical form').
+    Returns the isometries and the final 1x1 factor (the signed norm)."""
+    A = [a.copy() for a in A]
+    for j in range(len(A)):
+        al, p, ar = A[j].shape
+        Q, Rf = np.linalg.qr(A[j].reshape(al * p, ar))
+        A[j] = Q.reshape(al, p, Q.shape[1])
+        if j + 1 < len(A):
+            A[j + 1] = np.einsum("ab,bpc->apc", Rf, A[j + 1])
+    assert Rf.shape == (1, 1)
+    return A, Rf[0, 0]
+
+
+def truncate_rank(s, D, gap_guard=True):
+    """C-3 / S5 / S6: number of singular values kept."""
+    if s.size == 0 or s[0] == 0.0:
+        return 1
+    k = int(np.count_nonzero(s > RANK_TOL * s[0]))
+    if D > 0 and k > D:
+        k = D
+        if gap_guard:
+            while k > 1 and s[k] >= (1.0 - GAP_GUARD) * s[k - 1]:
+                k -= 1
+    return max(k, 1)
+
+
+def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
+    """R_y = compress(T_y R_{y+1}; D, sweeps).  A: tensors of R_{y+1} (any gauge).
+    Returns (tensors of R_y with unit norm, log of the norm removed)."""
+    n = len(positions)
+    A, r_last = left_canonicalize(A)
+    Renv = [None] * n
+    Renv[n - 1] = np.full((1, 1, 1), r_last)       # trivial unity connector x the folded norm
+    N = [None] * n
+    min_sigma = []
+    for j in range(n - 1, -1, -1):                  # C-2 zipper, right -> left
+        pos = positions[j]
+        Th = pos.theta(A[j], Renv[j])
+        U, s, Vt = np.linalg.svd(Th, full_matrices=False)
+        k = truncate_rank(s, D, gap_guard)
+        min_sigma.append(s[k - 1] / s[0] if s[0] > 0 else 0.0)
+        N[j] = Vt[:k].reshape(k, pos.pu, Renv[j].shape[0])
+        Cn = (U[:, :k] * s[:k]).reshape(A[j].shape[0], pos.wl, k)
+        if j > 0:
+            Renv[j - 1] = Cn.transpose(2, 1, 0)
+    assert Cn.shape == (1, 1, 1)
+    centre = 0
+    N[0] = N[0] * Cn[0, 0, 0]
+    norms = []
+    if D > 0:                                       # C-5: exact mode skips the passes
+        Lenv = [None] * n
+        Lenv[0] = np.ones((1, 1, 1))
+        for sweep in range(sweeps):                 # C-4
+            if sweep % 2 == 0:
+                for j in range(n):
+                    N[j] = positions[j].update(Lenv[j], A[j], Renv[j])
+                    norms.append(np.linalg.norm(N[j]))
+                    if j + 1 < n:
+                        g, p, g2 = N[j].shape
+                        Q, _ = np.linalg.qr(N[j].reshape(g * p, g2))
+                        N[j] = Q.reshape(g, p, Q.shape[1])
+                        Lenv[j + 1] = positions[j].env_left(Lenv[j], A[j], N[j])
+                centre = n - 1
+            else:
+                for j in range(n - 1, -1, -1):
+                    N[j] = positions[j].update(Lenv[j], A[j], Renv[j])
+                    norms.append(np.linalg.norm(N[j]))
+                    if j > 0:
+                        g, p, g2 = N[j].shape
+                        Q, _ = np.linalg.qr(N[j].reshape(g, p * g2).T)
+                        N[j] = Q.T.reshape(Q.shape[1], p, g2)
+                        Renv[j - 1] = positions[j].env_right(Renv[j], A[j], N[j])
+                centre = 0
+    nrm = np.linalg.norm(N[centre])
+    N[centre] = N[centre] / nrm
+    if stats is not None:
+        stats.setdefault("min_sigma", []).append(min(min_sigma))
+        stats.setdefault("pass_norms", []).append(norms)
+        stats.setdefault("bonds", []).append([t.shape[2] for t in N])
+    return N, float(np.log(nrm))
+
+
+def contract(model, D, sweeps, gap_guard=True, stats=None):
+    """Boundary MPS R_y for y = Ly .. 1 (R_0 is never needed: log Z comes from the first cell's
+    normaliser in the search, C-6).  Returns {y: tensors}, {y: log-norm}."""
+    R = {model.Ly: trivial_mps(model)}
+    lognorm = {model.Ly: 0.0}
+    for y in range(model.Ly - 1, 0, -1):
+        R[y], lognorm[y] = compress(row_positions(model, y), R[y + 1], D, sweeps, gap_guard, stats)
+    return R, lognorm
+
+
+def mps_to_dense(T):
+    """Boundary MPS -> dense array with one axis per position (tiny only)."""
+    v = T[0]
+    for t in T[1:]:
+        v = np.tensordot(v, t, axes=([v.ndim - 1], [0]))
+    return v.reshape(v.shape[1:-1])
+
+
+def mpo_mps_dense(positions, A):
+    """Exact (untruncated) T_y R_{y+1} as a dense array, via the explicit W tensors (tiny only)."""
+    v = None
+    for pos, a in zip(positions, A):
+        t = np.einsum("wpdv,adb->awpvb", pos.dense(), a)         # [al, wl, p', wr, ar]
+        if v is None:
+            v = t[0, 0]                                            # [p', wr, ar]
+        else:
+            v = np.tensordot(v, t, axes=([v.ndim - 2, v.ndim - 1], [1, 0]))
+    return v.reshape(v.shape[:-2])

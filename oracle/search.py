@@ -1,0 +1,185 @@
+"""T-2: branch and bound over cells driven by boundary-MPS conditionals; O-3 exact-marginal beam.
+Test infrastructure (see oracle/__init__.py).
+
+PAPER.md:94-98 Eq. (7) chain rule p(x_{n+1}) = p(x_{n+1} | x_n) p(x_n); Fig. 3
+(branch to d*M candidates, keep the M most probable); Eqs. (8)-(9) PAPER.md:100-107 (conditionals
+depend only on the boundary of the prefix); Fig. 6(b) PAPER.md:143 (fixed legs above, one open site,
+boundary MPS R_{y+1} below, contracted numerically exactly, 'up to normalization'); p_d
+PAPER.md:113 (largest discarded probability).  Search order: row-major.
+
+For beam element m at cell (x, y) (rows < y and cells < x of row y fixed; S, Q = tensors of R_{y+1}):
+  u(m; X) = hvec[Pl X] dvec[Pi X] uvec[Pu X] w(X) * (Lv . S[:,Pd X,:] . Q[:,Po X,:] . RM_x[:, Pr X])
+  hvec = Bh_x[Pr(left neighbour state), :], uvec = Bv_x[Pd(upper state), :], dvec = Bd_x[Po(upper-left), :]
+  Lv    = product of S.Q of the already fixed cells of row y (row vector)
+  RM_x  = right block: contraction of columns > x of rows y (summed) with the fixed row y-1 above,
+          RM_{Lx-1} = 1;  RS_x[b', l] = sum_{X: Pl X = l} dvec uvec w(X) (S[b',Pd X,:] Q[:,Po X,:] RM_x[:, Pr X]);
+          RM_{x-1}[b', r] = sum_l Bh_x[r, l] RS_x[b', l]
+  p = max(u, 0) / sum max(u, 0)   (S7: a truncated MPS can give small negative u; they are clamped)
+Ties (S8): candidates are ordered by (logp desc, parent rank asc, cell state asc).
+Positive rescalings of Lv and RM cancel in p; their logs are tracked only where log Z needs them.
+"""
+import numpy as np
+from . import energy as _energy
+
+
+def select_top(scores, parent, state, M):
+    """Indices of the M best candidates in the S8 total order, best first, and the best
+    discarded score (or -inf)."""
+    n = scores.size
+    if n > M + 1:                      # prefilter: everything >= the (M+1)-th largest score
+        kth = n - (M + 1)
+        thr = np.partition(scores, kth)[kth]
+        sub = np.flatnonzero(scores >= thr)
+    else:
+        sub = np.arange(n)
+    order = sub[np.lexsort((state[sub], parent[sub], -scores[sub]))]
+    keep = order[:M]
+    disc = scores[order[M]] if order.size > M else -np.inf
+    return keep, disc
+
+
+class _RowCtx:
+    """Per-row tables of the search: cells of row y and the tensors of R_{y+1}."""
+
+    def __init__(self, model, y, Rnext):
+        self.cells = model.cells[y]
+        Lx = model.Lx
+        if model.has_med:
+            self.S = [Rnext[2 * x] for x in range(Lx)]
+            self.Q = [Rnext[2 * x + 1] if x + 1 < Lx else None for x in range(Lx)]
+        else:
+            self.S = list(Rnext)
+            self.Q = [None] * Lx
+        self.G = []          # G[x][pd, po] = S[:,pd,:] @ Q[:,po,:]  -> [n_down, n_dout, Dl, Dr']
+        for x in range(Lx):
+            S = self.S[x]
+            if self.Q[x] is None:
+                assert self.cells[x].n["dout"] == 1
+                self.G.append(S.transpose(1, 0, 2)[:, None, :, :])
+            else:
+                self.G.append(np.einsum("apb,bqc->pqac", S, self.Q[x]))
+
+
+def _right_blocks(model, y, ctx, above):
+    """RM_x for x = 0..Lx-1 given the states `above` of row y-1 (None for y = 0).
+    Returns list of (RM [D', n_r], log-scale)."""
+    Lx = model.Lx
+    RM = [None] * Lx
+    RM[Lx - 1] = (np.ones((1, 1)), 0.0)
+    for x in range(Lx - 1, 0, -1):
+        c = ctx.cells[x]
+        uvec, dvec = _above_vectors(model, y, x, above)
+        rm, ls = RM[x]
+        Gx = ctx.G[x][c.P["down"], c.P["dout"]]                     # [d, Dl, Dr']
+        v = np.einsum("xab,bx->xa", Gx, rm[:, c.P["right"]])         # [d, Dl]
+        v = v * (dvec[c.P["din"]] * uvec[c.P["up"]] * c.w)[:, None]
+        RS = np.zeros((c.n["left"], v.shape[1]))
+        np.add.at(RS, c.P["left"], v)
+        new = (model.Bh[(y, x)] @ RS).T                             # [Dl, n_r(x-1)]
+        s = np.abs(new).max()
+        RM[x - 1] = (new / s, ls + np.log(s))
+    return RM
+
+
+def _above_vectors(model, y, x, above):
+    if y == 0 or above is None:
+        return np.ones(1), np.ones(1)
+    up = model.cells[y - 1][x]
+    uvec = model.Bv[(y, x)][up.P["down"][above[x]], :]
+    if x > 0:
+        ul = model.cells[y - 1][x - 1]
+        dvec = model.Bd[(y, x)][ul.P["dout"][above[x - 1]], :]
+    else:
+        dvec = np.ones(1)
+    return uvec, dvec
+
+
+def branch_and_bound(model, R, lognorm, M, stats=None):
+    """Returns dict(states [n, N] int8 +-1, energies [n], logp [n] (descending), log_pd, log_z,
+    cell_states [n, Ly*Lx])."""
+    Ly, Lx = model.Ly, model.Lx
+    beam_states = [[]]                  # per element: list of chosen cell states (row-major)
+    beam_logp = np.zeros(1)
+    log_pd = -np.inf
+    log_z = None
+    n_neg = 0
+    for y in range(Ly):
+        ctx = _RowCtx(model, y, R[y + 1])
+        # B-1: right blocks at the row start, memoised by the boundary they depend on (Eq. (9))
+        cache = {}
+        slots = []
+        for st in beam_states:
+            above = tuple(st[(y - 1) * Lx:(y - 1) * Lx + Lx]) if y > 0 else None
+            if above not in cache:
+                cache[above] = _right_blocks(model, y, ctx, above)
+            slots.append(cache[above])
+        Lv = [np.ones(1) for _ in beam_states]
+        for x in range(Lx):
+            c = ctx.cells[x]
+            cand_score, cand_parent, cand_state = [], [], []
+            tables = []
+            for m, st in enumerate(beam_states):
+                above = st[(y - 1) * Lx:(y - 1) * Lx + Lx] if y > 0 else None
+                uvec, dvec = _above_vectors(model, y, x, above)
+                hvec = model.Bh[(y, x)][ctx.cells[x - 1].P["right"][st[-1]], :] if x > 0 else np.ones(1)
+                rm, rm_ls = slots[m][x]
+                tab = np.einsum("a,pqac->pqc", Lv[m], ctx.G[x])          # Lv.S.Q for every (pd, po)
+                val = np.einsum("xc,cx->x", tab[c.P["down"], c.P["dout"]], rm[:, c.P["right"]])
+                u = hvec[c.P["left"]] * dvec[c.P["din"]] * uvec[c.P["up"]] * c.w * val
+                n_neg += int(np.count_nonzero(u < 0))
+                u = np.maximum(u, 0.0)                                     # S7
+                Z = u.sum()
+                if y == 0 and x == 0:                                      # C-6
+                    log_z = (-model.beta * model.offset + sum(lognorm[yy] for yy in range(1, Ly))
+                             + np.log(Z) + rm_ls)
+                with np.errstate(divide="ignore"):
+                    cand_score.append(beam_logp[m] + np.log(u / Z))
+                cand_parent.append(np.full(c.d, m))
+                cand_state.append(np.arange(c.d))
+                tables.append(tab)
+            score = np.concatenate(cand_score)
+            parent = np.concatenate(cand_parent)
+            state = np.concatenate(cand_state)
+            keep, disc = select_top(score, parent, state, M)
+            keep = keep[np.isfinite(score[keep])]                          # never keep p = 0
+            log_pd = max(log_pd, disc)
+            new_states, new_Lv, new_slots = [], [], []
+            for k in keep:
+                m, X = int(parent[k]), int(state[k])
+                new_states.append(beam_states[m] + [X])
+                lv = tables[m][c.P["down"][X], c.P["dout"][X]]
+                new_Lv.append(lv / np.abs(lv).max())
+                new_slots.append(slots[m])
+            beam_states, Lv, slots = new_states, new_Lv, new_slots
+            beam_logp = score[keep]
+    cs = np.asarray(beam_states, dtype=np.int64)
+    spins = model.spins_of_cells(cs)
+    if stats is not None:
+        stats["negative_u"] = n_neg
+    return dict(states=spins, energies=_energy.energies(model.inst, spins), logp=beam_logp,
+                log_pd=log_pd, log_z=log_z, cell_states=cs)
+
+
+def exact_marginal_beam(model, E_all, M):
+    """O-3: the same beam, with conditionals from brute-force prefix marginals (Eq. (7))."""
+    from . import brute
+    inst = model.inst
+    N, nb = inst.n_spins, model.nbits
+    ncell = model.Ly * model.Lx
+    d = 1 << nb
+    prefix = np.zeros(1, dtype=np.int64)      # prefix value = low bits of the global state index
+    logp = np.zeros(1)
+    log_pd = -np.inf
+    for n in range(ncell):
+        lm = brute.prefix_log_marginals(E_all, model.beta, N, (n + 1) * nb)
+        X = np.arange(d, dtype=np.int64)
+        cand_prefix = (prefix[:, None] | (X[None, :] << (n * nb))).reshape(-1)
+        score = lm[cand_prefix]
+        parent = np.repeat(np.arange(prefix.size), d)
+        state = np.tile(X, prefix.size)
+        keep, disc = select_top(score, parent, state, M)
+        log_pd = max(log_pd, disc)
+        prefix, logp = cand_prefix[keep], score[keep]
+    cs = (prefix[:, None] >> (np.arange(ncell) * nb)[None, :]) & (d - 1)
+    spins = model.spins_of_cells(cs)
+    return dict(states=spins, energies=_energy.energies(inst, spins), logp=logp, log_pd=log_pd, cell_states=cs)

@@ -1,0 +1,357 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+P-numbers follow SURVEY.md section 8(c) / DESIGN.md section 5.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import instances
+from oracle import brute, energy, model, mps, search, transfer
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "cfg1_bruteforce.txt")
+
+MINIS = [  # (Ly, Lx, S, n_s, p_keep, seed, beta): all small enough for brute force
+    (2, 2, 3, 2, 0.8, 3, 1.3),      # Pegasus-shaped miniature (mediating tensors, thinned edges)
+    (3, 2, 2, 2, 0.9, 5, 0.7),      # Zephyr-shaped miniature
+    (2, 3, 1, 4, 1.0, 1, 1.5),      # config-1 shape, other seed
+    (2, 3, 2, 2, 0.9, 7, 0.9),
+]
+
+
+def read_golden():
+    lz, rows = None, []
+    for line in open(GOLD):
+        t = line.split()
+        if t[0] == "log_z":
+            lz = float(t[1])
+        elif t[0] == "state":
+            rows.append((int(t[1]), float(t[3])))
+    return lz, rows
+
+
+# ---------------------------------------------------------------- O-0 energy
+def test_energy_fixed_order_matches_python_loop():
+    inst = instances.lattice(2, 2, 3, 4, p_keep=0.9, seed=11)
+    rng = np.random.default_rng(0)
+    s = (1 - 2 * rng.integers(0, 2, size=(5, inst.n_spins))).astype(np.int8)
+    Ev = energy.energies(inst, s)
+    for k in range(5):
+        assert Ev[k] == energy.energy(inst, s[k])          # bit-exact
+    # independent closed evaluation: quadratic form (different summation order -> tolerance)
+    A = np.zeros((inst.n_spins, inst.n_spins))
+    A[inst.edge_u, inst.edge_v] += inst.J
+    ref = np.einsum("ki,ij,kj->k", s.astype(float), A, s.astype(float)) + s @ inst.h
+    assert np.allclose(Ev, ref, rtol=0, atol=1e-12)
+
+
+def test_energy_hand_example():
+    # two spins, one bond: H = J s0 s1 + h0 s0 + h1 s1
+    inst = instances.Instance(n_spins=2, edge_u=np.array([0]), edge_v=np.array([1]), J=np.array([0.5]),
+                              h=np.array([0.25, -1.0]))
+    assert energy.energy(inst, [1, 1]) == 0.5 + 0.25 - 1.0
+    assert energy.energy(inst, [1, -1]) == -0.5 + 0.25 + 1.0
+    assert energy.energy(inst, [-1, -1]) == 0.5 - 0.25 + 1.0
+
+
+# ---------------------------------------------------------------- P1: brute force == exact transfer
+def test_cfg1_bruteforce_matches_golden_and_transfer(cfg1):
+    inst, run, E = cfg1
+    beta = run["beta"][0]
+    lz_gold, rows = read_golden()
+    assert abs(brute.log_z(E, beta) - lz_gold) <= 1e-13 * abs(lz_gold)
+    idx, El = brute.lowest(E, 16)
+    assert [k for k, _ in rows] == idx.tolist()
+    s = brute.index_to_spins(idx, inst.n_spins)
+    assert np.allclose(energy.energies(inst, s), [e for _, e in rows], rtol=0, atol=1e-12)
+    m = model.Model(inst).set_beta(beta)
+    lz, _ = transfer.log_z(m)
+    assert abs(lz - lz_gold) <= 1e-12 * abs(lz_gold)
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta", MINIS)
+def test_transfer_matches_bruteforce(Ly, Lx, S, ns, p, seed, beta):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    E = brute.all_energies(inst)
+    m = model.Model(inst).set_beta(beta)
+    lz, _ = transfer.log_z(m)
+    assert abs(lz - brute.log_z(E, beta)) <= 1e-12 * abs(lz)
+
+
+# ---------------------------------------------------------------- sparse diagrams == explicit MPO
+@pytest.mark.parametrize("S,ns", [(1, 4), (2, 2), (3, 2)])
+def test_sparse_diagrams_match_dense_mpo(S, ns):
+    inst = instances.lattice(2, 3, S, ns, p_keep=0.85, seed=2)
+    m = model.Model(inst).set_beta(0.8)
+    rng = np.random.default_rng(1)
+    for y in range(2):
+        for pos in mps.row_positions(m, y):
+            W = pos.dense()
+            wl, pu, pd, wr = W.shape
+            g, al, ar, g2 = 3, 2, 4, 5
+            L = rng.normal(size=(g, wl, al))
+            A = rng.normal(size=(al, pd, ar))
+            R = rng.normal(size=(g2, wr, ar))
+            N = rng.normal(size=(g, pu, g2))
+            assert np.allclose(pos.update(L, A, R), np.einsum("gwa,wpdv,adb,hvb->gph", L, W, A, R), atol=1e-11)
+            assert np.allclose(pos.env_left(L, A, N), np.einsum("gwa,gph,wpdv,adb->hvb", L, N, W, A), atol=1e-11)
+            assert np.allclose(pos.env_right(R, A, N), np.einsum("gph,wpdv,adb,hvb->gwa", N, W, A, R), atol=1e-11)
+            th = np.einsum("adb,wpdv,hvb->awph", A, W, R).reshape(al * wl, pu * g2)
+            assert np.allclose(pos.theta(A, R), th, atol=1e-11)
+
+
+# ---------------------------------------------------------------- P2: exact-D MPS == exact transfer
+def _dense_of_mps(m, T, shape):
+    v = mps.mps_to_dense(T)
+    if m.has_med:
+        n = m.Lx
+        v = np.transpose(v, [2 * x for x in range(n)] + [2 * x + 1 for x in range(n - 1)])
+    return v.reshape(shape)
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta", MINIS + [(3, 3, 3, 2, 0.85, 7, 0.9)])
+def test_exact_mps_reproduces_transfer_vectors(Ly, Lx, S, ns, p, seed, beta):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    m = model.Model(inst).set_beta(beta)
+    _, R = transfer.log_z(m)
+    Rm, ln = mps.contract(m, 0, 0)
+    acc = 0.0
+    for y in range(Ly - 1, 0, -1):
+        acc += ln[y]
+        arr, ls = R[y]
+        v = _dense_of_mps(m, Rm[y], arr.shape)
+        assert abs(1 - abs((arr / np.linalg.norm(arr) * v).sum())) < 1e-12
+        assert abs(acc - (ls + np.log(np.linalg.norm(arr)))) < 1e-12 * max(1.0, abs(acc))
+
+
+# ---------------------------------------------------------------- P3: beam at exact D == exact-marginal beam
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta", MINIS)
+def test_beam_exact_D_matches_exact_marginal_beam(Ly, Lx, S, ns, p, seed, beta):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    E = brute.all_energies(inst)
+    lzb = brute.log_z(E, beta)
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, 8)
+    ref = search.exact_marginal_beam(m, E, 8)
+    assert abs(out["log_z"] - lzb) <= 1e-12 * abs(lzb)
+    assert np.array_equal(out["states"], ref["states"])
+    assert np.allclose(out["logp"], ref["logp"], rtol=0, atol=1e-10)
+    assert abs(out["log_pd"] - ref["log_pd"]) < 1e-10
+    assert np.array_equal(out["energies"], ref["energies"])
+    # final log-probabilities are Boltzmann: log p(s) = -beta E(s) - log Z   (Eq. (6))
+    assert np.allclose(out["logp"], -beta * out["energies"] - lzb, rtol=0, atol=1e-10)
+    # conditionals are normalised: sum over the d candidates of one parent (checked through P6's
+    # identity: the kept log-probabilities never exceed 0 and p_d is a probability)
+    assert out["logp"].max() <= 1e-12 and out["log_pd"] <= 1e-12
+
+
+def test_cfg1_beam_against_golden(cfg1):
+    """Config 1 at its stated settings (beta = 1, exact D, M = 16).  S12: the beam ranks by marginal
+    probability, so equality with the brute-force lowest-16 is not a theorem; the ground state and
+    the Boltzmann identity are."""
+    inst, run, E = cfg1
+    beta = run["beta"][0]
+    lz_gold, rows = read_golden()
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, run["M"])
+    assert abs(out["log_z"] - lz_gold) <= 1e-12 * abs(lz_gold)
+    assert abs(out["energies"].min() - rows[0][1]) < 1e-12
+    assert np.array_equal(out["states"][0], brute.index_to_spins(np.array([rows[0][0]]), inst.n_spins)[0])
+    assert np.allclose(out["logp"], -beta * out["energies"] - lz_gold, atol=1e-10)
+    ref = search.exact_marginal_beam(m, E, run["M"])
+    assert np.array_equal(out["states"], ref["states"])
+
+
+# ---------------------------------------------------------------- P4: closed forms (lattices too big for brute force)
+def _logz_mps(inst, beta, D=8, sweeps=1):
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, D, sweeps)
+    return search.branch_and_bound(m, Rm, ln, 4)["log_z"]
+
+
+@pytest.mark.parametrize("S,ns", [(2, 4), (3, 2)])
+def test_closed_form_zero_couplings(S, ns):
+    inst = instances.lattice(3, 3, S, ns, p_keep=0.9, seed=4)
+    inst["J"] = np.zeros_like(inst.J)
+    beta = 0.7
+    ref = np.log(2 * np.cosh(beta * inst.h)).sum()
+    assert abs(_logz_mps(inst, beta) - ref) <= 1e-12 * abs(ref)
+
+
+@pytest.mark.parametrize("S,ns", [(2, 4), (3, 2)])
+def test_closed_form_tree(S, ns):
+    """Spanning forest of the lattice graph, h = 0:  Z = 2^(#components) ... = 2^N prod cosh(beta J_e)."""
+    inst = instances.lattice(3, 3, S, ns, p_keep=1.0, seed=6, h="zero")
+    parent = list(range(inst.n_spins))
+
+    def find(a):
+        while parent[a] != a:
+            parent[a] = parent[parent[a]]
+            a = parent[a]
+        return a
+    keep = []
+    for e, (u, v) in enumerate(zip(inst.edge_u.tolist(), inst.edge_v.tolist())):
+        ru, rv = find(u), find(v)
+        if ru != rv:
+            parent[ru] = rv
+            keep.append(e)
+    for k in ("edge_u", "edge_v", "J"):
+        inst[k] = inst[k][keep]
+    beta = 0.9
+    ref = inst.n_spins * np.log(2.0) + np.log(np.cosh(beta * inst.J)).sum()
+    assert abs(_logz_mps(inst, beta, D=16) - ref) <= 1e-11 * abs(ref)
+
+
+def test_small_beta_expansion():
+    """log Z = N log 2 + beta^2/2 (sum J^2 + sum h^2) + O(beta^3)."""
+    inst = instances.lattice(3, 3, 2, 4, p_keep=0.95, seed=8)
+    beta = 1e-3
+    ref = inst.n_spins * np.log(2.0) + 0.5 * beta ** 2 * ((inst.J ** 2).sum() + (inst.h ** 2).sum())
+    got = _logz_mps(inst, beta)
+    assert abs(got - ref) < 50 * beta ** 3 * (np.abs(inst.J).sum() + np.abs(inst.h).sum())
+    assert abs(got - inst.n_spins * np.log(2.0)) > 0.4 * (ref - inst.n_spins * np.log(2.0))
+
+
+# ---------------------------------------------------------------- P5: invariances
+def test_gauge_invariance_and_z2():
+    inst = instances.lattice(2, 3, 2, 2, p_keep=0.9, seed=9)
+    beta, M = 1.1, 12
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, M)
+    g = np.where(np.random.default_rng(5).random(inst.n_spins) < 0.5, -1.0, 1.0)
+    inst2 = instances.Instance(inst)
+    inst2["J"] = inst.J * g[inst.edge_u] * g[inst.edge_v]
+    inst2["h"] = inst.h * g
+    m2 = model.Model(inst2).set_beta(beta)
+    R2, ln2 = mps.contract(m2, 0, 0)
+    out2 = search.branch_and_bound(m2, R2, ln2, M)
+    assert abs(out["log_z"] - out2["log_z"]) < 1e-11
+    assert np.allclose(np.sort(out["energies"]), np.sort(out2["energies"]), atol=1e-11)
+    a = {tuple(r) for r in (out["states"] * g.astype(np.int8)).tolist()}
+    b = {tuple(r) for r in out2["states"].tolist()}
+    assert a == b
+    # h = 0  =>  p(s) = p(-s): the returned list is closed under global flip (M even, no pruning ties)
+    inst3 = instances.lattice(2, 2, 2, 2, p_keep=1.0, seed=10, h="zero")
+    m3 = model.Model(inst3).set_beta(0.8)
+    R3, ln3 = mps.contract(m3, 0, 0)
+    o3 = search.branch_and_bound(m3, R3, ln3, 1 << 16)
+    lp = {tuple(r): l for r, l in zip(o3["states"].tolist(), o3["logp"].tolist())}
+    for r, l in list(lp.items())[:200]:
+        assert abs(lp[tuple(-np.array(r))] - l) < 1e-10
+
+
+# ---------------------------------------------------------------- P7: no-prune beam == brute-force ordering
+def test_no_prune_beam_equals_bruteforce_order():
+    inst = instances.lattice(2, 2, 1, 4, p_keep=1.0, seed=12)           # N = 16, d^n = 65536
+    beta = 1.0
+    E = brute.all_energies(inst)
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, 1 << 16)
+    assert out["states"].shape[0] == 1 << 16
+    idx, El = brute.lowest(E, 64)
+    assert np.allclose(out["energies"][:64], El, rtol=0, atol=1e-12)
+    k = (((1 - out["states"][:64].astype(np.int64)) // 2) << np.arange(16)).sum(axis=1)
+    gaps = np.diff(El)
+    for r in range(64):
+        if (r == 0 or gaps[r - 1] > 1e-9) and (r == 63 or gaps[r] > 1e-9):
+            assert k[r] == idx[r]
+    assert out["log_pd"] == -np.inf
+
+
+# ---------------------------------------------------------------- P8: loop-planted ground state
+@pytest.mark.parametrize("seed", [0, 1])
+def test_loop_planted_ground_state(seed):
+    inst = instances.loop_planted(2, 3, 1, 4, seed=seed)                # N = 24
+    E = brute.all_energies(inst)
+    assert abs(E.min() - inst.E0) < 1e-12
+    assert energy.energy(inst, inst.s_star) == inst.E0
+    assert energy.energy(inst, -inst.s_star) == inst.E0
+    assert np.all((inst.loop_lengths >= 4) & (inst.loop_lengths <= 8))
+    m = model.Model(inst).set_beta(2.0)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, 16)
+    assert out["energies"].min() == inst.E0
+
+
+def test_loop_planted_zephyr_shape_energy_of_planted_state():
+    inst = instances.loop_planted(3, 3, 2, 8, seed=0)
+    assert energy.energy(inst, inst.s_star) == inst.E0
+
+
+# ---------------------------------------------------------------- P10-P12: compress
+def _row_problem(seed=3, D=4):
+    inst = instances.lattice(3, 4, 2, 2, p_keep=0.9, seed=seed)
+    m = model.Model(inst).set_beta(0.9)
+    Rex, _ = mps.contract(m, 0, 0)
+    return m, Rex
+
+
+def test_compress_gauge_independent_and_monotone():
+    m, Rex = _row_problem()
+    y = 1
+    pos = mps.row_positions(m, y)
+    A = Rex[y + 1]
+    rng = np.random.default_rng(2)
+    A2 = [a.copy() for a in A]
+    for j in range(len(A) - 1):                       # random invertible gauge on every bond
+        b = A2[j].shape[2]
+        G = rng.normal(size=(b, b)) + 2 * np.eye(b)
+        A2[j] = np.einsum("apb,bc->apc", A2[j], G)
+        A2[j + 1] = np.einsum("ab,bpc->apc", np.linalg.inv(G), A2[j + 1])
+    exact = mpo_dense = mps.mpo_mps_dense(pos, A)
+    exact = exact / np.linalg.norm(exact)
+    fid = {}
+    for sweeps in (0, 1, 2):
+        st = {}
+        N1, l1 = mps.compress(pos, A, 3, sweeps, stats=st)
+        N2, l2 = mps.compress(pos, A2, 3, sweeps)
+        v1, v2 = mps.mps_to_dense(N1), mps.mps_to_dense(N2)
+        assert abs(1 - abs((v1 * v2).sum())) < 1e-10                 # P10
+        assert abs(l1 - l2) < 1e-10
+        fid[sweeps] = abs((v1 * exact).sum())
+        for k in range(0, len(st["pass_norms"][0]), len(pos)):       # P11: norm non-decreasing in a pass
+            nrm = st["pass_norms"][0][k:k + len(pos)]
+            assert all(b >= a * (1 - 1e-12) for a, b in zip(nrm, nrm[1:]))
+    assert fid[1] >= fid[0] - 1e-12 and fid[2] >= fid[1] - 1e-12     # P11: passes do not lower fidelity
+    assert fid[0] < 1 - 1e-9                                         # the cut really truncates
+
+
+def test_compress_large_D_equals_exact():
+    m, Rex = _row_problem()
+    y = 1
+    pos = mps.row_positions(m, y)
+    N0, l0 = mps.compress(pos, Rex[y + 1], 0, 0)
+    N1, l1 = mps.compress(pos, Rex[y + 1], 64, 2)                    # P12
+    v0, v1 = mps.mps_to_dense(N0), mps.mps_to_dense(N1)
+    assert abs(1 - abs((v0 * v1).sum())) < 1e-12 and abs(l0 - l1) < 1e-12
+    ex = mps.mpo_mps_dense(pos, Rex[y + 1])
+    assert abs(1 - abs((v0 * ex).sum()) / np.linalg.norm(ex)) < 1e-12
+    assert abs(l0 - np.log(np.linalg.norm(ex))) < 1e-12
+
+
+def test_truncate_rank_rules():
+    s = np.array([1.0, 0.5, 0.25, 0.25 * (1 - 1e-9), 1e-3, 1e-15, 0.0])
+    assert mps.truncate_rank(s, 0) == 5                 # S6: drops <= 1e-14 sigma_1
+    assert mps.truncate_rank(s, 3) == 2                 # S5: does not split the degenerate pair
+    assert mps.truncate_rank(s, 3, gap_guard=False) == 3
+    assert mps.truncate_rank(s, 4) == 4
+    assert mps.truncate_rank(np.zeros(3), 2) == 1
+
+
+def test_truncated_marginals_close_to_exact():
+    """Truncated D: conditionals still sum to 1 (logp <= 0) and log Z stays within the truncation error."""
+    inst = instances.lattice(3, 3, 2, 4, p_keep=0.95, seed=13)
+    m = model.Model(inst).set_beta(1.0)
+    Rex, lex = mps.contract(m, 0, 0)
+    ex = search.branch_and_bound(m, Rex, lex, 16)
+    st = {}
+    Rt, lt = mps.contract(m, 4, 2, stats=st)
+    tr = search.branch_and_bound(m, Rt, lt, 16)
+    assert abs(tr["log_z"] - ex["log_z"]) < 1e-3 * abs(ex["log_z"])
+    assert tr["energies"].min() == ex["energies"].min()
+    assert max(st["min_sigma"]) < 1.0
