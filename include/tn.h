@@ -1,0 +1,159 @@
+/* tn.h -- C ABI of the B200-native boundary-MPS / branch-and-bound hot path of
+ * arXiv 2411.16431 (Dziubyna et al., "Limitations of tensor-network approaches for
+ * optimization and sampling ...").  Citations are PAPER.md:<line> + section / equation.
+ *
+ * Problem (Eq. (1)):  H(s) = sum_<ij> J_ij s_i s_j + sum_i h_i s_i,  s_i = +-1,
+ * on a quasi-2D graph whose spins are grouped into unit cells on an Ly x Lx grid (Eq. (3),
+ * PAPER.md:69-74, Fig. 1).  The library samples low-energy states from the
+ * Boltzmann distribution p ~ exp(-beta H) (Eq. (6)) by
+ *   (1) tn_set_beta : local Boltzmann tables, projectors and edge matrices (Eqs. (3)-(5)
+ *                     PAPER.md:69-84, Fig. 5(c)),
+ *   (2) tn_contract : boundary-MPS contraction of the sparse PEPS, row after row, bond <= D
+ *                     (zipper + truncated SVD + one-site variational passes,
+ *                     Sec. III B 2 PAPER.md:165-179, Fig. 8; sparse diagrams Fig. 7
+ *                     PAPER.md:155-163),
+ *   (3) tn_branch_and_bound : beam search over cells driven by the conditional probabilities
+ *                     of Fig. 6(b) PAPER.md:143 (Eqs. (7)-(9) PAPER.md:94-107, Fig. 3).
+ *
+ * Conventions
+ *   - every entry point returns a tn_status (0 = TN_OK, < 0 = error); no exception, abort or
+ *     exit crosses this boundary; tn_last_error() gives a thread-local message.
+ *   - pointers marked HOST are host memory, read (inputs) or written (outputs) synchronously;
+ *     inputs are copied at tn_create, the caller keeps ownership of everything it passes in;
+ *     outputs are caller-allocated with the stated capacity.
+ *   - a handle owns all its device memory; it is single-threaded; distinct handles are
+ *     independent.  All work is queued on the stream given by tn_set_stream (default: the
+ *     legacy default stream) and calls return after the stream has been synchronised
+ *     (tn_contract / tn_branch_and_bound need host-side control flow anyway).
+ *   - there is NO CPU fallback: without a CUDA device every compute call returns TN_ERR_CUDA.
+ *   - call order: tn_create -> tn_set_beta -> tn_contract -> tn_log_z / tn_branch_and_bound;
+ *     a call made too early returns TN_ERR_STATE.  tn_set_beta drops the boundary MPS.
+ *
+ * Geometry accepted by tn_create (BASELINE.json "Pegasus-/Zephyr-shaped" synthetic lattices):
+ *   a cell is a chain of S = subs_per_cell (1..3) sub-clusters of n_s = spins_per_sub spins
+ *   (n_s even, 2..8); lo = positions [0, n_s/2), hi = [n_s/2, n_s).  Allowed edges:
+ *     inside a sub-cluster: any pair;   sub s hi -- sub s+1 lo  (same cell);
+ *     horizontal (x,y)-(x+1,y): sub 0 -- sub 0;  vertical (x,y)-(x,y+1): sub v -- sub v with
+ *     v = min(1, S-1);  diagonal (x,y)-(x+1,y+1) (S == 3 only): sub 2 lo -- sub 2 hi.
+ *   Anything else (e.g. a real D-Wave working graph) returns TN_ERR_GEOMETRY.
+ */
+#ifndef TN_B200_H
+#define TN_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tn_handle tn_handle; /* opaque */
+
+typedef enum {
+  TN_OK = 0,
+  TN_ERR_ARG = -1,      /* NULL / out-of-range argument                         */
+  TN_ERR_GEOMETRY = -2, /* edge or cluster map outside the accepted geometry     */
+  TN_ERR_STATE = -3,    /* call order violated                                   */
+  TN_ERR_CUDA = -4,     /* CUDA runtime error or no device                       */
+  TN_ERR_OOM = -5,      /* device allocation failed                              */
+  TN_ERR_NUMERIC = -6   /* NaN / Inf / non-convergence detected                  */
+} tn_status;
+
+/* option keys for tn_set_option */
+enum {
+  TN_OPT_GAP_GUARD = 1,   /* 1 (default) / 0: never cut between singular values closer than 1e-6
+                             relative (reading S5)                                   */
+  TN_OPT_SVD_TOL = 2,     /* residual tolerance of the truncated SVD relative to sigma_1
+                             (default 1e-11; reading S1)            */
+  TN_OPT_SVD_MAXIT = 3,   /* max block-subspace iterations per zipper step (default 40)       */
+  TN_OPT_OVERSAMPLE = 4,  /* extra block columns of the subspace iteration (default 16)       */
+  TN_OPT_EXACT_CAP = 5    /* largest bond allowed when D <= 0 (default 512)                   */
+};
+
+/* Counters and timers filled by tn_get_stats (all since the last tn_set_beta). */
+typedef struct {
+  double ms_tables;          /* a1: local tables kernel                                     */
+  double ms_contract;        /* a2-a4(i): whole tn_contract                                  */
+  double ms_theta_build;     /*   Theta-core builds (gather + batched DxDxD + weights)       */
+  double ms_theta_apply;     /*   Theta x skinny / Theta^T x skinny DMMA GEMMs               */
+  double ms_orth_svd;        /*   orthonormalisation + Jacobi SVD                            */
+  double ms_search;          /* a4(ii)-a5: whole tn_branch_and_bound                         */
+  double ms_search_rblocks;  /*   right blocks at row starts                                 */
+  double ms_search_cond;     /*   conditional-probability GEMM + scores                      */
+  double ms_search_select;   /*   top-M radix selection                                      */
+  double flop_theta_build;   /* algorithmic FLOP of the builds                              */
+  double flop_theta_apply;   /* algorithmic FLOP of the skinny GEMMs                        */
+  double bytes_theta_apply;  /* algorithmic bytes of the skinny GEMMs (one read of Theta)    */
+  double flop_search;        /* algorithmic FLOP of the search GEMMs                        */
+  double min_sigma_rel;      /* max over bonds of (smallest retained sigma / sigma_1), Fig. 12(b)
+                                PAPER.md:306                                                 */
+  int64_t svd_iterations;    /* total block-subspace iterations                             */
+  int64_t kernel_launches;   /* kernels launched by this library                            */
+  int64_t negative_u;        /* conditionals clamped to 0 (reading S7)         */
+  int64_t rows_contracted;   /* boundary-MPS rows built                                      */
+  int64_t bytes_device;      /* device bytes currently held                                  */
+} tn_stats;
+
+/* tn_create: validates the geometry and copies the instance to the device.
+ *   n_spins, n_edges; edge_u/edge_v/J HOST [n_edges] (Eq. (1)); h HOST [n_spins] or NULL (= 0);
+ *   Ly, Lx: cell grid (y = row, 0 = top; x = column, 0 = left);
+ *   cell_y/cell_x/sub/pos HOST [n_spins]: cluster map (cell, sub-cluster in the cell, bit position
+ *   in the sub-cluster; each (cell, sub, pos) slot holds exactly one spin; Eq. (3)).
+ * Errors: TN_ERR_ARG, TN_ERR_GEOMETRY (message names the offending edge), TN_ERR_CUDA, TN_ERR_OOM. */
+int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges,
+              const int32_t* edge_u, const int32_t* edge_v, const double* J, const double* h,
+              int32_t Ly, int32_t Lx, int32_t subs_per_cell, int32_t spins_per_sub,
+              const int32_t* cell_y, const int32_t* cell_x, const int32_t* sub, const int32_t* pos);
+
+/* tn_set_stream: cudaStream_t to launch on (borrowed; NULL = default stream). */
+int tn_set_stream(tn_handle*, void* cuda_stream);
+
+/* tn_set_allocator: device allocator callbacks (e.g. torch's caching allocator); must be set
+ * before tn_set_beta; alloc returns NULL on failure; NULL callbacks restore cudaMalloc/cudaFree. */
+int tn_set_allocator(tn_handle*, void* (*alloc)(size_t bytes, void* ctx),
+                     void (*free_)(void* ptr, void* ctx), void* ctx);
+
+int tn_set_option(tn_handle*, int32_t key, double value);
+
+/* tn_set_beta (a1): Boltzmann weights exp(-beta (E - min E)) of every sub-cluster and
+ * inter-sub-cluster table, projector index tables (Eq. (5)), edge matrices
+ * exp(-beta (Ebar - min)) (Eq. (4), Fig. 5(c)).  Drops boundary MPS. */
+int tn_set_beta(tn_handle*, double beta);
+
+/* tn_contract (a2-a4): boundary MPS R_y for y = Ly-1 .. 1 with bond <= D, `sweeps` one-site
+ * variational passes after each zipper.  D <= 0: no truncation (exact;
+ * TN_ERR_ARG if a bond would exceed TN_OPT_EXACT_CAP), sweeps ignored. */
+int tn_contract(tn_handle*, int32_t D, int32_t sweeps);
+
+/* tn_log_z: log Z (Eq. (10)) from the contraction + the first cell's normaliser. */
+int tn_log_z(tn_handle*, double* log_z /* HOST */);
+
+/* tn_row_lognorm: log of the norm removed from R_y (y in 1..Ly-1), for row-wise parity. */
+int tn_row_lognorm(tn_handle*, int32_t y, double* lognorm /* HOST */);
+
+/* tn_mps_shape / tn_mps_tensor: copy boundary-MPS tensor `j` of R_y to the host, layout
+ * [left bond][physical][right bond] row-major (padding directions are exactly zero). */
+int tn_mps_shape(tn_handle*, int32_t y, int32_t j, int32_t* n_pos, int32_t* dl, int32_t* p, int32_t* dr);
+int tn_mps_tensor(tn_handle*, int32_t y, int32_t j, double* out /* HOST dl*p*dr */);
+
+/* tn_branch_and_bound (a4(ii)-a5): beam of width M over cells in row-major order (Fig. 3
+ * PAPER.md:125).  Outputs (HOST, caller-allocated): *n_out <= M states; states [M][n_spins] int8
+ * +-1 in spin-id order; energies [M] recomputed from J, h in input order (one running fp64
+ * sum: edges first, then fields); logp [M] descending; *log_p_discarded = log of the largest
+ * discarded probability p_d (-inf if nothing was discarded; may be NULL).
+ * Ties: logp desc, then parent rank asc, then cell state asc (reading S8). */
+int tn_branch_and_bound(tn_handle*, int32_t M, int32_t* n_out, int8_t* states, double* energies,
+                        double* logp, double* log_p_discarded);
+
+int tn_get_stats(tn_handle*, tn_stats* out /* HOST */);
+
+/* tn_energy: O-0 fixed-order energies of n given states (HOST int8 [n][n_spins]) on the device. */
+int tn_energy(tn_handle*, int32_t n, const int8_t* states, double* energies /* HOST [n] */);
+
+const char* tn_last_error(void);
+void tn_destroy(tn_handle*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TN_B200_H */

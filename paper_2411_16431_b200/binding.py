@@ -1,0 +1,242 @@
+"""ctypes binding of libtn_b200.so: same names and argument order as include/tn.h."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
+
+EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
+                    "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
+                    "tn_get_stats", "tn_energy", "tn_last_error", "tn_destroy"]
+OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP = 1, 2, 3, 4, 5
+
+
+class TnError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("tn error %d: %s" % (code, msg))
+        self.code = code
+
+
+class TnStats(C.Structure):
+    _fields_ = [(n, C.c_double) for n in (
+        "ms_tables", "ms_contract", "ms_theta_build", "ms_theta_apply", "ms_orth_svd", "ms_search",
+        "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
+        "bytes_theta_apply", "flop_search", "min_sigma_rel")] + [(n, C.c_int64) for n in (
+            "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device")]
+
+    def asdict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+def lib():
+    """Loads the shared library (building it is `python -m paper_2411_16431_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError("libtn_b200.so is missing: run `python -m paper_2411_16431_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        p_i32, p_f64, p_i8 = C.POINTER(C.c_int32), C.POINTER(C.c_double), C.POINTER(C.c_int8)
+        L.tn_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_int64, p_i32, p_i32, p_f64, p_f64, C.c_int32,
+                                C.c_int32, C.c_int32, C.c_int32, p_i32, p_i32, p_i32, p_i32]
+        L.tn_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+        L.tn_set_allocator.argtypes = [C.c_void_p, ALLOC_FN, FREE_FN, C.c_void_p]
+        L.tn_set_option.argtypes = [C.c_void_p, C.c_int32, C.c_double]
+        L.tn_set_beta.argtypes = [C.c_void_p, C.c_double]
+        L.tn_contract.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.tn_log_z.argtypes = [C.c_void_p, p_f64]
+        L.tn_row_lognorm.argtypes = [C.c_void_p, C.c_int32, p_f64]
+        L.tn_mps_shape.argtypes = [C.c_void_p, C.c_int32, C.c_int32, p_i32, p_i32, p_i32, p_i32]
+        L.tn_mps_tensor.argtypes = [C.c_void_p, C.c_int32, C.c_int32, p_f64]
+        L.tn_branch_and_bound.argtypes = [C.c_void_p, C.c_int32, p_i32, p_i8, p_f64, p_f64, p_f64]
+        L.tn_get_stats.argtypes = [C.c_void_p, C.POINTER(TnStats)]
+        L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
+        L.tn_last_error.restype = C.c_char_p
+        L.tn_destroy.argtypes = [C.c_void_p]
+        L.tn_destroy.restype = None
+        for n in EXPORTED_SYMBOLS:
+            if n not in ("tn_last_error", "tn_destroy"):
+                getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def tn_last_error() -> str:
+    return lib().tn_last_error().decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise TnError(rc, tn_last_error())
+
+
+def _ptr(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+def tn_create(n_spins, edge_u, edge_v, J, h, Ly, Lx, subs_per_cell, spins_per_sub, cell_y, cell_x, sub, pos):
+    eu = np.ascontiguousarray(edge_u, dtype=np.int32)
+    ev = np.ascontiguousarray(edge_v, dtype=np.int32)
+    Jv = np.ascontiguousarray(J, dtype=np.float64)
+    hv = None if h is None else np.ascontiguousarray(h, dtype=np.float64)
+    cy, cx, sb, ps = (np.ascontiguousarray(a, dtype=np.int32) for a in (cell_y, cell_x, sub, pos))
+    out = C.c_void_p()
+    _check(lib().tn_create(C.byref(out), int(n_spins), int(eu.size), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32),
+                           _ptr(Jv, C.c_double), None if hv is None else _ptr(hv, C.c_double), int(Ly), int(Lx),
+                           int(subs_per_cell), int(spins_per_sub), _ptr(cy, C.c_int32), _ptr(cx, C.c_int32),
+                           _ptr(sb, C.c_int32), _ptr(ps, C.c_int32)))
+    return out
+
+
+def tn_set_stream(handle, cuda_stream):
+    _check(lib().tn_set_stream(handle, C.c_void_p(cuda_stream)))
+
+
+def tn_set_allocator(handle, alloc, free_, ctx=None):
+    _check(lib().tn_set_allocator(handle, alloc, free_, ctx))
+
+
+def tn_set_option(handle, key, value):
+    _check(lib().tn_set_option(handle, int(key), float(value)))
+
+
+def tn_set_beta(handle, beta):
+    _check(lib().tn_set_beta(handle, float(beta)))
+
+
+def tn_contract(handle, D, sweeps):
+    _check(lib().tn_contract(handle, int(D), int(sweeps)))
+
+
+def tn_log_z(handle) -> float:
+    v = C.c_double()
+    _check(lib().tn_log_z(handle, C.byref(v)))
+    return v.value
+
+
+def tn_row_lognorm(handle, y) -> float:
+    v = C.c_double()
+    _check(lib().tn_row_lognorm(handle, int(y), C.byref(v)))
+    return v.value
+
+
+def tn_mps_shape(handle, y, j):
+    n, dl, p, dr = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
+    _check(lib().tn_mps_shape(handle, int(y), int(j), C.byref(n), C.byref(dl), C.byref(p), C.byref(dr)))
+    return n.value, dl.value, p.value, dr.value
+
+
+def tn_mps_tensor(handle, y, j):
+    _, dl, p, dr = tn_mps_shape(handle, y, j)
+    out = np.empty((dl, p, dr), dtype=np.float64)
+    _check(lib().tn_mps_tensor(handle, int(y), int(j), _ptr(out, C.c_double)))
+    return out
+
+
+def tn_branch_and_bound(handle, M, n_spins):
+    """Returns (states [n, n_spins] int8, energies [n], logp [n], log_p_discarded)."""
+    states = np.empty((M, n_spins), dtype=np.int8)
+    energies = np.empty(M, dtype=np.float64)
+    logp = np.empty(M, dtype=np.float64)
+    n = C.c_int32()
+    pd = C.c_double()
+    _check(lib().tn_branch_and_bound(handle, int(M), C.byref(n), _ptr(states, C.c_int8), _ptr(energies, C.c_double),
+                                     _ptr(logp, C.c_double), C.byref(pd)))
+    k = n.value
+    return states[:k], energies[:k], logp[:k], pd.value
+
+
+def tn_energy(handle, states):
+    s = np.ascontiguousarray(states, dtype=np.int8)
+    if s.ndim == 1:
+        s = s[None, :]
+    out = np.empty(s.shape[0], dtype=np.float64)
+    _check(lib().tn_energy(handle, s.shape[0], _ptr(s, C.c_int8), _ptr(out, C.c_double)))
+    return out
+
+
+def tn_get_stats(handle) -> dict:
+    st = TnStats()
+    _check(lib().tn_get_stats(handle, C.byref(st)))
+    return st.asdict()
+
+
+def tn_destroy(handle):
+    lib().tn_destroy(handle)
+
+
+class TensorNetwork:
+    """Convenience owner of a tn_handle for an `instances.Instance`-like object (attributes n_spins,
+    edge_u, edge_v, J, h, Ly, Lx, S, n_s, cell_y, cell_x, sub, pos).  Uses torch's caching allocator
+    and current stream when torch sees a CUDA device."""
+
+    def __init__(self, inst, use_torch: bool = True):
+        self.n_spins = int(inst.n_spins)
+        self.handle = tn_create(inst.n_spins, inst.edge_u, inst.edge_v, inst.J, inst.h, inst.Ly, inst.Lx, inst.S,
+                                inst.n_s, inst.cell_y, inst.cell_x, inst.sub, inst.pos)
+        self._cb = None
+        if use_torch:
+            try:
+                import torch
+                if torch.cuda.is_available():
+                    alloc = ALLOC_FN(lambda n, ctx: torch.cuda.caching_allocator_alloc(n))
+                    free_ = FREE_FN(lambda p, ctx: torch.cuda.caching_allocator_delete(p))
+                    self._cb = (alloc, free_)
+                    tn_set_allocator(self.handle, alloc, free_)
+                    tn_set_stream(self.handle, torch.cuda.current_stream().cuda_stream)
+            except ImportError:
+                pass
+
+    def set_option(self, key, value):
+        tn_set_option(self.handle, key, value)
+
+    def set_beta(self, beta):
+        tn_set_beta(self.handle, beta)
+
+    def contract(self, D, sweeps):
+        tn_contract(self.handle, D, sweeps)
+
+    def log_z(self):
+        return tn_log_z(self.handle)
+
+    def row_lognorm(self, y):
+        return tn_row_lognorm(self.handle, y)
+
+    def mps(self, y):
+        n = tn_mps_shape(self.handle, y, 0)[0]
+        return [tn_mps_tensor(self.handle, y, j) for j in range(n)]
+
+    def branch_and_bound(self, M):
+        return tn_branch_and_bound(self.handle, M, self.n_spins)
+
+    def energy(self, states):
+        return tn_energy(self.handle, states)
+
+    def stats(self):
+        return tn_get_stats(self.handle)
+
+    def close(self):
+        if self.handle is not None:
+            tn_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

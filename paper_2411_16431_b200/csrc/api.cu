@@ -1,0 +1,341 @@
+// C ABI of libtn_b200.so (include/tn.h).  No exception crosses this file's extern "C" functions.
+#include "kernels.cuh"
+#include <cstdarg>
+#include <algorithm>
+
+static thread_local std::string g_last_error;
+
+[[noreturn]] void tn_throw(int code, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  throw TnError{code, buf};
+}
+
+// ---- device memory: allocator callbacks + a size-bucketed free list (all use is stream-ordered) ----
+static void* raw_alloc(tn_handle* h, size_t bytes, int* src) {
+  void* p = nullptr;
+  if (h->alloc_cb) {
+    p = h->alloc_cb(bytes, h->alloc_ctx);
+    if (!p) tn_throw(TN_ERR_OOM, "allocator callback failed for %zu bytes", bytes);
+    *src = 1;
+  } else {
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      tn_throw(e == cudaErrorMemoryAllocation ? TN_ERR_OOM : TN_ERR_CUDA, "cudaMalloc(%zu): %s", bytes,
+               cudaGetErrorString(e));
+    }
+    *src = 0;
+  }
+  return p;
+}
+static void raw_free(tn_handle* h, const tn_handle::Block& b) {
+  if (b.src == 1 && h->free_cb) h->free_cb(b.p, h->alloc_ctx);
+  else if (b.src == 0) cudaFree(b.p);
+}
+static void trim_free_list(tn_handle* h) {
+  if (h->cached.empty()) return;
+  cudaStreamSynchronize(h->stream);
+  for (auto& b : h->cached) { raw_free(h, b); h->bytes_held -= (i64)b.bytes; }
+  h->cached.clear();
+}
+
+void* tn_handle::dmalloc(size_t bytes) {
+  bytes = (bytes + 255) & ~(size_t)255;
+  auto& fl = cached;
+  int best = -1;
+  for (int i = 0; i < (int)fl.size(); i++)
+    if (fl[i].bytes >= bytes && fl[i].bytes <= 2 * bytes + 4096 && (best < 0 || fl[i].bytes < fl[best].bytes)) best = i;
+  Block blk;
+  if (best >= 0) {
+    blk = fl[best];
+    fl.erase(fl.begin() + best);
+  } else {
+    try {
+      blk.p = raw_alloc(this, bytes, &blk.src);
+    } catch (TnError&) {
+      trim_free_list(this);
+      blk.p = raw_alloc(this, bytes, &blk.src);
+    }
+    blk.bytes = bytes;
+    bytes_held += (i64)bytes;
+  }
+  live.push_back(blk);
+  return blk.p;
+}
+void tn_handle::dfree(void* p) {
+  if (!p) return;
+  for (size_t i = live.size(); i-- > 0;)
+    if (live[i].p == p) {
+      cached.push_back(live[i]);
+      live[i] = live.back();
+      live.pop_back();
+      return;
+    }
+}
+
+StageTimer::StageTimer(tn_handle* h_, double* dst_) : h(h_), dst(dst_) {
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  cudaEventRecord(a, h->stream);
+}
+StageTimer::~StageTimer() {
+  cudaEventRecord(b, h->stream);
+  cudaEventSynchronize(b);
+  float ms = 0;
+  if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) *dst += ms;
+  cudaEventDestroy(a); cudaEventDestroy(b);
+}
+
+#define TN_API_BEGIN try {
+#define TN_API_END                                                     \
+  return TN_OK;                                                        \
+  }                                                                    \
+  catch (const TnError& e) { g_last_error = e.msg; return e.code; }    \
+  catch (const std::bad_alloc&) { g_last_error = "host out of memory"; return TN_ERR_OOM; } \
+  catch (const std::exception& e) { g_last_error = e.what(); return TN_ERR_ARG; }            \
+  catch (...) { g_last_error = "unknown error"; return TN_ERR_ARG; }
+
+static void need_device() {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n == 0) {
+    cudaGetLastError();
+    tn_throw(TN_ERR_CUDA, "no CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+  }
+}
+
+extern "C" {
+
+const char* tn_last_error(void) { return g_last_error.c_str(); }
+
+int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges, const int32_t* edge_u, const int32_t* edge_v,
+              const double* J, const double* hfield, int32_t Ly, int32_t Lx, int32_t S, int32_t ns,
+              const int32_t* cell_y, const int32_t* cell_x, const int32_t* sub, const int32_t* pos) {
+  tn_handle* h = nullptr;
+  try {
+    if (!out) tn_throw(TN_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (n_spins <= 0 || n_edges < 0 || Ly <= 0 || Lx <= 0) tn_throw(TN_ERR_ARG, "non-positive size");
+    if ((n_edges > 0 && (!edge_u || !edge_v || !J)) || !cell_y || !cell_x || !sub || !pos)
+      tn_throw(TN_ERR_ARG, "NULL input array");
+    if (S < 1 || S > 3 || ns < 2 || ns > 8 || (ns & 1))
+      tn_throw(TN_ERR_GEOMETRY, "subs_per_cell must be 1..3 and spins_per_sub even in 2..8 (got %d, %d)", S, ns);
+    if ((i64)n_spins != (i64)Ly * Lx * S * ns)
+      tn_throw(TN_ERR_GEOMETRY, "n_spins = %d but the cluster map has Ly*Lx*S*n_s = %lld slots", n_spins,
+               (long long)Ly * Lx * S * ns);
+    need_device();
+    h = new tn_handle();
+    memset(&h->st, 0, sizeof(h->st));
+    h->n_spins = n_spins; h->n_edges = n_edges; h->Ly = Ly; h->Lx = Lx; h->S = S; h->ns = ns;
+    h->edge_u.assign(edge_u, edge_u + n_edges);
+    h->edge_v.assign(edge_v, edge_v + n_edges);
+    h->J.assign(J, J + n_edges);
+    h->h.assign(n_spins, 0.0);
+    if (hfield) h->h.assign(hfield, hfield + n_spins);
+    h->cell_of.resize(n_spins); h->bit_of.resize(n_spins);
+    std::vector<char> used((size_t)n_spins, 0);
+    for (int i = 0; i < n_spins; i++) {
+      if (cell_y[i] < 0 || cell_y[i] >= Ly || cell_x[i] < 0 || cell_x[i] >= Lx || sub[i] < 0 || sub[i] >= S ||
+          pos[i] < 0 || pos[i] >= ns)
+        tn_throw(TN_ERR_GEOMETRY, "spin %d: cluster map entry out of range", i);
+      h->cell_of[i] = cell_y[i] * Lx + cell_x[i];
+      h->bit_of[i] = sub[i] * ns + pos[i];
+      size_t slot = (size_t)h->cell_of[i] * S * ns + h->bit_of[i];
+      if (used[slot]) tn_throw(TN_ERR_GEOMETRY, "spin %d: (cell, sub, pos) slot already taken", i);
+      used[slot] = 1;
+    }
+    for (i64 e = 0; e < n_edges; e++) {
+      if (edge_u[e] < 0 || edge_u[e] >= n_spins || edge_v[e] < 0 || edge_v[e] >= n_spins)
+        tn_throw(TN_ERR_ARG, "edge %lld: spin index out of range", (long long)e);
+      if (!std::isfinite(J[e])) tn_throw(TN_ERR_ARG, "edge %lld: J is not finite", (long long)e);
+    }
+    tables_create(h);
+    h->d_eu = h->dalloc<int>(n_edges + 1); h->d_ev = h->dalloc<int>(n_edges + 1);
+    h->d_J = h->dalloc<double>(n_edges + 1); h->d_h = h->dalloc<double>(n_spins);
+    h->d_cell_of = h->dalloc<int>(n_spins); h->d_bit_of = h->dalloc<int>(n_spins);
+    if (n_edges) {
+      TN_CUDA(cudaMemcpy(h->d_eu, h->edge_u.data(), sizeof(int) * n_edges, cudaMemcpyHostToDevice));
+      TN_CUDA(cudaMemcpy(h->d_ev, h->edge_v.data(), sizeof(int) * n_edges, cudaMemcpyHostToDevice));
+      TN_CUDA(cudaMemcpy(h->d_J, h->J.data(), sizeof(double) * n_edges, cudaMemcpyHostToDevice));
+    }
+    TN_CUDA(cudaMemcpy(h->d_h, h->h.data(), sizeof(double) * n_spins, cudaMemcpyHostToDevice));
+    TN_CUDA(cudaMemcpy(h->d_cell_of, h->cell_of.data(), sizeof(int) * n_spins, cudaMemcpyHostToDevice));
+    TN_CUDA(cudaMemcpy(h->d_bit_of, h->bit_of.data(), sizeof(int) * n_spins, cudaMemcpyHostToDevice));
+    *out = h;
+    return TN_OK;
+  } catch (const TnError& e) {
+    g_last_error = e.msg;
+    if (h) tn_destroy(h);
+    return e.code;
+  } catch (const std::exception& e) {
+    g_last_error = e.what();
+    if (h) tn_destroy(h);
+    return TN_ERR_ARG;
+  }
+}
+
+int tn_set_stream(tn_handle* h, void* s) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  h->stream = (cudaStream_t)s;
+  TN_API_END
+}
+
+int tn_set_allocator(tn_handle* h, void* (*alloc)(size_t, void*), void (*free_)(void*, void*), void* ctx) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  if ((alloc == nullptr) != (free_ == nullptr)) tn_throw(TN_ERR_ARG, "alloc and free must both be set or both NULL");
+  if (h->have_beta) tn_throw(TN_ERR_STATE, "tn_set_allocator must precede tn_set_beta");
+  if (h->alloc_cb && (h->alloc_cb != alloc || h->alloc_ctx != ctx))
+    tn_throw(TN_ERR_STATE, "allocator callbacks can be set only once per handle");
+  trim_free_list(h);   // blocks already handed out keep the origin they were allocated with
+  h->alloc_cb = alloc; h->free_cb = free_; h->alloc_ctx = ctx;
+  TN_API_END
+}
+
+int tn_set_option(tn_handle* h, int32_t key, double v) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  switch (key) {
+    case TN_OPT_GAP_GUARD: h->gap_guard = v != 0.0; break;
+    case TN_OPT_SVD_TOL:
+      if (!(v > 0.0)) tn_throw(TN_ERR_ARG, "svd tol must be > 0");
+      h->svd_tol = v; break;
+    case TN_OPT_SVD_MAXIT:
+      if (v < 1) tn_throw(TN_ERR_ARG, "maxit must be >= 1");
+      h->svd_maxit = (int)v; break;
+    case TN_OPT_OVERSAMPLE:
+      if (v < 0 || v > 256) tn_throw(TN_ERR_ARG, "oversample out of range");
+      h->oversample = (int)v; break;
+    case TN_OPT_EXACT_CAP:
+      if (v < 1 || v > 1024) tn_throw(TN_ERR_ARG, "exact cap must be in 1..1024");
+      h->exact_cap = (int)v; break;
+    default: tn_throw(TN_ERR_ARG, "unknown option key %d", key);
+  }
+  TN_API_END
+}
+
+int tn_set_beta(tn_handle* h, double beta) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  if (!std::isfinite(beta) || beta < 0.0) tn_throw(TN_ERR_ARG, "beta must be finite and >= 0");
+  mps_free(h);
+  memset(&h->st, 0, sizeof(h->st));
+  tables_set_beta(h, beta);
+  h->have_beta = true;
+  TN_API_END
+}
+
+int tn_contract(tn_handle* h, int32_t D, int32_t sweeps) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  if (!h->have_beta) tn_throw(TN_ERR_STATE, "tn_contract before tn_set_beta");
+  if (sweeps < 0) tn_throw(TN_ERR_ARG, "sweeps < 0");
+  if (D > 1008) tn_throw(TN_ERR_ARG, "D > 1008 not supported");
+  try {
+    contract_run(h, D, sweeps);
+  } catch (...) {
+    mps_free(h);
+    trim_free_list(h);
+    throw;
+  }
+  trim_free_list(h);
+  search_logz(h);
+  trim_free_list(h);
+  TN_API_END
+}
+
+int tn_log_z(tn_handle* h, double* log_z) {
+  TN_API_BEGIN
+  if (!h || !log_z) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (!h->have_mps || !h->have_logz) tn_throw(TN_ERR_STATE, "tn_log_z before tn_contract");
+  *log_z = h->log_z;
+  TN_API_END
+}
+
+int tn_row_lognorm(tn_handle* h, int32_t y, double* lognorm) {
+  TN_API_BEGIN
+  if (!h || !lognorm) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_row_lognorm before tn_contract");
+  if (y < 1 || y > h->Ly) tn_throw(TN_ERR_ARG, "row out of range");
+  *lognorm = h->lognorm[y];
+  TN_API_END
+}
+
+int tn_mps_shape(tn_handle* h, int32_t y, int32_t j, int32_t* n_pos, int32_t* dl, int32_t* p, int32_t* dr) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_mps_shape before tn_contract");
+  if (y < 1 || y > h->Ly || j < 0 || j >= (int)h->rows[y].size()) tn_throw(TN_ERR_ARG, "index out of range");
+  const MpsTensor& t = h->rows[y][j];
+  if (n_pos) *n_pos = (int)h->rows[y].size();
+  if (dl) *dl = t.dl;
+  if (p) *p = t.p;
+  if (dr) *dr = t.dr;
+  TN_API_END
+}
+
+int tn_mps_tensor(tn_handle* h, int32_t y, int32_t j, double* out) {
+  TN_API_BEGIN
+  if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_mps_tensor before tn_contract");
+  if (y < 1 || y > h->Ly || j < 0 || j >= (int)h->rows[y].size()) tn_throw(TN_ERR_ARG, "index out of range");
+  const MpsTensor& t = h->rows[y][j];
+  TN_CUDA(cudaMemcpyAsync(out, t.d, sizeof(double) * t.dl * t.p * t.dr, cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+  TN_API_END
+}
+
+int tn_branch_and_bound(tn_handle* h, int32_t M, int32_t* n_out, int8_t* states, double* energies, double* logp,
+                        double* log_pd) {
+  TN_API_BEGIN
+  if (!h || !n_out || !states || !energies || !logp) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (M < 1 || M > (1 << 20)) tn_throw(TN_ERR_ARG, "M must be in 1..2^20");
+  if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_branch_and_bound before tn_contract");
+  try {
+    search_run(h, M, n_out, states, energies, logp, log_pd);
+  } catch (...) {
+    trim_free_list(h);
+    throw;
+  }
+  trim_free_list(h);
+  TN_API_END
+}
+
+int tn_energy(tn_handle* h, int32_t n, const int8_t* states, double* energies) {
+  TN_API_BEGIN
+  if (!h || !states || !energies || n < 0) tn_throw(TN_ERR_ARG, "bad argument");
+  energy_run(h, n, states, energies);
+  trim_free_list(h);
+  TN_API_END
+}
+
+int tn_get_stats(tn_handle* h, tn_stats* out) {
+  TN_API_BEGIN
+  if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");
+  *out = h->st;
+  out->bytes_device = h->bytes_held;
+  TN_API_END
+}
+
+void tn_destroy(tn_handle* h) {
+  if (!h) return;
+  try {
+    cudaStreamSynchronize(h->stream);
+    mps_free(h);
+    tables_destroy(h);
+    for (void* p : {(void*)h->d_eu, (void*)h->d_ev, (void*)h->d_J, (void*)h->d_h, (void*)h->d_cell_of,
+                    (void*)h->d_bit_of})
+      if (p) h->dfree(p);
+    trim_free_list(h);
+    for (auto& l : h->live) raw_free(h, l);
+    h->live.clear();
+  } catch (...) {
+  }
+  delete h;
+}
+
+}  // extern "C"

@@ -1,0 +1,500 @@
+// a2-a4(i): boundary-MPS contraction.  PAPER.md:137 (row after row), Sec. III B 1 + Fig. 7
+// (sparse diagrams), Sec. III B 2 + Fig. 8 PAPER.md:165-179 (zipper from a left-canonical MPS with the
+// trivial connector, truncated SVD keeping chi values, one-site variational passes).
+//
+// Every chain position j exposes its "dashed box" Theta_j (Fig. 8(c)) as an implicit operator
+//     Theta = Lmap^T . Tc . Umap          rows (outer bond, MPO bond), columns (upper physical leg, new bond)
+// where Tc is the only large object (state-indexed, built once per position by theta_core / the
+// mediating GEMMs) and Lmap / Umap are cheap maps on the skinny side (projector gathers, c_hi fold,
+// edge matrices Bh / Bv).  Zipper SVD, variational update and environment update are then all
+// "Tc x skinny" / "Tc^T x skinny" DMMA GEMMs.
+#include "kernels.cuh"
+#include <algorithm>
+
+namespace {
+
+struct PosInfo {
+  int kind;   // 0 site, 1 mediating
+  int x;
+  int wl, wr, pu, pd;
+  bool fold;          // site of a lattice without mediating tensors: Bh folded into the left leg
+  const CellDev* c;   // site: its cell; med: the left cell
+  const CellDev* cr;  // med: the right cell
+};
+
+struct ThetaOp {
+  const PosInfo* pos = nullptr;
+  bool left = false;   // false: built from the right environment; true: from the left one
+  int dx = 1, g = 1;   // outer old bond on Theta's rows; new bond inside Theta's columns
+  i64 m = 0, n = 0, mk = 0, nk = 0;
+  double* Tc = nullptr;
+};
+
+struct EvPair { cudaEvent_t a, b; double* dst; };
+
+struct Ctx {
+  tn_handle* h;
+  int* d_keep = nullptr;      // device: number of singular values kept at the current bond
+  int* d_flag = nullptr;      // device: convergence flag
+  double* d_stat = nullptr;   // device: [0] running max of (smallest retained sigma / sigma_1)
+  double* d_scal = nullptr;   // device scratch scalars
+  std::vector<EvPair> evs;
+  uint64_t seed = 1;
+  void tic(double* dst) {
+    EvPair e; e.dst = dst;
+    cudaEventCreate(&e.a); cudaEventCreate(&e.b);
+    cudaEventRecord(e.a, h->stream);
+    evs.push_back(e);
+  }
+  void toc() { cudaEventRecord(evs.back().b, h->stream); }
+  void flush() {
+    cudaStreamSynchronize(h->stream);
+    for (auto& e : evs) {
+      float ms = 0;
+      if (cudaEventElapsedTime(&ms, e.a, e.b) == cudaSuccess) *e.dst += ms;
+      cudaEventDestroy(e.a); cudaEventDestroy(e.b);
+    }
+    evs.clear();
+  }
+};
+
+std::vector<PosInfo> row_positions(tn_handle* h, int y) {
+  std::vector<PosInfo> pos;
+  for (int x = 0; x < h->Lx; x++) {
+    const CellDev& c = h->cell(y, x);
+    PosInfo s;
+    s.kind = 0; s.x = x; s.c = &c; s.cr = nullptr;
+    s.fold = !h->has_med();
+    s.wl = s.fold ? c.bh_rows : c.n_l * c.n_i;
+    s.wr = c.n_r * c.n_o;
+    s.pu = c.bv_rows;
+    s.pd = c.n_d;
+    pos.push_back(s);
+    if (h->has_med() && x + 1 < h->Lx) {
+      const CellDev& cr = h->cell(y, x + 1);
+      PosInfo m;
+      m.kind = 1; m.x = x; m.c = &c; m.cr = &cr; m.fold = false;
+      m.wl = c.n_r * c.n_o;
+      m.wr = cr.n_l * cr.n_i;
+      m.pu = cr.bd_rows;
+      m.pd = c.n_o;
+      pos.push_back(m);
+    }
+  }
+  return pos;
+}
+
+// ---- skinny GEMMs on Tc ----------------------------------------------------------------------
+void tc_apply_N(Ctx& cx, const ThetaOp& op, const double* X, double* Y, int s) {   // Y[mk x s] = Tc X[nk x s]
+  cx.tic(&cx.h->st.ms_theta_apply);
+  gemm_rm(cx.h, false, false, (int)op.mk, s, (int)op.nk, op.Tc, (int)op.nk, X, s, Y, s);
+  cx.toc();
+  cx.h->st.flop_theta_apply += 2.0 * op.mk * op.nk * s;
+  cx.h->st.bytes_theta_apply += 8.0 * op.mk * op.nk;
+}
+void tc_apply_T(Ctx& cx, const ThetaOp& op, const double* Y, double* Z, int s) {   // Z[nk x s] = Tc^T Y[mk x s]
+  cx.tic(&cx.h->st.ms_theta_apply);
+  gemm_rm(cx.h, true, false, (int)op.nk, s, (int)op.mk, op.Tc, (int)op.nk, Y, s, Z, s);
+  cx.toc();
+  cx.h->st.flop_theta_apply += 2.0 * op.mk * op.nk * s;
+  cx.h->st.bytes_theta_apply += 8.0 * op.mk * op.nk;
+}
+
+// Y[m x s] = Theta X[n x s]
+void apply_N(Ctx& cx, const ThetaOp& op, const double* X, double* Y, int s) {
+  tn_handle* h = cx.h;
+  const PosInfo& p = *op.pos;
+  if (p.kind == 1) { tc_apply_N(cx, op, X, Y, s); return; }
+  const CellDev& c = *p.c;
+  DBuf<double> Xb(h, (size_t)op.nk * s), Yk(h, (size_t)op.mk * s);
+  gemm_rm(h, true, false, c.nB, op.g * s, p.pu, c.BvS, c.nB, X, op.g * s, Xb.p, op.g * s);
+  tc_apply_N(cx, op, Xb.p, Yk.p, s);
+  if (op.left) map_RT(h, c, Yk.p, Y, op.dx, s);
+  else map_LT(h, c, p.fold, Yk.p, Y, op.dx, s);
+}
+// Z[n x s] = Theta^T Y[m x s]
+void apply_T(Ctx& cx, const ThetaOp& op, const double* Y, double* Z, int s) {
+  tn_handle* h = cx.h;
+  const PosInfo& p = *op.pos;
+  if (p.kind == 1) { tc_apply_T(cx, op, Y, Z, s); return; }
+  const CellDev& c = *p.c;
+  DBuf<double> Yk(h, (size_t)op.mk * s), Zb(h, (size_t)op.nk * s);
+  if (op.left) map_R(h, c, Y, Yk.p, op.dx, s);
+  else map_L(h, c, p.fold, Y, Yk.p, op.dx, s);
+  tc_apply_T(cx, op, Yk.p, Zb.p, s);
+  gemm_rm(h, false, false, p.pu, op.g * s, c.nB, c.BvS, c.nB, Zb.p, op.g * s, Z, op.g * s);
+}
+
+// ---- Theta build -----------------------------------------------------------------------------
+// A: old MPS tensor [al][pd][ar]; E: environment on the far side, [(dy, w), g]
+ThetaOp build_op(Ctx& cx, const PosInfo& p, bool left, const MpsTensor& A, const double* E, int g) {
+  tn_handle* h = cx.h;
+  ThetaOp op;
+  op.pos = &p; op.left = left; op.g = g;
+  const int al = A.dl, ar = A.dr;
+  op.dx = left ? ar : al;
+  const int dy = left ? al : ar;
+  cx.tic(&h->st.ms_theta_build);
+  if (p.kind == 0) {
+    const CellDev& c = *p.c;
+    op.m = (i64)op.dx * (left ? p.wr : p.wl);
+    op.n = (i64)p.pu * g;
+    op.mk = (i64)op.dx * c.nK;
+    op.nk = (i64)c.nB * g;
+    op.Tc = h->dalloc<double>((size_t)op.mk * op.nk);
+    DBuf<double> Ek(h, (size_t)dy * c.nK * g);
+    if (left) {
+      map_L(h, c, p.fold, E, Ek.p, dy, g);
+      DBuf<double> At(h, (size_t)al * A.p * ar);
+      permute3(h, At.p, A.d, ar, A.p, al, 1, ar, (i64)A.p * ar);
+      theta_core(h, c, At.p, op.dx, dy, Ek.p, g, op.Tc);
+    } else {
+      map_R(h, c, E, Ek.p, dy, g);
+      theta_core(h, c, A.d, op.dx, dy, Ek.p, g, op.Tc);
+    }
+  } else {
+    const CellDev& cl = *p.c;
+    const CellDev& cr = *p.cr;
+    const int n_r = cl.n_r, n_o = cl.n_o, n_lp = cr.n_l, n_i = cr.n_i, n_q = cr.bd_rows;
+    if (!left) {
+      op.m = op.mk = (i64)al * n_r * n_o;
+      op.n = op.nk = (i64)n_q * g;
+      op.Tc = h->dalloc<double>((size_t)op.mk * op.nk);
+      DBuf<double> Rm2(h, (size_t)ar * n_r * n_i * g), T1(h, (size_t)al * n_o * n_r * n_i * g);
+      GemmDesc d;
+      d.B1 = ar; d.M = n_r; d.N = n_i * g; d.K = n_lp;
+      d.A = cr.Bh; d.a_i = n_lp; d.a_k = 1;
+      d.B = E; d.b_b1 = (i64)n_lp * n_i * g; d.b_k = (i64)n_i * g; d.b_j = 1;
+      d.C = Rm2.p; d.c_b1 = (i64)n_r * n_i * g; d.c_i = (i64)n_i * g; d.c_j = 1;
+      d.nsplit = 1;
+      gemm_general(h, d);
+      gemm_rm(h, false, false, al * n_o, n_r * n_i * g, ar, A.d, ar, Rm2.p, n_r * n_i * g, T1.p, n_r * n_i * g);
+      med_apply_bd(h, T1.p, cr.Bd, op.Tc, al, n_o, n_r, n_i, n_q, g);
+      h->st.flop_theta_build += 2.0 * ar * n_r * n_i * g * n_lp + 2.0 * al * n_o * (double)n_r * n_i * g * ar +
+                                2.0 * (double)op.mk * op.nk * n_i;
+    } else {
+      op.m = op.mk = (i64)ar * n_lp * n_i;
+      op.n = op.nk = (i64)n_q * g;
+      op.Tc = h->dalloc<double>((size_t)op.mk * op.nk);
+      DBuf<double> Lk(h, (size_t)n_lp * al * n_o * g), TL(h, (size_t)ar * n_lp * g);
+      GemmDesc d;
+      d.B1 = al; d.B2 = n_o; d.M = n_lp; d.N = g; d.K = n_r;
+      d.A = cr.Bh; d.a_i = 1; d.a_k = n_lp;
+      d.B = E; d.b_b1 = (i64)n_r * n_o * g; d.b_b2 = g; d.b_k = (i64)n_o * g; d.b_j = 1;
+      d.C = Lk.p; d.c_b1 = (i64)n_o * g; d.c_b2 = g; d.c_i = (i64)al * n_o * g; d.c_j = 1;
+      d.nsplit = 1;
+      gemm_general(h, d);
+      GemmDesc e;
+      e.B1 = n_lp; e.M = ar; e.N = g; e.K = al * n_o;
+      e.A = A.d; e.a_i = 1; e.a_k = ar;
+      e.B = Lk.p; e.b_b1 = (i64)al * n_o * g; e.b_k = g; e.b_j = 1;
+      e.C = TL.p; e.c_b1 = g; e.c_i = (i64)n_lp * g; e.c_j = 1;
+      e.nsplit = 1;
+      gemm_general(h, e);
+      med_outer_bd(h, TL.p, cr.Bd, op.Tc, (i64)ar * n_lp, n_i, n_q, g);
+      h->st.flop_theta_build += 2.0 * al * n_o * (double)n_lp * g * n_r + 2.0 * n_lp * (double)ar * g * al * n_o;
+    }
+  }
+  cx.toc();
+  return op;
+}
+void free_op(Ctx& cx, ThetaOp& op) {
+  if (op.Tc) cx.h->dfree(op.Tc);
+  op.Tc = nullptr;
+}
+
+// ---- truncated SVD of the implicit Theta: block subspace iteration + Rayleigh-Ritz -----------
+__global__ void k_rank_decide(const double* sig, int ks, int chi, int gap_guard, int* keep, double* stat) {
+  if (threadIdx.x || blockIdx.x) return;
+  double s0 = sig[0];
+  int k = 0;
+  if (s0 > 0.0)
+    for (int i = 0; i < ks; i++) k += sig[i] > 1e-14 * s0 ? 1 : 0;
+  if (k > chi) {
+    k = chi;
+    if (gap_guard)
+      while (k > 1 && sig[k] >= (1.0 - 1e-6) * sig[k - 1]) k--;
+  }
+  if (k < 1) k = 1;
+  *keep = k;
+  stat[1] = s0 > 0.0 ? sig[k - 1] / s0 : 0.0;   // candidate for the running max, committed at convergence
+}
+__global__ void k_commit_stat(double* stat) {
+  if (threadIdx.x || blockIdx.x) return;
+  stat[0] = fmax(stat[0], stat[1]);
+}
+// partial column sums of squares of (P - Q), both [m x k]
+__global__ void k_coldiff_part(const double* P, const double* Q, i64 m, int k, int rows_per_block, double* part) {
+  int col = threadIdx.x;
+  if (col >= k) return;
+  i64 r0 = (i64)blockIdx.x * rows_per_block, r1 = min(m, r0 + rows_per_block);
+  double s = 0.0;
+  for (i64 r = r0; r < r1; r++) {
+    double d = P[r * k + col] - Q[r * k + col];
+    s += d * d;
+  }
+  part[(i64)blockIdx.x * k + col] = s;
+}
+__global__ void k_resid_flag(const double* part, int nblk, int k, const int* keep, const double* sig, double tol,
+                             int* flag) {
+  __shared__ int bad;
+  if (threadIdx.x == 0) bad = 0;
+  __syncthreads();
+  int col = threadIdx.x;
+  if (col < k && col < *keep) {
+    double s = 0.0;
+    for (int b = 0; b < nblk; b++) s += part[(i64)b * k + col];
+    if (!(sqrt(s) <= tol * sig[0])) bad = 1;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) *flag = bad ? 0 : 1;
+}
+
+// Outputs: Vz [n x chi] leading right singular vectors, C [m x chi] = Theta Vz; columns >= keep are zero.
+void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* C) {
+  tn_handle* h = cx.h;
+  const i64 m = op.m, n = op.n;
+  DBuf<double> Om(h, (size_t)n * ks), Z(h, (size_t)n * ks), Ya(h, (size_t)m * ks), Yb(h, (size_t)m * ks);
+  DBuf<double> TV(h, (size_t)m * ks), US(h, (size_t)m * ks);
+  DBuf<double> B(h, (size_t)ks * ks), Bo(h, (size_t)ks * ks), Wt(h, (size_t)ks * ks), sig(h, ks);
+  double* Y = Ya.p;
+  double* Yn = Yb.p;
+  fill_random(h, Om.p, n * ks, cx.seed++);
+  cx.tic(&h->st.ms_orth_svd);
+  orth_columns(h, Om.p, n, ks, 2);
+  cx.toc();
+  const int rpb = 512;
+  const int nblk = cdiv(m, rpb);
+  DBuf<double> part(h, (size_t)nblk * ks);
+  bool prev = false;
+  for (int it = 0;; it++) {
+    apply_N(cx, op, Om.p, Yn, ks);
+    if (prev) {
+      gemm_rm(h, false, true, (int)m, ks, ks, Yn, ks, Wt.p, ks, TV.p, ks);
+      gemm_rm(h, false, true, (int)m, ks, ks, Y, ks, Bo.p, ks, US.p, ks);
+      k_coldiff_part<<<nblk, std::max(32, (ks + 31) / 32 * 32), 0, h->stream>>>(TV.p, US.p, m, ks, rpb, part.p);
+      TN_LAUNCH_CHECK(h);
+      k_resid_flag<<<1, std::max(32, (ks + 31) / 32 * 32), 0, h->stream>>>(part.p, nblk, ks, cx.d_keep, sig.p,
+                                                                        h->svd_tol, cx.d_flag);
+      TN_LAUNCH_CHECK(h);
+      int flag = 0;
+      TN_CUDA(cudaMemcpyAsync(&flag, cx.d_flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+      TN_CUDA(cudaStreamSynchronize(h->stream));
+      if (flag || it >= h->svd_maxit) break;
+    }
+    std::swap(Y, Yn);
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Y, m, ks, 4);
+    cx.toc();
+    apply_T(cx, op, Y, Z.p, ks);
+    TN_CUDA(cudaMemcpyAsync(Om.p, Z.p, sizeof(double) * n * ks, cudaMemcpyDeviceToDevice, h->stream));
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Om.p, n, ks, 4);
+    gemm_rm(h, true, false, ks, ks, (int)n, Om.p, ks, Z.p, ks, B.p, ks);
+    jacobi_rows(h, B.p, ks, ks, ks, Bo.p, Wt.p, sig.p);
+    k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, ks, chi, h->gap_guard, cx.d_keep, cx.d_stat);
+    TN_LAUNCH_CHECK(h);
+    cx.toc();
+    prev = true;
+    h->st.svd_iterations++;
+  }
+  k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
+  TN_LAUNCH_CHECK(h);
+  gemm_rm(h, false, true, (int)n, ks, ks, Om.p, ks, Wt.p, ks, Z.p, ks);        // V = Omega W
+  permute3(h, Vz, Z.p, 1, (int)n, chi, 0, ks, 1, 2, cx.d_keep);
+  permute3(h, C, TV.p, 1, (int)m, chi, 0, ks, 1, 2, cx.d_keep);
+}
+
+MpsTensor new_tensor(tn_handle* h, int dl, int p, int dr) {
+  MpsTensor t;
+  t.dl = dl; t.p = p; t.dr = dr;
+  t.d = h->dalloc<double>((size_t)dl * p * dr);
+  return t;
+}
+
+// R_y = compress(T_y R_{y+1}; D, sweeps).  Returns the tensors of R_y (unit norm) and log of the norm removed.
+std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Aold, int D, int sweeps,
+                                double* lognorm) {
+  tn_handle* h = cx.h;
+  std::vector<PosInfo> pos = row_positions(h, y);
+  const int n = (int)pos.size();
+  const bool exact = D <= 0;
+  // ---- C-1: left-canonicalise a working copy of R_{y+1}
+  std::vector<MpsTensor> A(n);
+  for (int j = 0; j < n; j++) {
+    A[j] = new_tensor(h, Aold[j].dl, Aold[j].p, Aold[j].dr);
+    TN_CUDA(cudaMemcpyAsync(A[j].d, Aold[j].d, sizeof(double) * A[j].dl * A[j].p * A[j].dr, cudaMemcpyDeviceToDevice,
+                            h->stream));
+  }
+  DBuf<double> rlast(h, 1);
+  for (int j = 0; j < n; j++) {
+    const i64 rows = (i64)A[j].dl * A[j].p;
+    const int ar = A[j].dr;
+    DBuf<double> Q(h, (size_t)rows * ar), Rf(h, (size_t)ar * ar);
+    TN_CUDA(cudaMemcpyAsync(Q.p, A[j].d, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Q.p, rows, ar, 4);
+    cx.toc();
+    gemm_rm(h, true, false, ar, ar, (int)rows, Q.p, ar, A[j].d, ar, Rf.p, ar);
+    TN_CUDA(cudaMemcpyAsync(A[j].d, Q.p, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
+    if (j + 1 < n) {
+      const int cols = A[j + 1].p * A[j + 1].dr;
+      DBuf<double> T(h, (size_t)ar * cols);
+      gemm_rm(h, false, false, ar, cols, ar, Rf.p, ar, A[j + 1].d, cols, T.p, cols);
+      TN_CUDA(cudaMemcpyAsync(A[j + 1].d, T.p, sizeof(double) * ar * cols, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+      TN_CUDA(cudaMemcpyAsync(rlast.p, Rf.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    }
+  }
+  // ---- static bond dimensions of the new MPS (zero-padded where the numerical rank is lower)
+  std::vector<int> chi(n + 1, 1);
+  const int cap = exact ? h->exact_cap : D;
+  for (int j = n - 1; j >= 0; j--) {
+    i64 mm = (i64)A[j].dl * pos[j].wl, nn = (i64)pos[j].pu * chi[j + 1];
+    i64 full = std::min(mm, nn);
+    if (exact && full > cap)
+      tn_throw(TN_ERR_ARG, "exact contraction (D <= 0) needs bond %lld > TN_OPT_EXACT_CAP = %d at row %d position %d",
+               (long long)full, cap, y, j);
+    chi[j] = (int)std::min<i64>(cap, full);
+  }
+  // ---- C-2/C-3: zipper right -> left
+  std::vector<double*> Renv(n, nullptr), Lenv(n, nullptr);
+  std::vector<MpsTensor> N(n);
+  Renv[n - 1] = h->dalloc<double>(1);
+  TN_CUDA(cudaMemcpyAsync(Renv[n - 1], rlast.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  for (int j = n - 1; j >= 0; j--) {
+    const int g = chi[j + 1];
+    ThetaOp op = build_op(cx, pos[j], false, A[j], Renv[j], g);
+    const int ks = exact ? (int)std::min(op.m, op.n)
+                         : (int)std::min<i64>((i64)chi[j] + h->oversample, std::min(op.m, op.n));
+    DBuf<double> Vz(h, (size_t)op.n * chi[j]);
+    double* C = h->dalloc<double>((size_t)op.m * chi[j]);
+    svd_trunc(cx, op, chi[j], ks, Vz.p, C);
+    N[j] = new_tensor(h, chi[j], pos[j].pu, g);
+    permute3(h, N[j].d, Vz.p, chi[j], pos[j].pu, g, 1, (i64)g * chi[j], chi[j]);
+    if (j > 0) {
+      Renv[j - 1] = C;
+    } else {
+      scale_by(h, N[0].d, (i64)N[0].dl * N[0].p * N[0].dr, C, false);
+      h->dfree(C);
+    }
+    free_op(cx, op);
+  }
+  // ---- C-4: one-site variational passes, alternating, first left -> right
+  int centre = 0;
+  if (!exact && sweeps > 0) {
+    Lenv[0] = h->dalloc<double>(1);
+    fill_value(h, Lenv[0], 1, 1.0);
+    for (int sw = 0; sw < sweeps; sw++) {
+      if (sw % 2 == 0) {
+        for (int j = 0; j < n; j++) {
+          const int g = chi[j], s = chi[j + 1];
+          ThetaOp op = build_op(cx, pos[j], true, A[j], Lenv[j], g);
+          DBuf<double> Z(h, (size_t)op.n * s);
+          apply_T(cx, op, Renv[j], Z.p, s);
+          if (j + 1 < n) {
+            cx.tic(&h->st.ms_orth_svd);
+            orth_columns(h, Z.p, op.n, s, 4);
+            cx.toc();
+            if (Lenv[j + 1]) h->dfree(Lenv[j + 1]);
+            Lenv[j + 1] = h->dalloc<double>((size_t)op.m * s);
+            apply_N(cx, op, Z.p, Lenv[j + 1], s);
+          }
+          permute3(h, N[j].d, Z.p, g, pos[j].pu, s, s, (i64)g * s, 1);
+          free_op(cx, op);
+        }
+        centre = n - 1;
+      } else {
+        for (int j = n - 1; j >= 0; j--) {
+          const int g = chi[j + 1], s = chi[j];
+          ThetaOp op = build_op(cx, pos[j], false, A[j], Renv[j], g);
+          DBuf<double> Z(h, (size_t)op.n * s);
+          apply_T(cx, op, Lenv[j], Z.p, s);
+          if (j > 0) {
+            cx.tic(&h->st.ms_orth_svd);
+            orth_columns(h, Z.p, op.n, s, 4);
+            cx.toc();
+            h->dfree(Renv[j - 1]);
+            Renv[j - 1] = h->dalloc<double>((size_t)op.m * s);
+            apply_N(cx, op, Z.p, Renv[j - 1], s);
+          }
+          permute3(h, N[j].d, Z.p, s, pos[j].pu, g, 1, (i64)g * s, s);
+          free_op(cx, op);
+        }
+        centre = 0;
+      }
+    }
+  }
+  // ---- norm of the centre tensor -> log-scale
+  const i64 nc = (i64)N[centre].dl * N[centre].p * N[centre].dr;
+  frob_norm(h, N[centre].d, nc, cx.d_scal);
+  scale_by(h, N[centre].d, nc, cx.d_scal, true);
+  double nrm = 0.0;
+  TN_CUDA(cudaMemcpyAsync(&nrm, cx.d_scal, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+  if (!(nrm > 0.0) || !std::isfinite(nrm)) tn_throw(TN_ERR_NUMERIC, "row %d: boundary MPS norm is %g", y, nrm);
+  *lognorm = std::log(nrm);
+  for (int j = 0; j < n; j++) {
+    h->dfree(A[j].d);
+    if (Renv[j]) h->dfree(Renv[j]);
+    if (Lenv[j]) h->dfree(Lenv[j]);
+  }
+  return N;
+}
+
+}  // namespace
+
+void mps_free(tn_handle* h) {
+  for (auto& row : h->rows)
+    for (auto& t : row)
+      if (t.d) h->dfree(t.d);
+  h->rows.clear();
+  h->lognorm.clear();
+  h->have_mps = false;
+  h->have_logz = false;
+}
+
+void contract_run(tn_handle* h, int D, int sweeps) {
+  mps_free(h);
+  Ctx cx;
+  cx.h = h;
+  DBuf<int> ints(h, 4);
+  DBuf<double> dbl(h, 8);
+  cx.d_keep = ints.p; cx.d_flag = ints.p + 1;
+  cx.d_stat = dbl.p; cx.d_scal = dbl.p + 4;
+  TN_CUDA(cudaMemsetAsync(dbl.p, 0, sizeof(double) * 8, h->stream));
+  cudaEvent_t e0, e1;
+  TN_CUDA(cudaEventCreate(&e0)); TN_CUDA(cudaEventCreate(&e1));
+  TN_CUDA(cudaEventRecord(e0, h->stream));
+  const int Ly = h->Ly;
+  const int npos = h->has_med() ? 2 * h->Lx - 1 : h->Lx;
+  h->rows.assign(Ly + 1, std::vector<MpsTensor>());
+  h->lognorm.assign(Ly + 1, 0.0);
+  h->rows[Ly].resize(npos);
+  for (int j = 0; j < npos; j++) {
+    h->rows[Ly][j] = new_tensor(h, 1, 1, 1);
+    fill_value(h, h->rows[Ly][j].d, 1, 1.0);
+  }
+  try {
+    for (int y = Ly - 1; y >= 1; y--) {
+      h->rows[y] = compress(cx, y, h->rows[y + 1], D, sweeps, &h->lognorm[y]);
+      h->st.rows_contracted++;
+      cx.flush();
+    }
+  } catch (...) {
+    cx.flush();
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    throw;
+  }
+  double stat = 0.0;
+  TN_CUDA(cudaMemcpyAsync(&stat, cx.d_stat, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaEventRecord(e1, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  h->st.ms_contract += ms;
+  h->st.min_sigma_rel = std::max(h->st.min_sigma_rel, stat);
+  h->D = D; h->sweeps = sweeps;
+  h->have_mps = true;
+}

@@ -1,0 +1,651 @@
+// a4(ii)-a5: branch and bound over cells.  Eq. (7) PAPER.md:94-98 (chain rule), Fig. 3
+// (branch to d*M candidates, keep the M most probable), Eqs. (8)-(9) PAPER.md:100-107 (conditionals
+// depend on the boundary only -> right blocks are computed once per row start and inherited),
+// Fig. 6(b) PAPER.md:143 (fixed legs above, one open site, boundary MPS R_{y+1} below, contracted
+// exactly, "up to normalization"), p_d PAPER.md:113.
+//
+// For beam element m at cell (x,y), with S, Q the tensors of R_{y+1} under columns x and x+1/2:
+//   u(m;a,b,cl,ch) = hS[a] wA[a] X[t(a)][b] vS[b] Yc[b][cl] * (wC[cl][ch] dvec[Pi ch])
+//                    * sum_{b''} LG_m[(Pd b, Po cl)][b''] RM_{m,x}[b''][Pr a],     LG_m = Lv_m . (S Q)
+//   hS = BhS_x[Pr(a of the cell on the left)], vS = BvS_x[Pd(b of the cell above)], dvec = Bd_x[Po(c_lo of upper-left)].
+#include "kernels.cuh"
+#include <algorithm>
+#include <cfloat>
+
+namespace {
+
+struct Cand { double score; int parent; unsigned state; };
+
+struct RowTab {          // device tables of one column of the current row
+  const CellDev* c;
+  double* G = nullptr;   // [npp][Dl][Dr],  npp = n_d * n_o
+  int Dl = 1, Dr = 1, npp = 1;
+  double* RM = nullptr;  // [slot][Dr][n_r]
+  double* ls = nullptr;  // [slot] log-scale of RM
+};
+
+// ---- functors ----------------------------------------------------------------------------------
+struct LdLv { const double* Lv; int ld; __device__ __forceinline__ double operator()(int, int m, int k) const { return Lv[(i64)m * ld + k]; } };
+struct LdGj { const double* G; int Dl, Dr; __device__ __forceinline__ double operator()(int, int k, int j) const { return __ldg(G + (i64)(j / Dr) * Dl * Dr + (i64)k * Dr + (j % Dr)); } };
+struct StPlain { double* C; i64 ld; __device__ __forceinline__ void operator()(int, int, int i, int j, double v) const { C[(i64)i * ld + j] = v; } };
+
+struct LdPA {   // A(m; i=(b,cl), k) = LG[m][(Pd b * n_o + Po cl)][k]
+  const double* LG; const int *Pd, *Po; int nCl, n_o, npp, Dr;
+  __device__ __forceinline__ double operator()(int m, int i, int k) const {
+    int b = i / nCl, cl = i % nCl;
+    return LG[((i64)m * npp + Pd[b] * n_o + Po[cl]) * Dr + k];
+  }
+};
+struct LdPB {   // B(m; k, a) = RM[slot m][k][Pr a]
+  const double* RM; const int *slot, *Pr; int Dr, n_r;
+  __device__ __forceinline__ double operator()(int m, int k, int a) const {
+    return RM[((i64)slot[m] * Dr + k) * n_r + Pr[a]];
+  }
+};
+struct StPV {
+  double* V; const double *hS, *wA, *X, *vS, *Yc; const int *hrow, *vrow, *slot;
+  int nA, nB, nCl, tshift; i64 per_m;
+  __device__ __forceinline__ void operator()(int m, int, int i, int a, double acc) const {
+    int b = i / nCl, cl = i % nCl;
+    double w = hS[(i64)hrow[m] * nA + a] * wA[a] * X[(a >> tshift) * nB + b] * vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl];
+    V[(i64)m * per_m + (i64)i * nA + a] = acc * w;
+  }
+};
+struct LdHA {   // A(i=(b',b''), kk=(b,cl)) = G[(Pd b * n_o + Po cl)][i]
+  const double* G; const int *Pd, *Po; int nCl, n_o; i64 DD;
+  __device__ __forceinline__ double operator()(int, int i, int kk) const {
+    int b = kk / nCl, cl = kk % nCl;
+    return __ldg(G + (i64)(Pd[b] * n_o + Po[cl]) * DD + i);
+  }
+};
+struct LdHB {   // B(kk=(b,cl), j=(m,t)) = X[t][b] vS[vrow m][b] Yc[b][cl] fc[m][cl]
+  const double *X, *vS, *Yc, *fc; const int* vrow; int nB, nCl, nT;
+  __device__ __forceinline__ double operator()(int, int kk, int j) const {
+    int b = kk / nCl, cl = kk % nCl, m = j / nT, t = j % nT;
+    return X[t * nB + b] * vS[(i64)vrow[m] * nB + b] * Yc[b * nCl + cl] * fc[(i64)m * nCl + cl];
+  }
+};
+struct StH { double* H; i64 DD; __device__ __forceinline__ void operator()(int, int, int i, int j, double v) const { H[(i64)j * DD + i] = v; } };
+
+// ---- small kernels -------------------------------------------------------------------------------
+// vrow[x][m], drow[x][m] from the states of the row above
+__global__ void k_above_rows(const unsigned* states, int ncell_ld, int nb, int y, int Lx, int ns, int S,
+                             const CellDev* cells, int* vrow, int* drow) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nb * Lx) return;
+  int x = t / nb, m = t % nb;
+  int v = 0, d = 0;
+  if (y > 0) {
+    const int half = ns / 2;
+    const CellDev& up = cells[(y - 1) * Lx + x];
+    unsigned st = states[(i64)m * ncell_ld + (y - 1) * Lx + x];
+    int b = S == 1 ? (st & ((1u << ns) - 1)) : ((st >> ns) & ((1u << ns) - 1));
+    v = up.Pd[b];
+    if (x > 0 && S == 3) {
+      const CellDev& ul = cells[(y - 1) * Lx + x - 1];
+      unsigned su = states[(i64)m * ncell_ld + (y - 1) * Lx + x - 1];
+      d = ul.Po[(su >> (2 * ns)) & ((1u << half) - 1)];
+    }
+  }
+  vrow[x * nb + m] = v;
+  drow[x * nb + m] = d;
+}
+__global__ void k_hrow(const unsigned* states, int ncell_ld, int nb, int cellidx, int x, int ns, const CellDev* cells,
+                       int* hrow) {
+  int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= nb) return;
+  int r = 0;
+  if (x > 0) {
+    unsigned st = states[(i64)m * ncell_ld + cellidx - 1];
+    r = cells[cellidx - 1].Pr[st & ((1u << ns) - 1)];
+  }
+  hrow[m] = r;
+}
+// fc[m][cl] = sum_ch wC[cl][ch] Bd[drow][Pi ch]
+__global__ void k_fc(CellDev c, const int* drow_x, const int* slot, int nb, double* fc) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nb * c.nCl) return;
+  int m = t / c.nCl, cl = t % c.nCl;
+  int dr = drow_x[slot ? slot[m] : m];
+  double s = 0.0;
+  for (int ch = 0; ch < c.nCh; ch++) s += c.wC[cl * c.nCh + ch] * c.Bd[dr * c.n_i + c.Pi[ch]];
+  fc[t] = s;
+}
+// RS[m][b'][a] = wA[a] sum_b'' H[(m*nT + t(a))][b'][b''] RM[m][b''][Pr a]
+__global__ void k_rs(CellDev c, const double* H, const double* RM, int nb, int Dl, int Dr, double* RS) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  i64 total = (i64)nb * Dl * c.nA;
+  if (t >= total) return;
+  int a = (int)(t % c.nA);
+  int bl = (int)((t / c.nA) % Dl);
+  int m = (int)(t / ((i64)c.nA * Dl));
+  const double* hh = H + (((i64)m * c.nT + (a >> c.tshift)) * Dl + bl) * Dr;
+  const double* rm = RM + (i64)m * Dr * c.n_r + c.Pr[a];
+  double s = 0.0;
+  for (int k = 0; k < Dr; k++) s += hh[k] * rm[(i64)k * c.n_r];
+  RS[t] = c.wA[a] * s;
+}
+// per-m max-abs normalisation with log-scale
+__global__ void k_norm_rm(double* RM, int per_m, const double* ls_in, double* ls_out) {
+  __shared__ double sh[256];
+  int m = blockIdx.x;
+  double* p = RM + (i64)m * per_m;
+  double mx = 0.0;
+  for (int i = threadIdx.x; i < per_m; i += blockDim.x) mx = fmax(mx, fabs(p[i]));
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + o]);
+    __syncthreads();
+  }
+  mx = sh[0];
+  if (mx > 0.0)
+    for (int i = threadIdx.x; i < per_m; i += blockDim.x) p[i] /= mx;
+  if (threadIdx.x == 0) ls_out[m] = ls_in[m] + (mx > 0.0 ? log(mx) : 0.0);
+}
+// Z[m] = sum max(v,0) fc[m][cl]; negatives counted and clamped in place (reading S7)
+__global__ void k_beam_Z(double* V, i64 per_m, int nA, int nCl, const double* fc, double* Z, unsigned long long* nneg) {
+  __shared__ double sh[256];
+  __shared__ unsigned long long shn[256];
+  int m = blockIdx.x;
+  double* v = V + (i64)m * per_m;
+  double s = 0.0;
+  unsigned long long neg = 0;
+  for (i64 i = threadIdx.x; i < per_m; i += blockDim.x) {
+    double x = v[i];
+    if (x < 0.0) { neg++; x = 0.0; v[i] = 0.0; }
+    if (!(x == x)) { x = 0.0; v[i] = 0.0; }
+    int cl = (int)((i / nA) % nCl);
+    s += x * fc[(i64)m * nCl + cl];
+  }
+  sh[threadIdx.x] = s; shn[threadIdx.x] = neg;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) { sh[threadIdx.x] += sh[threadIdx.x + o]; shn[threadIdx.x] += shn[threadIdx.x + o]; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { Z[m] = sh[0]; if (shn[0]) atomicAdd(nneg, shn[0]); }
+}
+// scale[m] = exp(logp[m] - max logp) / Z[m]
+__global__ void k_beam_scale(const double* logp, const double* Z, int nb, double* scale) {
+  __shared__ double sh[256];
+  double mx = -INFINITY;
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) mx = fmax(mx, logp[i]);
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + o]);
+    __syncthreads();
+  }
+  mx = sh[0];
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) scale[i] = Z[i] > 0.0 ? exp(logp[i] - mx) / Z[i] : 0.0;
+}
+
+// ---- top-M radix selection on r = v * fcd * scale (monotone in the score) ------------------------
+struct SelState {
+  unsigned long long prefix;   // key bits fixed so far (above `shift`)
+  unsigned long long want;     // rank still to locate inside the prefix class
+  unsigned long long above;    // candidates strictly above the prefix class
+  unsigned long long inbin;    // candidates inside the prefix class
+  unsigned long long thresh;   // final threshold key
+  int done, takeall;
+};
+struct SelArgs {
+  const double* V; const double *scale, *wC, *Bd; const int *drow_x, *slot, *Pi;
+  i64 per_m; int nb, nA, nCl, nCh, n_i;
+};
+__device__ __forceinline__ double sel_fcd(const SelArgs& a, int m, int cl, int ch) {
+  return a.wC[cl * a.nCh + ch] * a.Bd[a.drow_x[a.slot[m]] * a.n_i + a.Pi[ch]];
+}
+__global__ void k_sel_hist(SelArgs a, const SelState* st, int shift, int nbits, int first, unsigned* hist) {
+  __shared__ unsigned sh[4096];
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sh[i] = 0;
+  __syncthreads();
+  const unsigned long long prefix = st->prefix;
+  const i64 total = (i64)a.nb * a.per_m;
+  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+    double v = a.V[t];
+    if (!(v > 0.0)) continue;
+    int m = (int)(t / a.per_m);
+    int cl = (int)(((t % a.per_m) / a.nA) % a.nCl);
+    double vs = v * a.scale[m];
+    for (int ch = 0; ch < a.nCh; ch++) {
+      double r = vs * sel_fcd(a, m, cl, ch);
+      if (!(r > 0.0)) continue;
+      unsigned long long key = (unsigned long long)__double_as_longlong(r);
+      if (!first && (key >> (shift + nbits)) != prefix) continue;
+      atomicAdd(&sh[(key >> shift) & ((1u << nbits) - 1)], 1u);
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x)
+    if (sh[i]) atomicAdd(&hist[i], sh[i]);
+}
+__global__ void k_sel_resolve(SelState* st, unsigned* hist, int shift, int nbits, int first, unsigned long long cap) {
+  if (threadIdx.x || blockIdx.x) return;
+  const int nbin = 1 << nbits;
+  unsigned long long cum = 0;
+  int found = -1;
+  for (int b = nbin - 1; b >= 0; b--) {
+    unsigned long long hb = hist[b];
+    if (cum + hb >= st->want) { found = b; break; }
+    cum += hb;
+  }
+  if (found < 0) {            // fewer candidates than wanted: take everything positive
+    st->takeall = 1; st->done = 1; st->thresh = 1ull;
+    st->inbin = 0; st->above += cum;
+  } else {
+    st->prefix = first ? (unsigned long long)found : ((st->prefix << nbits) | (unsigned long long)found);
+    st->want -= cum;
+    st->above += cum;
+    st->inbin = hist[found];
+    st->thresh = st->prefix << shift;
+    if (st->above + st->inbin <= cap || shift == 0) st->done = 1;
+  }
+  for (int b = 0; b < 4096; b++) hist[b] = 0;
+}
+struct Raw { int m; int i; int a; int ch; };
+__global__ void k_sel_collect(SelArgs a, const SelState* st, Raw* out, unsigned* count, unsigned cap) {
+  double thr = __longlong_as_double((long long)st->thresh);
+  thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
+  const i64 total = (i64)a.nb * a.per_m;
+  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+    double v = a.V[t];
+    if (!(v > 0.0)) continue;
+    int m = (int)(t / a.per_m);
+    i64 rem = t % a.per_m;
+    int i = (int)(rem / a.nA), aa = (int)(rem % a.nA);
+    int cl = i % a.nCl;
+    double vs = v * a.scale[m];
+    for (int ch = 0; ch < a.nCh; ch++) {
+      double r = vs * sel_fcd(a, m, cl, ch);
+      if (r > 0.0 && r >= thr) {
+        unsigned idx = atomicAdd(count, 1u);
+        if (idx < cap) out[idx] = Raw{m, i, aa, ch};
+      }
+    }
+  }
+}
+// exact scores of the collected candidates:  logp_m + log(u / Z_m)
+__global__ void k_sel_score(SelArgs a, const Raw* raw, unsigned n, unsigned npad, const double* logp, const double* Z,
+                            int ns, int S, Cand* out) {
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= npad) return;
+  if (t >= n) { out[t] = Cand{-INFINITY, 0x7fffffff, 0xffffffffu}; return; }
+  Raw q = raw[t];
+  int b = q.i / a.nCl, cl = q.i % a.nCl;
+  double u = a.V[(i64)q.m * a.per_m + (i64)q.i * a.nA + q.a] * sel_fcd(a, q.m, cl, q.ch);
+  unsigned state = (unsigned)q.a;
+  if (S >= 2) state |= (unsigned)b << ns;
+  if (S == 3) state |= ((unsigned)cl | ((unsigned)q.ch << (ns / 2))) << (2 * ns);
+  out[t] = Cand{logp[q.m] + log(u / Z[q.m]), q.m, state};
+}
+__device__ __forceinline__ bool cand_before(const Cand& x, const Cand& y) {   // reading S8 total order
+  if (x.score != y.score) return x.score > y.score;
+  if (x.parent != y.parent) return x.parent < y.parent;
+  return x.state < y.state;
+}
+__global__ void k_bitonic_step(Cand* c, unsigned n, unsigned k, unsigned j) {
+  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  unsigned l = i ^ j;
+  if (l > i) {
+    Cand x = c[i], y = c[l];
+    bool up = (i & k) == 0;
+    if (up ? cand_before(y, x) : cand_before(x, y)) { c[i] = y; c[l] = x; }
+  }
+}
+__global__ void __launch_bounds__(1024) k_bitonic_smem(Cand* c, unsigned n) {
+  extern __shared__ Cand sc[];
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) sc[i] = c[i];
+  __syncthreads();
+  for (unsigned k = 2; k <= n; k <<= 1)
+    for (unsigned j = k >> 1; j > 0; j >>= 1) {
+      for (unsigned i = threadIdx.x; i < n; i += blockDim.x) {
+        unsigned l = i ^ j;
+        if (l > i) {
+          Cand x = sc[i], y = sc[l];
+          bool up = (i & k) == 0;
+          if (up ? cand_before(y, x) : cand_before(x, y)) { sc[i] = y; sc[l] = x; }
+        }
+      }
+      __syncthreads();
+    }
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) c[i] = sc[i];
+}
+// new beam from the sorted candidates
+__global__ void k_new_beam(const Cand* cand, int nkeep, int M, const unsigned* st_old, unsigned* st_new, int ncell_ld,
+                           int cellidx, const int* slot_old, int* slot_new, double* logp_new, const double* LG,
+                           int npp, int Dr, int ldLv, double* Lv_new, const int* Pd, const int* Po, int n_o, int ns,
+                           int S, double* pd_out) {
+  int i = blockIdx.x;
+  if (i >= nkeep) return;
+  Cand c = cand[i];
+  for (int k = threadIdx.x; k < cellidx; k += blockDim.x)
+    st_new[(i64)i * ncell_ld + k] = st_old[(i64)c.parent * ncell_ld + k];
+  __shared__ double sh[128];
+  const int half = ns / 2;
+  int b = S == 1 ? (c.state & ((1u << ns) - 1)) : ((c.state >> ns) & ((1u << ns) - 1));
+  int cl = S == 3 ? ((c.state >> (2 * ns)) & ((1u << half) - 1)) : 0;
+  const double* src = LG + ((i64)c.parent * npp + Pd[b] * n_o + Po[cl]) * Dr;
+  double mx = 0.0;
+  for (int k = threadIdx.x; k < Dr; k += blockDim.x) mx = fmax(mx, fabs(src[k]));
+  sh[threadIdx.x] = mx;
+  __syncthreads();
+  for (int o = 64; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + o]);
+    __syncthreads();
+  }
+  mx = sh[0];
+  for (int k = threadIdx.x; k < ldLv; k += blockDim.x)
+    Lv_new[(i64)i * ldLv + k] = (k < Dr && mx > 0.0) ? src[k] / mx : 0.0;
+  if (threadIdx.x == 0) {
+    st_new[(i64)i * ncell_ld + cellidx] = c.state;
+    slot_new[i] = slot_old[c.parent];
+    logp_new[i] = c.score;
+    if (i == 0 && pd_out) *pd_out = fmax(*pd_out, cand[M].score);   // cand padded: -inf when nothing was discarded
+  }
+}
+__global__ void k_iota(int* p, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = i;
+}
+__global__ void k_reset_lv(double* Lv, int nb, int ld) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < nb * ld) Lv[i] = (i % ld == 0) ? 1.0 : 0.0;
+}
+// unpack cell states to +-1 spins (spin-id order)
+__global__ void k_unpack(const unsigned* states, int ncell_ld, int n, int n_spins, const int* cell_of, const int* bit_of,
+                         int8_t* out) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)n * n_spins) return;
+  int m = (int)(t / n_spins), i = (int)(t % n_spins);
+  unsigned st = states[(i64)m * ncell_ld + cell_of[i]];
+  out[t] = (int8_t)(1 - 2 * (int)((st >> bit_of[i]) & 1u));
+}
+// O-0 energy: one running fp64 sum, edges in input order, then fields in spin order (Eq. (1))
+__global__ void k_energy(const int8_t* s, int n, int n_spins, i64 n_edges, const int* eu, const int* ev, const double* J,
+                         const double* hf, double* E) {
+  int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n) return;
+  const int8_t* sm = s + (i64)m * n_spins;
+  double e = 0.0;
+  for (i64 k = 0; k < n_edges; k++) e = e + J[k] * (double)((int)sm[eu[k]] * (int)sm[ev[k]]);
+  for (int i = 0; i < n_spins; i++) e = e + hf[i] * (double)sm[i];
+  E[m] = e;
+}
+
+template <class T>
+T d2h(tn_handle* h, const T* p) {
+  T v;
+  TN_CUDA(cudaMemcpyAsync(&v, p, sizeof(T), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+  return v;
+}
+
+struct Tic {
+  tn_handle* h; double* dst; cudaEvent_t a, b;
+  Tic(tn_handle* h_, double* d) : h(h_), dst(d) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, h->stream); }
+  void stop() {
+    cudaEventRecord(b, h->stream); cudaEventSynchronize(b);
+    float ms = 0; if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) *dst += ms;
+    cudaEventDestroy(a); cudaEventDestroy(b);
+  }
+};
+
+void build_G(tn_handle* h, const MpsTensor& S, const MpsTensor* Q, RowTab& rt) {
+  if (Q) {
+    rt.Dl = S.dl; rt.Dr = Q->dr; rt.npp = S.p * Q->p;
+    rt.G = h->dalloc<double>((size_t)rt.npp * rt.Dl * rt.Dr);
+    GemmDesc g;
+    g.B1 = S.p; g.B2 = Q->p; g.M = S.dl; g.N = Q->dr; g.K = S.dr;
+    g.A = S.d; g.a_b1 = S.dr; g.a_b2 = 0; g.a_i = (i64)S.p * S.dr; g.a_k = 1;
+    g.B = Q->d; g.b_b1 = 0; g.b_b2 = Q->dr; g.b_k = (i64)Q->p * Q->dr; g.b_j = 1;
+    g.C = rt.G; g.c_b1 = (i64)Q->p * rt.Dl * rt.Dr; g.c_b2 = (i64)rt.Dl * rt.Dr; g.c_i = rt.Dr; g.c_j = 1;
+    g.nsplit = 1;
+    gemm_general(h, g);
+    h->st.flop_search += 2.0 * rt.npp * rt.Dl * (double)rt.Dr * S.dr;
+  } else {
+    rt.Dl = S.dl; rt.Dr = S.dr; rt.npp = S.p;
+    rt.G = h->dalloc<double>((size_t)rt.npp * rt.Dl * rt.Dr);
+    permute3(h, rt.G, S.d, S.p, S.dl, S.dr, S.dr, (i64)S.p * S.dr, 1);
+  }
+}
+
+void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, double* energies, double* logp_out,
+         double* log_pd_out) {
+  const int Ly = h->Ly, Lx = h->Lx, ns = h->ns, S = h->S, ncell = Ly * Lx;
+  int Dmax = 1;
+  for (int y = 1; y <= Ly; y++)
+    for (auto& t : h->rows[y]) Dmax = std::max(Dmax, std::max(t.dl, t.dr));
+  const int ldLv = Dmax;
+  const unsigned cap = (unsigned)std::max(2 * (i64)M, (i64)M + 2048);
+  unsigned npad = 4096;
+  while (npad < cap) npad <<= 1;
+  DBuf<unsigned> stA(h, (size_t)M * ncell), stB(h, (size_t)M * ncell);
+  DBuf<double> lpA(h, M), lpB(h, M), LvA(h, (size_t)M * ldLv), LvB(h, (size_t)M * ldLv);
+  DBuf<int> slA(h, M), slB(h, M), hrow(h, M), vrow(h, (size_t)M * Lx), drow(h, (size_t)M * Lx);
+  DBuf<double> Z(h, M), scale(h, M), pd(h, 1), fc(h, (size_t)M * 16);
+  DBuf<unsigned long long> nneg(h, 1);
+  DBuf<SelState> sel(h, 1);
+  DBuf<unsigned> hist(h, 4096), count(h, 1);
+  DBuf<Raw> raw(h, cap);
+  DBuf<Cand> cand(h, npad);
+  unsigned* st_cur = stA.p; unsigned* st_nxt = stB.p;
+  double* lp_cur = lpA.p; double* lp_nxt = lpB.p;
+  double* Lv_cur = LvA.p; double* Lv_nxt = LvB.p;
+  int* sl_cur = slA.p; int* sl_nxt = slB.p;
+  int nb = 1;
+  fill_value(h, lp_cur, 1, 0.0);
+  fill_value(h, pd.p, 1, -INFINITY);
+  TN_CUDA(cudaMemsetAsync(nneg.p, 0, sizeof(unsigned long long), h->stream));
+  TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
+  TN_CUDA(cudaMemsetAsync(st_cur, 0, sizeof(unsigned) * ncell, h->stream));
+  static bool attr = false;
+  if (!attr) { TN_CUDA(cudaFuncSetAttribute(k_bitonic_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * (int)sizeof(Cand))); attr = true; }
+
+  for (int y = 0; y < Ly; y++) {
+    const std::vector<MpsTensor>& R = h->rows[y + 1];
+    std::vector<RowTab> rt(Lx);
+    const int nb_row = nb;   // beam size at the row start = number of right-block slots
+    // ---- row start: tables of R_{y+1}, above-row indices, right blocks (a4 (ii))
+    Tic t_rb(h, &h->st.ms_search_rblocks);
+    for (int x = 0; x < Lx; x++) {
+      rt[x].c = &h->cell(y, x);
+      const MpsTensor& Sx = h->has_med() ? R[2 * x] : R[x];
+      const MpsTensor* Qx = (h->has_med() && x + 1 < Lx) ? &R[2 * x + 1] : nullptr;
+      build_G(h, Sx, Qx, rt[x]);
+      rt[x].RM = h->dalloc<double>((size_t)nb * rt[x].Dr * rt[x].c->n_r);
+      rt[x].ls = h->dalloc<double>(nb);
+    }
+    k_above_rows<<<cdiv((i64)nb * Lx, 256), 256, 0, h->stream>>>(st_cur, ncell, nb, y, Lx, ns, S, h->d_cells, vrow.p, drow.p);
+    TN_LAUNCH_CHECK(h);
+    k_iota<<<cdiv(nb, 256), 256, 0, h->stream>>>(sl_cur, nb);
+    TN_LAUNCH_CHECK(h);
+    k_reset_lv<<<cdiv((i64)nb * ldLv, 256), 256, 0, h->stream>>>(Lv_cur, nb, ldLv);
+    TN_LAUNCH_CHECK(h);
+    fill_value(h, rt[Lx - 1].RM, (i64)nb * rt[Lx - 1].Dr * rt[Lx - 1].c->n_r, 1.0);
+    fill_value(h, rt[Lx - 1].ls, nb, 0.0);
+    for (int x = Lx - 1; x >= 1; x--) {
+      const CellDev& c = *rt[x].c;
+      const int Dl = rt[x].Dl, Dr = rt[x].Dr;
+      const i64 DD = (i64)Dl * Dr;
+      DBuf<double> fcx(h, (size_t)nb * c.nCl), H(h, (size_t)nb * c.nT * DD), RS(h, (size_t)nb * Dl * c.nA);
+      k_fc<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(c, drow.p + (size_t)x * nb, nullptr, nb, fcx.p);
+      TN_LAUNCH_CHECK(h);
+      {
+        LdHA a{rt[x].G, c.Pd, c.Po, c.nCl, c.n_o, DD};
+        LdHB b{c.X, c.BvS, c.Yc, fcx.p, vrow.p + (size_t)x * nb, c.nB, c.nCl, c.nT};
+        StH e{H.p, DD};
+        int Mg = (int)DD, Ng = nb * c.nT, Kg = c.nB * c.nCl;
+        dim3 grid(1, cdiv(Mg, 64), cdiv(Ng, 64));
+        k_gemm<64, 64, 16, 2, 2, false, true, LdHA, LdHB, StH><<<grid, 128, 0, h->stream>>>(Mg, Ng, Kg, 1, a, b, e);
+        TN_LAUNCH_CHECK(h);
+        h->st.flop_search += 2.0 * Mg * (double)Ng * Kg;
+      }
+      {
+        i64 total = (i64)nb * Dl * c.nA;
+        k_rs<<<cdiv(total, 256), 256, 0, h->stream>>>(c, H.p, rt[x].RM, nb, Dl, Dr, RS.p);
+        TN_LAUNCH_CHECK(h);
+      }
+      GemmDesc g;
+      g.B1 = nb; g.M = Dl; g.N = c.bh_rows; g.K = c.nA;
+      g.A = RS.p; g.a_b1 = (i64)Dl * c.nA; g.a_i = c.nA; g.a_k = 1;
+      g.B = c.BhS; g.b_k = 1; g.b_j = c.nA;
+      g.C = rt[x - 1].RM; g.c_b1 = (i64)Dl * c.bh_rows; g.c_i = c.bh_rows; g.c_j = 1;
+      g.nsplit = 1;
+      gemm_general(h, g);
+      k_norm_rm<<<nb, 256, 0, h->stream>>>(rt[x - 1].RM, Dl * c.bh_rows, rt[x].ls, rt[x - 1].ls);
+      TN_LAUNCH_CHECK(h);
+    }
+    t_rb.stop();
+
+    for (int x = 0; x < Lx; x++) {
+      const int cellidx = y * Lx + x;
+      const CellDev& c = *rt[x].c;
+      const int Dl = rt[x].Dl, Dr = rt[x].Dr, npp = rt[x].npp;
+      const i64 per_m = (i64)c.nB * c.nCl * c.nA;
+      Tic t_c(h, &h->st.ms_search_cond);
+      DBuf<double> LG(h, (size_t)nb * npp * Dr), V(h, (size_t)nb * per_m);
+      k_hrow<<<cdiv(nb, 256), 256, 0, h->stream>>>(st_cur, ncell, nb, cellidx, x, ns, h->d_cells, hrow.p);
+      TN_LAUNCH_CHECK(h);
+      k_fc<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(c, drow.p + (size_t)x * nb_row, sl_cur, nb, fc.p);
+      TN_LAUNCH_CHECK(h);
+      {   // LG[m][pp][b''] = sum_b' Lv[m][b'] G[pp][b'][b'']
+        LdLv a{Lv_cur, ldLv};
+        LdGj b{rt[x].G, Dl, Dr};
+        StPlain e{LG.p, (i64)npp * Dr};
+        int Ng = npp * Dr;
+        dim3 grid(1, cdiv(nb, 64), cdiv(Ng, 64));
+        k_gemm<64, 64, 16, 2, 2, true, true, LdLv, LdGj, StPlain><<<grid, 128, 0, h->stream>>>(nb, Ng, Dl, 1, a, b, e);
+        TN_LAUNCH_CHECK(h);
+        h->st.flop_search += 2.0 * nb * (double)Ng * Dl;
+      }
+      {   // V[m][(b,cl)][a]
+        LdPA a{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
+        LdPB b{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r};
+        StPV e{V.p, c.BhS, c.wA, c.X, c.BvS, c.Yc, hrow.p, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
+        int Mg = c.nB * c.nCl, Ng = c.nA;
+        dim3 grid(nb, cdiv(Mg, 64), cdiv(Ng, 64));
+        k_gemm<64, 64, 16, 2, 2, true, true, LdPA, LdPB, StPV><<<grid, 128, 0, h->stream>>>(Mg, Ng, Dr, 1, a, b, e);
+        TN_LAUNCH_CHECK(h);
+        h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
+      }
+      k_beam_Z<<<nb, 256, 0, h->stream>>>(V.p, per_m, c.nA, c.nCl, fc.p, Z.p, nneg.p);
+      TN_LAUNCH_CHECK(h);
+      t_c.stop();
+      if (y == 0 && x == 0) {
+        double z0 = d2h(h, Z.p), ls0 = d2h(h, rt[0].ls);
+        if (!(z0 > 0.0) || !std::isfinite(z0)) tn_throw(TN_ERR_NUMERIC, "first-cell normaliser is %g", z0);
+        double lz = -h->beta * h->offset + std::log(z0) + ls0;
+        for (int yy = 1; yy < Ly; yy++) lz += h->lognorm[yy];
+        h->log_z = lz;
+        h->have_logz = true;
+        if (logz_only) {
+          for (auto& r : rt) { h->dfree(r.G); h->dfree(r.RM); h->dfree(r.ls); }
+          return;
+        }
+      }
+      // ---- selection
+      Tic t_s(h, &h->st.ms_search_select);
+      k_beam_scale<<<1, 256, 0, h->stream>>>(lp_cur, Z.p, nb, scale.p);
+      TN_LAUNCH_CHECK(h);
+      SelArgs sa{V.p, scale.p, c.wC, c.Bd, drow.p + (size_t)x * nb_row, sl_cur, c.Pi, per_m, nb, c.nA, c.nCl, c.nCh, c.n_i};
+      SelState s0;
+      memset(&s0, 0, sizeof(s0));
+      s0.want = (unsigned long long)M + 1;
+      TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
+      const int shifts[6] = {52, 40, 28, 16, 4, 0}, nbitsv[6] = {12, 12, 12, 12, 12, 4};
+      const i64 total = (i64)nb * per_m;
+      const int gsel = (int)std::min<i64>(148 * 8, (total + 255) / 256);
+      for (int pass = 0; pass < 6; pass++) {
+        k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, hist.p);
+        TN_LAUNCH_CHECK(h);
+        k_sel_resolve<<<1, 32, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, cap);
+        TN_LAUNCH_CHECK(h);
+        SelState cur = d2h(h, sel.p);
+        if (cur.done) break;
+      }
+      TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+      k_sel_collect<<<gsel, 256, 0, h->stream>>>(sa, sel.p, raw.p, count.p, cap);
+      TN_LAUNCH_CHECK(h);
+      unsigned ncand = std::min(d2h(h, count.p), cap);
+      if (ncand == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
+      unsigned np2 = 2;
+      while (np2 < ncand + 1) np2 <<= 1;   // at least one sentinel so that cand[M] exists when ncand <= M
+      while (np2 <= (unsigned)M) np2 <<= 1;
+      if (np2 > npad) np2 = npad;
+      k_sel_score<<<cdiv(np2, 256), 256, 0, h->stream>>>(sa, raw.p, ncand, np2, lp_cur, Z.p, ns, S, cand.p);
+      TN_LAUNCH_CHECK(h);
+      if (np2 <= 4096) {
+        k_bitonic_smem<<<1, 1024, np2 * sizeof(Cand), h->stream>>>(cand.p, np2);
+        TN_LAUNCH_CHECK(h);
+      } else {
+        for (unsigned k = 2; k <= np2; k <<= 1)
+          for (unsigned j = k >> 1; j > 0; j >>= 1) {
+            k_bitonic_step<<<cdiv(np2, 256), 256, 0, h->stream>>>(cand.p, np2, k, j);
+            TN_LAUNCH_CHECK(h);
+          }
+      }
+      const int nkeep = (int)std::min<unsigned>(ncand, (unsigned)M);
+      k_new_beam<<<nkeep, 128, 0, h->stream>>>(cand.p, nkeep, M, st_cur, st_nxt, ncell, cellidx, sl_cur, sl_nxt, lp_nxt,
+                                               LG.p, npp, Dr, ldLv, Lv_nxt, c.Pd, c.Po, c.n_o, ns, S, pd.p);
+      TN_LAUNCH_CHECK(h);
+      std::swap(st_cur, st_nxt); std::swap(lp_cur, lp_nxt); std::swap(Lv_cur, Lv_nxt); std::swap(sl_cur, sl_nxt);
+      nb = nkeep;
+      t_s.stop();
+    }
+    for (auto& r : rt) { h->dfree(r.G); h->dfree(r.RM); h->dfree(r.ls); }
+  }
+  // ---- outputs: logp is already sorted descending (selection order)
+  DBuf<int8_t> sp(h, (size_t)nb * h->n_spins);
+  DBuf<double> E(h, nb);
+  k_unpack<<<cdiv((i64)nb * h->n_spins, 256), 256, 0, h->stream>>>(st_cur, ncell, nb, h->n_spins, h->d_cell_of, h->d_bit_of, sp.p);
+  TN_LAUNCH_CHECK(h);
+  k_energy<<<cdiv(nb, 64), 64, 0, h->stream>>>(sp.p, nb, h->n_spins, h->n_edges, h->d_eu, h->d_ev, h->d_J, h->d_h, E.p);
+  TN_LAUNCH_CHECK(h);
+  TN_CUDA(cudaMemcpyAsync(states_out, sp.p, (size_t)nb * h->n_spins, cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaMemcpyAsync(energies, E.p, sizeof(double) * nb, cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaMemcpyAsync(logp_out, lp_cur, sizeof(double) * nb, cudaMemcpyDeviceToHost, h->stream));
+  double pdv = 0;
+  TN_CUDA(cudaMemcpyAsync(&pdv, pd.p, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  unsigned long long neg = 0;
+  TN_CUDA(cudaMemcpyAsync(&neg, nneg.p, sizeof(neg), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+  *n_out = nb;
+  if (log_pd_out) *log_pd_out = pdv;
+  h->st.negative_u += (int64_t)neg;
+}
+
+}  // namespace
+
+void search_logz(tn_handle* h) { run(h, 1, true, nullptr, nullptr, nullptr, nullptr, nullptr); }
+
+void search_run(tn_handle* h, int M, int* n_out, int8_t* states, double* energies, double* logp, double* log_pd) {
+  cudaEvent_t e0, e1;
+  TN_CUDA(cudaEventCreate(&e0)); TN_CUDA(cudaEventCreate(&e1));
+  TN_CUDA(cudaEventRecord(e0, h->stream));
+  try {
+    run(h, M, false, n_out, states, energies, logp, log_pd);
+  } catch (...) {
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    throw;
+  }
+  TN_CUDA(cudaEventRecord(e1, h->stream));
+  TN_CUDA(cudaEventSynchronize(e1));
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  h->st.ms_search += ms;
+}
+
+void energy_run(tn_handle* h, int n, const int8_t* states, double* energies) {
+  if (n == 0) return;
+  DBuf<int8_t> sp(h, (size_t)n * h->n_spins);
+  DBuf<double> E(h, n);
+  TN_CUDA(cudaMemcpyAsync(sp.p, states, (size_t)n * h->n_spins, cudaMemcpyHostToDevice, h->stream));
+  k_energy<<<cdiv(n, 64), 64, 0, h->stream>>>(sp.p, n, h->n_spins, h->n_edges, h->d_eu, h->d_ev, h->d_J, h->d_h, E.p);
+  TN_LAUNCH_CHECK(h);
+  TN_CUDA(cudaMemcpyAsync(energies, E.p, sizeof(double) * n, cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaStreamSynchronize(h->stream));
+}

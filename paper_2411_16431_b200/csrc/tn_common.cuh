@@ -1,0 +1,139 @@
+// Internal declarations shared by the translation units of libtn_b200.so.
+// Product code: never includes or links anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <string>
+#include <vector>
+#include <stdexcept>
+#include "../../include/tn.h"
+
+struct TnError {
+  int code;
+  std::string msg;
+};
+[[noreturn]] void tn_throw(int code, const char* fmt, ...);
+#define TN_CUDA(expr)                                                                      \
+  do {                                                                                     \
+    cudaError_t e__ = (expr);                                                              \
+    if (e__ != cudaSuccess)                                                                \
+      tn_throw(e__ == cudaErrorMemoryAllocation ? TN_ERR_OOM : TN_ERR_CUDA, "%s: %s (%s:%d)", \
+               #expr, cudaGetErrorString(e__), __FILE__, __LINE__);                        \
+  } while (0)
+
+typedef long long i64;
+
+// ---------------------------------------------------------------------------------------------
+// Per-cell tables (a1).  State spaces of a cell made of S sub-clusters A, B, C of n_s spins:
+//   a in [0,nA)   sub-cluster 0 (carries the horizontal legs),
+//   b in [0,nB)   the sub-cluster that carries the vertical legs (sub 1; for S == 1 it IS a),
+//   c = c_lo + nCl*c_hi  sub-cluster 2 (S == 3): c_lo carries dout, c_hi carries din,
+//   k = a*nCl + c_lo in [0,nK): the part of the state that indexes the horizontal MPO bonds.
+// Cell weight  w(a,b,c) = g(k,b) * wC[c_lo][c_hi],   g(k,b) = wA[a] * X[a>>tshift][b] * Yc[b][c_lo].
+// ---------------------------------------------------------------------------------------------
+struct CellDev {
+  int nA, nB, nT, nCl, nCh, nK, tshift;
+  int n_l, n_r, n_u, n_d, n_i, n_o;   // projector ranges (Eq. (5))
+  int bh_rows, bv_rows, bd_rows;      // rows of the incoming edge matrices (ranges of the neighbours)
+  int m_left, m_right, m_din, m_dout; // coupled-bit masks (m_din relative to the hi half)
+  const double *wA, *X, *Yc, *wC;     // [nA] [nT*nB] [nB*nCl] [nCl*nCh]
+  const int *Pl, *Pr, *Pu, *Pd, *Pi, *Po;  // [nA] [nA] [nB] [nB] [nCh] [nCl]
+  const double *Bh, *Bv, *Bd;         // [bh_rows*n_l] [bv_rows*n_u] [bd_rows*n_i]
+  const double *BhS, *BvS;            // [bh_rows*nA] [bv_rows*nB]  (columns expanded to states)
+};
+
+struct MpsTensor {
+  double* d = nullptr;
+  int dl = 1, p = 1, dr = 1;
+};
+
+struct Timer {
+  cudaEvent_t a = nullptr, b = nullptr;
+};
+
+struct tn_handle {
+  // instance
+  int n_spins = 0;
+  i64 n_edges = 0;
+  int Ly = 0, Lx = 0, S = 0, ns = 0;
+  std::vector<int> edge_u, edge_v, cell_of, bit_of;   // bit_of: sub*ns+pos
+  std::vector<double> J, h;
+  int *d_eu = nullptr, *d_ev = nullptr, *d_cell_of = nullptr, *d_bit_of = nullptr;
+  double *d_J = nullptr, *d_h = nullptr;
+  // table build inputs
+  void* d_cell_edges = nullptr;
+  int* d_cell_edge_ptr = nullptr;
+  void* d_cell_desc = nullptr;
+  // tables
+  std::vector<CellDev> cells;   // host copy of the descriptors (pointers are device pointers)
+  CellDev* d_cells = nullptr;
+  double* pool_d = nullptr;
+  int* pool_i = nullptr;
+  double* d_offsets = nullptr;
+  double beta = 0, offset = 0;
+  bool have_beta = false, have_mps = false;
+  // boundary MPS: rows[y] for y = 1..Ly (rows[Ly] trivial)
+  std::vector<std::vector<MpsTensor>> rows;
+  std::vector<double> lognorm;
+  double log_z = 0;
+  bool have_logz = false;
+  int D = 0, sweeps = 0;
+  // options
+  int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512;
+  double svd_tol = 1e-11;
+  // runtime
+  cudaStream_t stream = nullptr;
+  void* (*alloc_cb)(size_t, void*) = nullptr;
+  void (*free_cb)(void*, void*) = nullptr;
+  void* alloc_ctx = nullptr;
+  i64 bytes_held = 0;
+  struct Block { void* p; size_t bytes; int src; };   // src: 0 cudaMalloc, 1 allocator callback
+  std::vector<Block> live, cached;
+  tn_stats st;
+  cudaEvent_t ev[2] = {nullptr, nullptr};
+
+  void* dmalloc(size_t bytes);
+  void dfree(void* p);
+  template <class T>
+  T* dalloc(size_t n) { return (T*)dmalloc(n * sizeof(T) + 16); }
+  const CellDev& cell(int y, int x) const { return cells[(size_t)y * Lx + x]; }
+  bool has_med() const { return S == 3; }
+};
+
+// simple scoped device buffer
+template <class T>
+struct DBuf {
+  tn_handle* h;
+  T* p = nullptr;
+  size_t n = 0;
+  DBuf(tn_handle* h_, size_t n_) : h(h_), n(n_) { p = h->dalloc<T>(n_ ? n_ : 1); }
+  ~DBuf() { if (p) h->dfree(p); }
+  DBuf(const DBuf&) = delete;
+  DBuf& operator=(const DBuf&) = delete;
+  DBuf(DBuf&& o) : h(o.h), p(o.p), n(o.n) { o.p = nullptr; }
+  T* release() { T* q = p; p = nullptr; return q; }
+};
+
+struct StageTimer {   // accumulates GPU milliseconds of a stage into a stats field (syncs at stop)
+  tn_handle* h;
+  double* dst;
+  cudaEvent_t a, b;
+  StageTimer(tn_handle* h_, double* dst_);
+  ~StageTimer();
+};
+
+// ---- tables.cu
+void tables_create(tn_handle* h);          // host preprocessing + device layout (tn_create)
+void tables_set_beta(tn_handle* h, double beta);
+void tables_destroy(tn_handle* h);
+// ---- contract.cu
+void contract_run(tn_handle* h, int D, int sweeps);
+void mps_free(tn_handle* h);
+// ---- search.cu
+void search_logz(tn_handle* h);
+void search_run(tn_handle* h, int M, int* n_out, int8_t* states, double* energies, double* logp,
+                double* log_pd);
+void energy_run(tn_handle* h, int n, const int8_t* states, double* energies);

@@ -1,0 +1,140 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): log Z and log-marginals 1e-9 relative at exact D, 1e-6 relative at
+truncated D; bitstrings identical wherever the oracle's logp gaps exceed the tolerance; energies bit-exact
+with the oracle's fixed-order recomputation (O-0)."""
+import numpy as np
+import pytest
+
+import instances
+from oracle import energy, model, mps, search
+
+pytestmark = pytest.mark.gpu
+
+
+def _tn(inst):
+    import paper_2411_16431_b200 as tnb
+    return tnb.TensorNetwork(inst)
+
+
+def mps_overlap(A, B):
+    """<A|B> / (|A| |B|) for two MPS given as lists of [dl, p, dr] arrays."""
+    def inner(X, Y):
+        E = np.ones((1, 1))
+        for x, y in zip(X, Y):
+            E = np.einsum("ab,apc,bpd->cd", E, x, y, optimize=True)
+        return E[0, 0]
+    return inner(A, B) / np.sqrt(inner(A, A) * inner(B, B))
+
+
+def run_oracle(inst, beta, D, sweeps, M):
+    m = model.Model(inst).set_beta(beta)
+    R, ln = mps.contract(m, D, sweeps)
+    out = search.branch_and_bound(m, R, ln, M)
+    return m, R, ln, out
+
+
+def compare(inst, beta, D, sweeps, M, tol, check_rows=True):
+    m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M)
+    with _tn(inst) as t:
+        t.set_beta(beta)
+        t.contract(D, sweeps)
+        if check_rows:
+            for y in range(inst.Ly - 1, 0, -1):
+                ov = mps_overlap(R[y], t.mps(y))
+                assert abs(1 - abs(ov)) <= max(tol * 1e-1, 1e-12), (y, ov)
+                # (row log-norms are not comparable: the two sides shift their local tables by different
+                #  minima, per factor here vs per cell in the oracle; the total enters log Z below)
+                assert np.isfinite(t.row_lognorm(y))
+        lz = t.log_z()
+        assert abs(lz - ref["log_z"]) <= tol * abs(ref["log_z"]), (lz, ref["log_z"])
+        states, E, logp, pd = t.branch_and_bound(M)
+        st = t.stats()
+    n = ref["logp"].size
+    assert states.shape[0] == n
+    assert np.allclose(logp, ref["logp"], rtol=tol, atol=0), np.abs(logp - ref["logp"]).max()
+    # energies: bit-exact with the oracle's fixed-order recomputation of the SAME states
+    assert np.array_equal(E, energy.energies(inst, states))
+    # bitstrings identical rank by rank wherever the oracle's adjacent logp gaps exceed the tolerance
+    lp = ref["logp"]
+    gap_tol = 10 * tol * np.abs(lp).max()
+    for r in range(n):
+        lo = r == 0 or lp[r - 1] - lp[r] > gap_tol
+        hi = r == n - 1 or lp[r] - lp[r + 1] > gap_tol
+        if lo and hi:
+            assert np.array_equal(states[r], ref["states"][r]), r
+    if np.isfinite(ref["log_pd"]):
+        assert abs(pd - ref["log_pd"]) <= 10 * tol * abs(ref["log_pd"]), (pd, ref["log_pd"])
+    else:
+        assert pd == ref["log_pd"]
+    return st
+
+
+EXACT = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, M)
+    (2, 2, 3, 2, 0.8, 3, 1.3, 8),
+    (3, 2, 2, 2, 0.9, 5, 0.7, 8),
+    (2, 3, 1, 4, 1.0, 1, 1.5, 16),
+    (2, 3, 2, 2, 0.9, 7, 0.9, 8),
+    (3, 3, 3, 2, 0.85, 7, 0.9, 32),
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,M", EXACT)
+def test_exact_contraction_parity(Ly, Lx, S, ns, p, seed, beta, M):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    compare(inst, beta, 0, 0, M, 1e-9)
+
+
+def test_config1_parity():
+    inst, run = instances.config(0)
+    compare(inst, run["beta"][0], run["D"], run["sweeps"], run["M"], 1e-9)
+
+
+TRUNC = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M)
+    (3, 4, 2, 2, 0.9, 3, 0.9, 3, 0, 16),
+    (3, 4, 2, 2, 0.9, 3, 0.9, 3, 1, 16),
+    (3, 4, 2, 2, 0.9, 3, 0.9, 3, 2, 16),
+    (4, 4, 2, 4, 0.95, 2, 1.0, 6, 1, 64),      # Zephyr-shaped miniature: 256 states per cell, ragged projectors
+    (3, 3, 3, 4, 0.9, 4, 1.0, 6, 2, 64),       # Pegasus-shaped miniature: 4096 states per cell, mediating tensors
+    (4, 3, 3, 2, 0.85, 9, 1.5, 4, 3, 32),
+    (3, 3, 1, 4, 1.0, 6, 2.0, 5, 1, 16),
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,D,sweeps,M", TRUNC)
+def test_truncated_contraction_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    compare(inst, beta, D, sweeps, M, 1e-6)
+
+
+def test_zero_field_z2_instance():
+    inst = instances.lattice(3, 3, 2, 4, p_keep=1.0, seed=21, h="zero")
+    compare(inst, 2.0, 8, 1, 32, 1e-6)
+
+
+def test_energy_kernel_bit_exact():
+    inst = instances.lattice(3, 3, 3, 4, p_keep=0.9, seed=11)
+    rng = np.random.default_rng(0)
+    s = (1 - 2 * rng.integers(0, 2, size=(37, inst.n_spins))).astype(np.int8)
+    with _tn(inst) as t:
+        assert np.array_equal(t.energy(s), energy.energies(inst, s))
+
+
+def test_error_codes():
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(2, 2, 2, 2, seed=1)
+    with _tn(inst) as t:
+        with pytest.raises(tnb.TnError) as e:
+            t.contract(4, 1)
+        assert e.value.code == -3          # TN_ERR_STATE: contract before set_beta
+        t.set_beta(1.0)
+        with pytest.raises(tnb.TnError) as e:
+            t.branch_and_bound(4)
+        assert e.value.code == -3
+    bad = instances.Instance(inst)
+    bad["edge_u"] = np.append(inst.edge_u, 0).astype(np.int32)
+    bad["edge_v"] = np.append(inst.edge_v, inst.n_spins - 1).astype(np.int32)   # cell (0,0) -- (1,1) on S = 2
+    bad["J"] = np.append(inst.J, 1.0)
+    with pytest.raises(tnb.TnError) as e:
+        tnb.TensorNetwork(bad)
+    assert e.value.code == -2              # TN_ERR_GEOMETRY
