@@ -85,8 +85,8 @@ typedef struct {
   double flop_theta_apply;   /* algorithmic FLOP of the skinny GEMMs                        */
   double bytes_theta_apply;  /* algorithmic bytes of the skinny GEMMs (one read of Theta)    */
   double flop_search;        /* algorithmic FLOP of the search GEMMs                        */
-  double min_sigma_rel;      /* max over bonds of (smallest retained sigma / sigma_1), Fig. 12(b)
-                                PAPER.md:306                                                 */
+  double min_sigma_rel;      /* max over the truncated bonds of (smallest retained sigma / sigma_1):
+                                the worst cut of Fig. 12(b); 0 if nothing was cut */
   int64_t svd_iterations;    /* total block-subspace iterations                             */
   int64_t kernel_launches;   /* kernels launched by this library                            */
   int64_t negative_u;        /* conditionals clamped to 0 (reading S7)         */

@@ -206,13 +206,21 @@ def truncate_rank(s, D, gap_guard=True):
 
 def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
     """R_y = compress(T_y R_{y+1}; D, sweeps).  A: tensors of R_{y+1} (any gauge).
-    Returns (tensors of R_y with unit norm, log of the norm removed)."""
+    Returns (tensors of R_y with unit norm, log of the norm removed).
+
+    Range (reading S19): the norm of a row is exp(-O(beta N_row)) and under/overflows fp64 on
+    the large lattices, so every environment is kept at O(1) and the positive scale removed from it is
+    carried as a logarithm: the zipper connector is divided by sigma_1 of each step, the variational
+    environments by their Frobenius norm; lsR[j] / lsL[j] are the logs of what was removed from
+    Renv[j] / Lenv[j].  Positive rescalings change nothing but the bookkeeping."""
     n = len(positions)
     A, r_last = left_canonicalize(A)
     Renv = [None] * n
+    lsR = [0.0] * n
     Renv[n - 1] = np.full((1, 1, 1), r_last)       # trivial unity connector x the folded norm
     N = [None] * n
     min_sigma = []
+    ls0 = 0.0
     for j in range(n - 1, -1, -1):                  # C-2 zipper, right -> left
         pos = positions[j]
         Th = pos.theta(A[j], Renv[j])
@@ -220,36 +228,50 @@ def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
         k = truncate_rank(s, D, gap_guard)
         min_sigma.append(s[k - 1] / s[0] if s[0] > 0 else 0.0)
         N[j] = Vt[:k].reshape(k, pos.pu, Renv[j].shape[0])
-        Cn = (U[:, :k] * s[:k]).reshape(A[j].shape[0], pos.wl, k)
+        scale = s[0] if s[0] > 0 else 1.0
+        Cn = (U[:, :k] * (s[:k] / scale)).reshape(A[j].shape[0], pos.wl, k)
         if j > 0:
             Renv[j - 1] = Cn.transpose(2, 1, 0)
+            lsR[j - 1] = lsR[j] + np.log(scale)
+        else:
+            ls0 = lsR[0] + np.log(scale)
     assert Cn.shape == (1, 1, 1)
     centre = 0
     N[0] = N[0] * Cn[0, 0, 0]
+    lsL = [0.0] * n
+    log_centre = ls0                                # log of the scale carried beside N[centre]
     norms = []
-    if D > 0:                                       # C-5: exact mode skips the passes
+    if D > 0 and sweeps > 0:                        # C-5: exact mode skips the passes
         Lenv = [None] * n
         Lenv[0] = np.ones((1, 1, 1))
         for sweep in range(sweeps):                 # C-4
             if sweep % 2 == 0:
                 for j in range(n):
                     N[j] = positions[j].update(Lenv[j], A[j], Renv[j])
-                    norms.append(np.linalg.norm(N[j]))
+                    log_centre = lsL[j] + lsR[j]
+                    norms.append(np.linalg.norm(N[j]) * np.exp(log_centre))
                     if j + 1 < n:
                         g, p, g2 = N[j].shape
                         Q, _ = np.linalg.qr(N[j].reshape(g * p, g2))
                         N[j] = Q.reshape(g, p, Q.shape[1])
-                        Lenv[j + 1] = positions[j].env_left(Lenv[j], A[j], N[j])
+                        E = positions[j].env_left(Lenv[j], A[j], N[j])
+                        nE = np.linalg.norm(E)
+                        Lenv[j + 1] = E / nE
+                        lsL[j + 1] = lsL[j] + np.log(nE)
                 centre = n - 1
             else:
                 for j in range(n - 1, -1, -1):
                     N[j] = positions[j].update(Lenv[j], A[j], Renv[j])
-                    norms.append(np.linalg.norm(N[j]))
+                    log_centre = lsL[j] + lsR[j]
+                    norms.append(np.linalg.norm(N[j]) * np.exp(log_centre))
                     if j > 0:
                         g, p, g2 = N[j].shape
                         Q, _ = np.linalg.qr(N[j].reshape(g, p * g2).T)
                         N[j] = Q.T.reshape(Q.shape[1], p, g2)
-                        Renv[j - 1] = positions[j].env_right(Renv[j], A[j], N[j])
+                        E = positions[j].env_right(Renv[j], A[j], N[j])
+                        nE = np.linalg.norm(E)
+                        Renv[j - 1] = E / nE
+                        lsR[j - 1] = lsR[j] + np.log(nE)
                 centre = 0
     nrm = np.linalg.norm(N[centre])
     N[centre] = N[centre] / nrm
@@ -257,7 +279,7 @@ def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
         stats.setdefault("min_sigma", []).append(min(min_sigma))
         stats.setdefault("pass_norms", []).append(norms)
         stats.setdefault("bonds", []).append([t.shape[2] for t in N])
-    return N, float(np.log(nrm))
+    return N, float(np.log(nrm) + log_centre)
 
 
 def contract(model, D, sweeps, gap_guard=True, stats=None):

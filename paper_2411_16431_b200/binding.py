@@ -188,8 +188,10 @@ class TensorNetwork:
             try:
                 import torch
                 if torch.cuda.is_available():
-                    alloc = ALLOC_FN(lambda n, ctx: torch.cuda.caching_allocator_alloc(n))
-                    free_ = FREE_FN(lambda p, ctx: torch.cuda.caching_allocator_delete(p))
+                    t_alloc = torch.cuda.caching_allocator_alloc      # bound now: module attributes are
+                    t_free = torch.cuda.caching_allocator_delete      # gone at interpreter shutdown
+                    alloc = ALLOC_FN(lambda n, ctx: t_alloc(n))
+                    free_ = FREE_FN(lambda p, ctx: t_free(p))
                     self._cb = (alloc, free_)
                     tn_set_allocator(self.handle, alloc, free_)
                     tn_set_stream(self.handle, torch.cuda.current_stream().cuda_stream)

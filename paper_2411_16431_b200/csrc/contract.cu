@@ -210,18 +210,28 @@ __global__ void k_rank_decide(const double* sig, int ks, int chi, int gap_guard,
   int k = 0;
   if (s0 > 0.0)
     for (int i = 0; i < ks; i++) k += sig[i] > 1e-14 * s0 ? 1 : 0;
+  bool cut = false;
   if (k > chi) {
+    cut = true;
     k = chi;
     if (gap_guard)
       while (k > 1 && sig[k] >= (1.0 - 1e-6) * sig[k - 1]) k--;
   }
   if (k < 1) k = 1;
   *keep = k;
-  stat[1] = s0 > 0.0 ? sig[k - 1] / s0 : 0.0;   // candidate for the running max, committed at convergence
+  stat[1] = (cut && s0 > 0.0) ? sig[k - 1] / s0 : 0.0;   // only bonds that really truncate; committed at convergence
 }
 __global__ void k_commit_stat(double* stat) {
   if (threadIdx.x || blockIdx.x) return;
   stat[0] = fmax(stat[0], stat[1]);
+}
+// Range bookkeeping (reading S19): *safe = (*s > 0 ? *s : 1), *ls_out = (ls_in ? *ls_in : 0) + log(*safe)
+__global__ void k_ls_step(const double* s, const double* ls_in, double* ls_out, double* safe) {
+  if (threadIdx.x || blockIdx.x) return;
+  double v = *s;
+  if (!(v > 0.0) || !isfinite(v)) v = 1.0;
+  *safe = v;
+  *ls_out = (ls_in ? *ls_in : 0.0) + log(v);
 }
 // partial column sums of squares of (P - Q), both [m x k]
 __global__ void k_coldiff_part(const double* P, const double* Q, i64 m, int k, int rows_per_block, double* part) {
@@ -251,7 +261,7 @@ __global__ void k_resid_flag(const double* part, int nblk, int k, const int* kee
 }
 
 // Outputs: Vz [n x chi] leading right singular vectors, C [m x chi] = Theta Vz; columns >= keep are zero.
-void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* C) {
+void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* C, double* sig0_out) {
   tn_handle* h = cx.h;
   const i64 m = op.m, n = op.n;
   DBuf<double> Om(h, (size_t)n * ks), Z(h, (size_t)n * ks), Ya(h, (size_t)m * ks), Yb(h, (size_t)m * ks);
@@ -303,6 +313,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
   gemm_rm(h, false, true, (int)n, ks, ks, Om.p, ks, Wt.p, ks, Z.p, ks);        // V = Omega W
   permute3(h, Vz, Z.p, 1, (int)n, chi, 0, ks, 1, 2, cx.d_keep);
   permute3(h, C, TV.p, 1, (int)m, chi, 0, ks, 1, 2, cx.d_keep);
+  TN_CUDA(cudaMemcpyAsync(sig0_out, sig.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
 }
 
 MpsTensor new_tensor(tn_handle* h, int dl, int p, int dr) {
@@ -360,6 +371,12 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
   // ---- C-2/C-3: zipper right -> left
   std::vector<double*> Renv(n, nullptr), Lenv(n, nullptr);
   std::vector<MpsTensor> N(n);
+  // log-scales removed from the environments: lsR[j] = ls[j], lsL[j] = ls[n + j], ls0 = ls[2n] (reading S19)
+  DBuf<double> lsbuf(h, 2 * (size_t)n + 2);
+  double* ls = lsbuf.p;
+  TN_CUDA(cudaMemsetAsync(ls, 0, sizeof(double) * (2 * (size_t)n + 2), h->stream));
+  double* d_sig0 = cx.d_scal + 1;
+  double* d_safe = cx.d_scal + 2;
   Renv[n - 1] = h->dalloc<double>(1);
   TN_CUDA(cudaMemcpyAsync(Renv[n - 1], rlast.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
   for (int j = n - 1; j >= 0; j--) {
@@ -369,9 +386,13 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
                          : (int)std::min<i64>((i64)chi[j] + h->oversample, std::min(op.m, op.n));
     DBuf<double> Vz(h, (size_t)op.n * chi[j]);
     double* C = h->dalloc<double>((size_t)op.m * chi[j]);
-    svd_trunc(cx, op, chi[j], ks, Vz.p, C);
+    svd_trunc(cx, op, chi[j], ks, Vz.p, C, d_sig0);
     N[j] = new_tensor(h, chi[j], pos[j].pu, g);
     permute3(h, N[j].d, Vz.p, chi[j], pos[j].pu, g, 1, (i64)g * chi[j], chi[j]);
+    // connector <- connector / sigma_1, log sigma_1 carried beside it
+    k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + j, j > 0 ? ls + j - 1 : ls + 2 * n, d_safe);
+    TN_LAUNCH_CHECK(h);
+    scale_by(h, C, op.m * chi[j], d_safe, true);
     if (j > 0) {
       Renv[j - 1] = C;
     } else {
@@ -399,6 +420,10 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
             if (Lenv[j + 1]) h->dfree(Lenv[j + 1]);
             Lenv[j + 1] = h->dalloc<double>((size_t)op.m * s);
             apply_N(cx, op, Z.p, Lenv[j + 1], s);
+            frob_norm(h, Lenv[j + 1], op.m * s, d_sig0);
+            k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + n + j, ls + n + j + 1, d_safe);
+            TN_LAUNCH_CHECK(h);
+            scale_by(h, Lenv[j + 1], op.m * s, d_safe, true);
           }
           permute3(h, N[j].d, Z.p, g, pos[j].pu, s, s, (i64)g * s, 1);
           free_op(cx, op);
@@ -417,6 +442,10 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
             h->dfree(Renv[j - 1]);
             Renv[j - 1] = h->dalloc<double>((size_t)op.m * s);
             apply_N(cx, op, Z.p, Renv[j - 1], s);
+            frob_norm(h, Renv[j - 1], op.m * s, d_sig0);
+            k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + j, ls + j - 1, d_safe);
+            TN_LAUNCH_CHECK(h);
+            scale_by(h, Renv[j - 1], op.m * s, d_safe, true);
           }
           permute3(h, N[j].d, Z.p, s, pos[j].pu, g, 1, (i64)g * s, s);
           free_op(cx, op);
@@ -430,10 +459,14 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
   frob_norm(h, N[centre].d, nc, cx.d_scal);
   scale_by(h, N[centre].d, nc, cx.d_scal, true);
   double nrm = 0.0;
+  std::vector<double> lsh(2 * (size_t)n + 2);
   TN_CUDA(cudaMemcpyAsync(&nrm, cx.d_scal, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaMemcpyAsync(lsh.data(), ls, sizeof(double) * lsh.size(), cudaMemcpyDeviceToHost, h->stream));
   TN_CUDA(cudaStreamSynchronize(h->stream));
   if (!(nrm > 0.0) || !std::isfinite(nrm)) tn_throw(TN_ERR_NUMERIC, "row %d: boundary MPS norm is %g", y, nrm);
-  *lognorm = std::log(nrm);
+  const bool swept = !exact && sweeps > 0;
+  *lognorm = std::log(nrm) + (swept ? lsh[centre] + lsh[n + centre] : lsh[2 * (size_t)n]);
+  if (!std::isfinite(*lognorm)) tn_throw(TN_ERR_NUMERIC, "row %d: log-norm is not finite", y);
   for (int j = 0; j < n; j++) {
     h->dfree(A[j].d);
     if (Renv[j]) h->dfree(Renv[j]);
