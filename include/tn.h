@@ -92,6 +92,8 @@ typedef struct {
   int64_t negative_u;        /* conditionals clamped to 0 (reading S7)         */
   int64_t rows_contracted;   /* boundary-MPS rows built                                      */
   int64_t bytes_device;      /* device bytes currently held                                  */
+  int64_t jacobi_calls;      /* one-sided Jacobi kernel launches                             */
+  int64_t jacobi_sweeps;     /* total Jacobi sweeps over all calls                           */
 } tn_stats;
 
 /* tn_create: validates the geometry and copies the instance to the device.
@@ -149,6 +151,11 @@ int tn_get_stats(tn_handle*, tn_stats* out /* HOST */);
 
 /* tn_energy: O-0 fixed-order energies of n given states (HOST int8 [n][n_spins]) on the device. */
 int tn_energy(tn_handle*, int32_t n, const int8_t* states, double* energies /* HOST [n] */);
+
+/* tn_fp64_peak: measured FP64 tensor-core (mma.sync m8n8k4 f64 = SASS DMMA) peak of the current device
+ * in TFLOP/s, from a register-resident chain (about 10 ms); the roofline denominator of the GEMM stages
+ * ("FP64 tensor peak to be measured first").  Needs no handle. */
+int tn_fp64_peak(double* tflops /* HOST */);
 
 const char* tn_last_error(void);
 void tn_destroy(tn_handle*);

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_energy", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_energy", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP = 1, 2, 3, 4, 5
 
 
@@ -26,7 +26,8 @@ class TnStats(C.Structure):
         "ms_tables", "ms_contract", "ms_theta_build", "ms_theta_apply", "ms_orth_svd", "ms_search",
         "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
         "bytes_theta_apply", "flop_search", "min_sigma_rel")] + [(n, C.c_int64) for n in (
-            "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device")]
+            "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
+            "jacobi_sweeps")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -60,6 +61,7 @@ def lib():
         L.tn_branch_and_bound.argtypes = [C.c_void_p, C.c_int32, p_i32, p_i8, p_f64, p_f64, p_f64]
         L.tn_get_stats.argtypes = [C.c_void_p, C.POINTER(TnStats)]
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
+        L.tn_fp64_peak.argtypes = [p_f64]
         L.tn_last_error.restype = C.c_char_p
         L.tn_destroy.argtypes = [C.c_void_p]
         L.tn_destroy.restype = None
@@ -162,6 +164,14 @@ def tn_energy(handle, states):
     out = np.empty(s.shape[0], dtype=np.float64)
     _check(lib().tn_energy(handle, s.shape[0], _ptr(s, C.c_int8), _ptr(out, C.c_double)))
     return out
+
+
+def tn_fp64_peak() -> float:
+    v = C.c_double()
+    rc = lib().tn_fp64_peak(C.byref(v))
+    if rc != 0:
+        raise TnError(rc, "tn_fp64_peak failed (no CUDA device?)")
+    return v.value
 
 
 def tn_get_stats(handle) -> dict:

@@ -224,6 +224,7 @@ int tn_set_beta(tn_handle* h, double beta) {
   if (!std::isfinite(beta) || beta < 0.0) tn_throw(TN_ERR_ARG, "beta must be finite and >= 0");
   mps_free(h);
   memset(&h->st, 0, sizeof(h->st));
+  if (h->d_cnt) TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
   tables_set_beta(h, beta);
   h->have_beta = true;
   TN_API_END
@@ -318,6 +319,13 @@ int tn_get_stats(tn_handle* h, tn_stats* out) {
   if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");
   *out = h->st;
   out->bytes_device = h->bytes_held;
+  if (h->d_cnt) {
+    unsigned long long c[2] = {0, 0};
+    TN_CUDA(cudaMemcpyAsync(c, h->d_cnt, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaStreamSynchronize(h->stream));
+    out->jacobi_calls = (int64_t)c[0];
+    out->jacobi_sweeps = (int64_t)c[1];
+  }
   TN_API_END
 }
 
@@ -328,7 +336,7 @@ void tn_destroy(tn_handle* h) {
     mps_free(h);
     tables_destroy(h);
     for (void* p : {(void*)h->d_eu, (void*)h->d_ev, (void*)h->d_J, (void*)h->d_h, (void*)h->d_cell_of,
-                    (void*)h->d_bit_of})
+                    (void*)h->d_bit_of, (void*)h->d_cnt})
       if (p) h->dfree(p);
     trim_free_list(h);
     for (auto& l : h->live) raw_free(h, l);

@@ -177,7 +177,8 @@ void frob_norm(tn_handle* h, const double* X, i64 n, double* out) {
 // ============================================================================================
 // Working storage: Mw [c x r] (ldm), Ww [c x c].  Round-robin pair ordering; each warp owns a pair.
 __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld, int c, int r, double* Mout,
-                                                      double* Wt, double* sig, double* gwork, int use_smem) {
+                                                      double* Wt, double* sig, double* gwork, int use_smem,
+                                                      unsigned long long* cnt) {
   extern __shared__ double sm[];
   __shared__ int s_rot;
   __shared__ double s_norm[1024];   // c <= 1024
@@ -186,6 +187,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
   double* Ww = Mw + (size_t)c * r;
   for (int i = tid; i < c * r; i += blockDim.x) Mw[i] = Min[(size_t)(i / r) * ld + (i % r)];
   for (int i = tid; i < c * c; i += blockDim.x) Ww[i] = (i / c == i % c) ? 1.0 : 0.0;
+  if (tid == 0 && cnt) cnt[0]++;
   __syncthreads();
   const int ce = c + (c & 1);
   const double tol = 1e-15;
@@ -236,6 +238,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
       }
       int rot = s_rot;
       __syncthreads();
+      if (tid == 0 && cnt) cnt[1]++;
       if (!rot) break;
     }
   }
@@ -271,12 +274,16 @@ void jacobi_rows(tn_handle* h, const double* Min, int ld, int c, int r, double* 
     TN_CUDA(cudaFuncSetAttribute(k_jacobi_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     attr_set = true;
   }
+  if (!h->d_cnt) {
+    h->d_cnt = h->dalloc<unsigned long long>(2);
+    TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
+  }
   if (need <= 200 * 1024) {
-    k_jacobi_rows<<<1, 1024, need, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, nullptr, 1);
+    k_jacobi_rows<<<1, 1024, need, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, nullptr, 1, h->d_cnt);
     TN_LAUNCH_CHECK(h);
   } else {
     double* work = h->dalloc<double>((size_t)c * r + (size_t)c * c);
-    k_jacobi_rows<<<1, 1024, 0, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, work, 0);
+    k_jacobi_rows<<<1, 1024, 0, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, work, 0, h->d_cnt);
     TN_LAUNCH_CHECK(h);
     h->dfree(work);
   }

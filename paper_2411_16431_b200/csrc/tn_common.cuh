@@ -94,6 +94,7 @@ struct tn_handle {
   std::vector<Block> live, cached;
   tn_stats st;
   cudaEvent_t ev[2] = {nullptr, nullptr};
+  unsigned long long* d_cnt = nullptr;   // device counters: [0] Jacobi calls, [1] Jacobi sweeps
 
   void* dmalloc(size_t bytes);
   void dfree(void* p);
