@@ -152,6 +152,15 @@ int tn_get_stats(tn_handle*, tn_stats* out /* HOST */);
 /* tn_energy: O-0 fixed-order energies of n given states (HOST int8 [n][n_spins]) on the device. */
 int tn_energy(tn_handle*, int32_t n, const int8_t* states, double* energies /* HOST [n] */);
 
+/* tn_kernel_check: diagnostic -- runs ONE device building block of the path on host data (kernel-level parity
+ * tests call it; it is not a step of the path).  A, B, C are HOST row-major fp64.
+ *   op = TN_CHECK_ORTH   : C [m x k] = orthonormalised columns of A [m x k] (a3: QR canonicalisation; n, B unused)
+ *   op = TN_CHECK_GEMM_N : C [m x n] = A [m x k] . B [k x n]    (a2: Theta-core x skinny apply)
+ *   op = TN_CHECK_GEMM_T : C [k x n] = A^T . B,  A [m x k], B [m x n]   (a2: Theta-core^T x skinny apply) */
+enum { TN_CHECK_ORTH = 1, TN_CHECK_GEMM_N = 2, TN_CHECK_GEMM_T = 3 };
+int tn_kernel_check(tn_handle*, int32_t op, int64_t m, int32_t n, int32_t k, const double* A, const double* B,
+                    double* C);
+
 /* tn_fp64_peak: measured FP64 tensor-core (mma.sync m8n8k4 f64 = SASS DMMA) peak of the current device
  * in TFLOP/s, from a register-resident chain (about 10 ms); the roofline denominator of the GEMM stages
  * ("FP64 tensor peak to be measured first").  Needs no handle. */

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_energy", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP = 1, 2, 3, 4, 5
 
 
@@ -62,6 +62,7 @@ def lib():
         L.tn_get_stats.argtypes = [C.c_void_p, C.POINTER(TnStats)]
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
         L.tn_fp64_peak.argtypes = [p_f64]
+        L.tn_kernel_check.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, p_f64, p_f64, p_f64]
         L.tn_last_error.restype = C.c_char_p
         L.tn_destroy.argtypes = [C.c_void_p]
         L.tn_destroy.restype = None
@@ -163,6 +164,25 @@ def tn_energy(handle, states):
         s = s[None, :]
     out = np.empty(s.shape[0], dtype=np.float64)
     _check(lib().tn_energy(handle, s.shape[0], _ptr(s, C.c_int8), _ptr(out, C.c_double)))
+    return out
+
+
+CHECK_ORTH, CHECK_GEMM_N, CHECK_GEMM_T = 1, 2, 3
+
+
+def tn_kernel_check(handle, op, A, B=None):
+    """Diagnostic: one device building block on host data (see include/tn.h)."""
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    m, k = A.shape
+    if op == CHECK_ORTH:
+        n, out, Bp = 1, np.empty((m, k)), None
+    else:
+        B = np.ascontiguousarray(B, dtype=np.float64)
+        n = B.shape[1]
+        out = np.empty((m, n) if op == CHECK_GEMM_N else (k, n))
+        Bp = _ptr(B, C.c_double)
+    _check(lib().tn_kernel_check(handle, int(op), int(m), int(n), int(k), _ptr(A, C.c_double), Bp,
+                                 _ptr(out, C.c_double)))
     return out
 
 

@@ -314,6 +314,16 @@ int tn_energy(tn_handle* h, int32_t n, const int8_t* states, double* energies) {
   TN_API_END
 }
 
+int tn_kernel_check(tn_handle* h, int32_t op, int64_t m, int32_t n, int32_t k, const double* A, const double* B,
+                    double* Cout) {
+  TN_API_BEGIN
+  if (!h || !A || !Cout || m < 1 || n < 1 || k < 1) tn_throw(TN_ERR_ARG, "bad argument");
+  need_device();
+  kernel_check_run(h, op, m, n, k, A, B, Cout);
+  trim_free_list(h);
+  TN_API_END
+}
+
 int tn_get_stats(tn_handle* h, tn_stats* out) {
   TN_API_BEGIN
   if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");

@@ -299,7 +299,7 @@ __global__ void k_svqb_T(const double* Wt, const double* sig, int k, double* T) 
   T[t] = Wt[(size_t)j * k + i] * sc;
 }
 
-void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes) {
+void orth_columns_jacobi(tn_handle* h, double* Y, i64 m, int k, int passes) {
   if (m <= 0 || k <= 0) return;
   DBuf<double> G(h, (size_t)k * k), Go(h, (size_t)k * k), Wt(h, (size_t)k * k), T(h, (size_t)k * k), sig(h, k);
   DBuf<double> Y2(h, (size_t)m * k);

@@ -29,9 +29,9 @@ void frob_norm(tn_handle* h, const double* X, i64 n, double* out);
 // orthogonal.  Outputs sorted by descending row norm: Mout = W^T Min [c x r], Wt = W^T [c x c], sig [c].
 void jacobi_rows(tn_handle* h, const double* Min, int ld, int c, int r, double* Mout, double* Wt, double* sig);
 
-// Orthonormalise the columns of Y [m x k] (ld = k) in place: `passes` rounds of
-// (Gram -> Jacobi eigen-decomposition -> Y <- Y W Lambda^-1/2), eigenvalues floored at 1e-13 lambda_1
-// so that rank-deficient / exactly-zero columns are harmless (reading S6).
+// Orthonormalise the columns of Y [m x k] (ld = k) in place (orth.cu): up to `passes` rounds of pivot-floored
+// Cholesky-QR (k <= 96; Gram -> Jacobi eigen-decomposition rounds above that), early exit once Y^T Y = I to
+// rounding; rank-deficient / exactly-zero columns are harmless (reading S6).
 void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes);
 
 // ---- projector / fold maps on arrays laid out [outer][index][s] ----------

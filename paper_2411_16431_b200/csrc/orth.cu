@@ -1,0 +1,265 @@
+// Orthonormalisation of tall-skinny blocks (a3: QR canonicalisation, subspace-iteration bases).
+//
+// Y [m x k] (row-major, ld = k, k <= 96) is orthonormalised in place by up to `passes` rounds of
+// pivot-floored Cholesky-QR:   G = Y^T Y,  G = L L^T,  Y <- Y L^-T.
+// One launch per round does  [apply the previous round's T] -> [Gram of the result with DMMA] ->
+// [last CTA: ordered reduction of the per-CTA partial Grams, test ||G - I||, Cholesky, triangular
+// inverse], so a round costs one kernel instead of (split-K GEMM, reduce, Jacobi, scale, GEMM, copy).
+// Pivots below 1e-13 max_i G_ii are replaced by that floor (reading S6): a rank-deficient or
+// exactly-zero direction is scaled by a bounded factor instead of breaking the factorisation, and the
+// next round (conditioning improved by ~1e6.5) finishes the job; exactly-zero columns stay zero.
+// Rounds stop early (device flag) once ||G - I||_max is at rounding level.
+#include "kernels.cuh"
+
+namespace {
+
+constexpr int OR_ROWS = 64, OR_THREADS = 256;
+
+constexpr int OR_GS = 12, OR_MAXG = 16;   // two-level ordered reduction: groups of OR_GS CTAs
+struct OrthCtl { unsigned top; int done; int rounds; int pad; unsigned grp[OR_MAXG]; };
+
+__device__ __forceinline__ double block_max256(double v, double* sh) {
+  const int tid = threadIdx.x;
+  __syncthreads();
+  sh[tid] = v;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (tid < o) sh[tid] = fmax(sh[tid], sh[tid + o]);
+    __syncthreads();
+  }
+  double r = sh[0];
+  __syncthreads();
+  return r;
+}
+
+template <int KT>
+__global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y, i64 m, int k, const double* __restrict__ Tin,
+                                                          double* __restrict__ Tout, double* __restrict__ part, OrthCtl* ctl,
+                                                          int do_gram, double tol) {
+  constexpr int KP = 8 * KT, LD = smem_ld(KP), NQ = (KT + 7) / 8;
+  extern __shared__ double sm[];
+  __shared__ double s_red[OR_THREADS];
+  __shared__ int s_last;
+  if (ctl->done) return;
+  double* sT = sm;
+  double* sIn = sT + KP * LD;
+  double* sOut = sIn + OR_ROWS * LD;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (Tin)
+    for (int idx = tid; idx < KP * KP; idx += OR_THREADS) sT[(idx / KP) * LD + idx % KP] = Tin[idx];
+  double g[NQ][KT][2];
+#pragma unroll
+  for (int q = 0; q < NQ; q++)
+#pragma unroll
+    for (int j = 0; j < KT; j++) g[q][j][0] = g[q][j][1] = 0.0;
+
+  const i64 ntile = (m + OR_ROWS - 1) / OR_ROWS;
+  for (i64 tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+    const i64 r0 = tile * OR_ROWS;
+    __syncthreads();
+    for (int idx = tid; idx < OR_ROWS * KP; idx += OR_THREADS) {
+      int r = idx / KP, c = idx % KP;
+      i64 gr = r0 + r;
+      sIn[r * LD + c] = (gr < m && c < k) ? Y[gr * k + c] : 0.0;
+    }
+    __syncthreads();
+    const double* src = sIn;
+    if (Tin) {
+      double o[KT][2];
+#pragma unroll
+      for (int j = 0; j < KT; j++) o[j][0] = o[j][1] = 0.0;
+#pragma unroll 4
+      for (int kk = 0; kk < KP; kk += 4) {
+        double a = sIn[(8 * warp + (lane >> 2)) * LD + kk + (lane & 3)];
+#pragma unroll
+        for (int j = 0; j < KT; j++) dmma884(o[j][0], o[j][1], a, sT[(kk + (lane & 3)) * LD + 8 * j + (lane >> 2)]);
+      }
+#pragma unroll
+      for (int j = 0; j < KT; j++) {
+        int row = 8 * warp + (lane >> 2), col = 8 * j + 2 * (lane & 3);
+        sOut[row * LD + col] = o[j][0];
+        sOut[row * LD + col + 1] = o[j][1];
+      }
+      __syncthreads();
+      for (int idx = tid; idx < OR_ROWS * KP; idx += OR_THREADS) {
+        int r = idx / KP, c = idx % KP;
+        i64 gr = r0 + r;
+        if (gr < m && c < k) Y[gr * k + c] = sOut[r * LD + c];
+      }
+      src = sOut;
+    }
+    if (do_gram) {
+#pragma unroll
+      for (int q = 0; q < NQ; q++) {
+        const int ti = warp + 8 * q;
+        if (ti < KT) {
+#pragma unroll 4
+          for (int rr = 0; rr < OR_ROWS; rr += 4) {
+            const double* row = src + (rr + (lane & 3)) * LD + (lane >> 2);
+            double a = row[8 * ti];
+#pragma unroll
+            for (int j = 0; j < KT; j++) dmma884(g[q][j][0], g[q][j][1], a, row[8 * j]);
+          }
+        }
+      }
+    }
+  }
+  if (!do_gram) return;
+  // ---- partial Gram -> workspace; the last CTA to arrive reduces in CTA order (deterministic)
+  double* mine = part + (size_t)blockIdx.x * KP * KP;
+#pragma unroll
+  for (int q = 0; q < NQ; q++) {
+    const int ti = warp + 8 * q;
+    if (ti < KT) {
+#pragma unroll
+      for (int j = 0; j < KT; j++) {
+        int row = 8 * ti + (lane >> 2), col = 8 * j + 2 * (lane & 3);
+        mine[row * KP + col] = g[q][j][0];
+        mine[row * KP + col + 1] = g[q][j][1];
+      }
+    }
+  }
+  const int nb = gridDim.x, ngrp = (nb + OR_GS - 1) / OR_GS, grp = blockIdx.x / OR_GS;
+  const int g0 = grp * OR_GS, g1 = min(nb, g0 + OR_GS);
+  double* gpart = part + (size_t)nb * KP * KP;
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(&ctl->grp[grp], 1u) == (unsigned)(g1 - g0 - 1)) ? 1 : 0;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {   // level 1: this group's CTAs, in CTA order
+    double s = 0.0;
+#pragma unroll 4
+    for (int b = g0; b < g1; b++) s += __ldcg(part + (size_t)b * KP * KP + idx);
+    gpart[(size_t)grp * KP * KP + idx] = s;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(&ctl->top, 1u) == (unsigned)(ngrp - 1)) ? 1 : 0;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  constexpr int LG = KP + 1;
+  double* sG = sm;
+  double* sX = sm + KP * LG;
+  for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {   // level 2: groups in order
+    double s = 0.0;
+#pragma unroll 4
+    for (int b = 0; b < ngrp; b++) s += __ldcg(gpart + (size_t)b * KP * KP + idx);
+    sG[(idx / KP) * LG + idx % KP] = s;
+  }
+  __syncthreads();
+  double dev = 0.0, md = 0.0;
+  for (int idx = tid; idx < k * k; idx += OR_THREADS) {
+    int i = idx / k, j = idx % k;
+    double v = sG[i * LG + j];
+    dev = fmax(dev, fabs(v - (i == j ? 1.0 : 0.0)));
+    if (i == j) md = fmax(md, v);
+  }
+  dev = block_max256(dev, s_red);
+  md = block_max256(md, s_red);
+  if (tid == 0) { ctl->top = 0; ctl->rounds++; }
+  if (tid < OR_MAXG) ctl->grp[tid] = 0;
+  if (dev <= tol) {
+    if (tid == 0) ctl->done = 1;
+    return;
+  }
+  const double floor_ = 1e-13 * md;
+  // ---- Cholesky G = L L^T (lower triangle of sG, in place), pivots floored
+  for (int j = 0; j < k; j++) {
+    __syncthreads();
+    double d = sG[j * LG + j];
+    if (!(d > floor_)) d = floor_;
+    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;
+    __syncthreads();
+    for (int i = j + tid; i < k; i += OR_THREADS) sG[i * LG + j] = (i == j) ? d * inv : sG[i * LG + j] * inv;
+    __syncthreads();
+    const int n = k - j - 1;
+    for (int idx = tid; idx < n * n; idx += OR_THREADS) {
+      int i = j + 1 + idx / n, c = j + 1 + idx % n;
+      if (c <= i) sG[i * LG + c] -= sG[i * LG + j] * sG[c * LG + j];
+    }
+  }
+  // ---- X = L^-1 (lower triangular) by a column sweep of rank-1 updates
+  for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
+  for (int p = 0; p < k; p++) {
+    __syncthreads();
+    const double lp = sG[p * LG + p];
+    const double ip = lp > 0.0 ? 1.0 / lp : 0.0;
+    for (int c = tid; c <= p; c += OR_THREADS) sX[p * LG + c] *= ip;
+    __syncthreads();
+    const int n = k - p - 1, w = p + 1;
+    for (int idx = tid; idx < n * w; idx += OR_THREADS) {
+      int i = p + 1 + idx / w, c = idx % w;
+      sX[i * LG + c] -= sG[i * LG + p] * sX[p * LG + c];
+    }
+  }
+  __syncthreads();
+  // T = L^-T (upper triangular), zero-padded to KP x KP
+  for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
+    int c = idx / KP, j = idx % KP;
+    Tout[idx] = (c <= j && j < k) ? sX[j * LG + c] : 0.0;
+  }
+}
+
+template <int KT>
+void run_orth(tn_handle* h, double* Y, i64 m, int k, int passes) {
+  constexpr int KP = 8 * KT, LD = smem_ld(KP);
+  const size_t smem = sizeof(double) * ((size_t)KP * LD + 2 * (size_t)OR_ROWS * LD);
+  static bool attr = false;
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_orth_pass<KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr = true;
+  }
+  const int nb = (int)std::min<i64>(148, (m + OR_ROWS - 1) / OR_ROWS);
+  DBuf<double> part(h, (size_t)(nb + OR_MAXG) * KP * KP), T(h, 2 * (size_t)KP * KP);
+  DBuf<OrthCtl> ctl(h, 1);
+  TN_CUDA(cudaMemsetAsync(ctl.p, 0, sizeof(OrthCtl), h->stream));
+  const double tol = 1e-15 * (32.0 + std::sqrt((double)m));
+  for (int p = 0; p <= passes; p++) {
+    const double* Tin = p > 0 ? T.p + (size_t)((p - 1) & 1) * KP * KP : nullptr;
+    double* Tout = T.p + (size_t)(p & 1) * KP * KP;
+    k_orth_pass<KT><<<nb, OR_THREADS, smem, h->stream>>>(Y, m, k, Tin, Tout, part.p, ctl.p, p < passes ? 1 : 0, tol);
+    TN_LAUNCH_CHECK(h);
+  }
+}
+
+}  // namespace
+
+void orth_columns_jacobi(tn_handle* h, double* Y, i64 m, int k, int passes);   // kernels.cu (k > 96)
+
+void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes) {
+  if (m <= 0 || k <= 0) return;
+  if (k <= 16) run_orth<2>(h, Y, m, k, passes);
+  else if (k <= 32) run_orth<4>(h, Y, m, k, passes);
+  else if (k <= 48) run_orth<6>(h, Y, m, k, passes);
+  else if (k <= 64) run_orth<8>(h, Y, m, k, passes);
+  else if (k <= 80) run_orth<10>(h, Y, m, k, passes);
+  else if (k <= 96) run_orth<12>(h, Y, m, k, passes);
+  else orth_columns_jacobi(h, Y, m, k, passes);
+}
+
+// ---- tn_kernel_check: one building block on host data (kernel-level parity tests) ----------------
+void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A, const double* B, double* C) {
+  if (op == TN_CHECK_ORTH) {
+    DBuf<double> Y(h, (size_t)m * k);
+    TN_CUDA(cudaMemcpyAsync(Y.p, A, sizeof(double) * m * k, cudaMemcpyHostToDevice, h->stream));
+    orth_columns(h, Y.p, m, k, 4);
+    TN_CUDA(cudaMemcpyAsync(C, Y.p, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaStreamSynchronize(h->stream));
+  } else if (op == TN_CHECK_GEMM_N || op == TN_CHECK_GEMM_T) {
+    if (!B) tn_throw(TN_ERR_ARG, "B is NULL");
+    const bool t = op == TN_CHECK_GEMM_T;
+    const i64 nb = t ? m * n : (i64)k * n, nc = t ? (i64)k * n : m * n;
+    DBuf<double> dA(h, (size_t)m * k), dB(h, (size_t)nb), dC(h, (size_t)nc);
+    TN_CUDA(cudaMemcpyAsync(dA.p, A, sizeof(double) * m * k, cudaMemcpyHostToDevice, h->stream));
+    TN_CUDA(cudaMemcpyAsync(dB.p, B, sizeof(double) * nb, cudaMemcpyHostToDevice, h->stream));
+    if (t) gemm_rm(h, true, false, k, n, (int)m, dA.p, k, dB.p, n, dC.p, n);
+    else gemm_rm(h, false, false, (int)m, n, k, dA.p, k, dB.p, n, dC.p, n);
+    TN_CUDA(cudaMemcpyAsync(C, dC.p, sizeof(double) * nc, cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaStreamSynchronize(h->stream));
+  } else {
+    tn_throw(TN_ERR_ARG, "unknown op %d", op);
+  }
+}

@@ -138,3 +138,5 @@ void search_logz(tn_handle* h);
 void search_run(tn_handle* h, int M, int* n_out, int8_t* states, double* energies, double* logp,
                 double* log_pd);
 void energy_run(tn_handle* h, int n, const int8_t* states, double* energies);
+// ---- orth.cu
+void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A, const double* B, double* C);

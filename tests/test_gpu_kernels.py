@@ -1,0 +1,88 @@
+"""Kernel-level GPU parity: single device building blocks (through tn_kernel_check of the C ABI) against
+their plain definitions in numpy fp64."""
+import numpy as np
+import pytest
+
+import instances
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tn():
+    import paper_2411_16431_b200 as tnb
+    with tnb.TensorNetwork(instances.lattice(2, 2, 2, 2, seed=1)) as t:
+        yield t
+
+
+def _check(tn, op, A, B=None):
+    import paper_2411_16431_b200 as tnb
+    return tnb.tn_kernel_check(tn.handle, op, A, B)
+
+
+ORTH = [(1, 1), (7, 3), (64, 16), (65, 17), (1000, 32), (4097, 33), (20000, 48), (5000, 64), (9999, 80), (30011, 96),
+        (300, 100)]
+
+
+@pytest.mark.parametrize("m,k", ORTH)
+def test_orth_columns_well_conditioned(tn, m, k):
+    import paper_2411_16431_b200 as tnb
+    rng = np.random.default_rng(m * 131 + k)
+    k = min(k, m)
+    A = rng.standard_normal((m, k))
+    Q = _check(tn, tnb.CHECK_ORTH, A)
+    assert np.abs(Q.T @ Q - np.eye(k)).max() <= 1e-13
+    # same column space, and (Cholesky-QR keeps the column order) Q^T A is upper triangular
+    R = Q.T @ A
+    assert np.abs(Q @ R - A).max() <= 1e-12 * np.abs(A).max()
+    if k <= 96:
+        assert np.abs(np.tril(R, -1)).max() <= 1e-12 * np.abs(R).max()
+
+
+@pytest.mark.parametrize("m,k,cond", [(2000, 32, 1e8), (2000, 32, 1e14), (5000, 80, 1e12), (3000, 48, 1e20)])
+def test_orth_columns_ill_conditioned(tn, m, k, cond):
+    """Singular values decaying over `cond` (beyond 1/eps: numerically rank-deficient, reading S6)."""
+    import paper_2411_16431_b200 as tnb
+    rng = np.random.default_rng(k)
+    U, _ = np.linalg.qr(rng.standard_normal((m, k)))
+    V, _ = np.linalg.qr(rng.standard_normal((k, k)))
+    s = np.logspace(0, -np.log10(cond), k)
+    A = (U * s) @ V.T
+    Q = _check(tn, tnb.CHECK_ORTH, A)
+    assert np.isfinite(Q).all()
+    assert np.abs(Q.T @ Q - np.eye(k)).max() <= 1e-10
+    # the well-determined part of the column space is reproduced
+    keep = s > 1e-6
+    P = (U[:, keep] * s[keep]) @ V[:, keep].T
+    assert np.abs(Q @ (Q.T @ P) - P).max() <= 1e-9
+
+
+def test_orth_columns_zero_columns_stay_zero(tn):
+    import paper_2411_16431_b200 as tnb
+    rng = np.random.default_rng(5)
+    A = rng.standard_normal((777, 24))
+    A[:, 17:] = 0.0
+    Q = _check(tn, tnb.CHECK_ORTH, A)
+    assert np.all(Q[:, 17:] == 0.0)
+    assert np.abs(Q[:, :17].T @ Q[:, :17] - np.eye(17)).max() <= 1e-13
+    Z = _check(tn, tnb.CHECK_ORTH, np.zeros((100, 8)))
+    assert np.all(Z == 0.0)
+
+
+GEMM = [(1, 1, 1), (5, 3, 7), (128, 16, 128), (129, 17, 65), (1000, 32, 515), (4096, 80, 300), (333, 96, 2049),
+        (70000, 24, 64), (50, 130, 40)]
+
+
+@pytest.mark.parametrize("m,n,k", GEMM)
+def test_skinny_gemm_n_and_t(tn, m, n, k):
+    import paper_2411_16431_b200 as tnb
+    rng = np.random.default_rng(m + 7 * n + 13 * k)
+    A = rng.standard_normal((m, k))
+    B = rng.standard_normal((k, n))
+    C = _check(tn, tnb.CHECK_GEMM_N, A, B)
+    ref = A @ B
+    assert np.abs(C - ref).max() <= 1e-13 * k * max(1.0, np.abs(ref).max())
+    Bt = rng.standard_normal((m, n))
+    Ct = _check(tn, tnb.CHECK_GEMM_T, A, Bt)
+    reft = A.T @ Bt
+    assert np.abs(Ct - reft).max() <= 1e-13 * m * max(1.0, np.abs(reft).max())
