@@ -161,6 +161,12 @@ enum { TN_CHECK_ORTH = 1, TN_CHECK_GEMM_N = 2, TN_CHECK_GEMM_T = 3 };
 int tn_kernel_check(tn_handle*, int32_t op, int64_t m, int32_t n, int32_t k, const double* A, const double* B,
                     double* C);
 
+/* tn_kernel_bench: diagnostic -- device time (CUDA events on the handle's stream, one untimed warm-up call) of one
+ * building block on device-resident random data, averaged over `iters` calls, in ms per call:
+ *   TN_CHECK_GEMM_N / TN_CHECK_GEMM_T with the shapes of tn_kernel_check (2 m n k FLOP per call, one read of A);
+ *   TN_CHECK_ORTH: orthonormalisation of a random [m x n] block (k unused). */
+int tn_kernel_bench(tn_handle*, int32_t op, int64_t m, int32_t n, int64_t k, int32_t iters, double* ms_per_call);
+
 /* tn_fp64_peak: measured FP64 tensor-core (mma.sync m8n8k4 f64 = SASS DMMA) peak of the current device
  * in TFLOP/s, from a register-resident chain (about 10 ms); the roofline denominator of the GEMM stages
  * ("FP64 tensor peak to be measured first").  Needs no handle. */

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP = 1, 2, 3, 4, 5
 
 
@@ -62,6 +62,7 @@ def lib():
         L.tn_get_stats.argtypes = [C.c_void_p, C.POINTER(TnStats)]
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
         L.tn_fp64_peak.argtypes = [p_f64]
+        L.tn_kernel_bench.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int64, C.c_int32, p_f64]
         L.tn_kernel_check.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, p_f64, p_f64, p_f64]
         L.tn_last_error.restype = C.c_char_p
         L.tn_destroy.argtypes = [C.c_void_p]
@@ -184,6 +185,13 @@ def tn_kernel_check(handle, op, A, B=None):
     _check(lib().tn_kernel_check(handle, int(op), int(m), int(n), int(k), _ptr(A, C.c_double), Bp,
                                  _ptr(out, C.c_double)))
     return out
+
+
+def tn_kernel_bench(handle, op, m, n, k, iters=10) -> float:
+    """Diagnostic: device ms per call of one building block on device-resident random data."""
+    v = C.c_double(0.0)
+    _check(lib().tn_kernel_bench(handle, int(op), int(m), int(n), int(k), int(iters), C.byref(v)))
+    return v.value
 
 
 def tn_fp64_peak() -> float:

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtn_b200.so")
 PROBE = os.path.join(HERE, "fp64_peak_probe")
-SOURCES = ["api.cu", "kernels.cu", "tables.cu", "contract.cu", "search.cu", "probe.cu", "orth.cu"]
+SOURCES = ["api.cu", "kernels.cu", "tables.cu", "contract.cu", "search.cu", "probe.cu", "orth.cu", "tsgemm.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

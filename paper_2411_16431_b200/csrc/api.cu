@@ -324,6 +324,20 @@ int tn_kernel_check(tn_handle* h, int32_t op, int64_t m, int32_t n, int32_t k, c
   TN_API_END
 }
 
+int tn_kernel_bench(tn_handle* h, int32_t op, int64_t m, int32_t n, int64_t k, int32_t iters, double* ms_per_call) {
+  TN_API_BEGIN
+  if (!h || !ms_per_call || m < 1 || n < 1 || k < 1) tn_throw(TN_ERR_ARG, "bad argument");
+  need_device();
+  try {
+    kernel_bench_run(h, op, m, n, k, iters, ms_per_call);
+  } catch (...) {
+    trim_free_list(h);
+    throw;
+  }
+  trim_free_list(h);
+  TN_API_END
+}
+
 int tn_get_stats(tn_handle* h, tn_stats* out) {
   TN_API_BEGIN
   if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");

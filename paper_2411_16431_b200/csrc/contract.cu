@@ -271,7 +271,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
   double* Yn = Yb.p;
   fill_random(h, Om.p, n * ks, cx.seed++);
   cx.tic(&h->st.ms_orth_svd);
-  orth_columns(h, Om.p, n, ks, 2);
+  orth_columns(h, Om.p, n, ks, 3);
   cx.toc();
   const int rpb = 512;
   const int nblk = cdiv(m, rpb);
@@ -294,12 +294,12 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     }
     std::swap(Y, Yn);
     cx.tic(&h->st.ms_orth_svd);
-    orth_columns(h, Y, m, ks, 4);
+    orth_columns(h, Y, m, ks, 5);
     cx.toc();
     apply_T(cx, op, Y, Z.p, ks);
     TN_CUDA(cudaMemcpyAsync(Om.p, Z.p, sizeof(double) * n * ks, cudaMemcpyDeviceToDevice, h->stream));
     cx.tic(&h->st.ms_orth_svd);
-    orth_columns(h, Om.p, n, ks, 4);
+    orth_columns(h, Om.p, n, ks, 5);
     gemm_rm(h, true, false, ks, ks, (int)n, Om.p, ks, Z.p, ks, B.p, ks);
     jacobi_rows(h, B.p, ks, ks, ks, Bo.p, Wt.p, sig.p);
     k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, ks, chi, h->gap_guard, cx.d_keep, cx.d_stat);
@@ -344,7 +344,7 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
     DBuf<double> Q(h, (size_t)rows * ar), Rf(h, (size_t)ar * ar);
     TN_CUDA(cudaMemcpyAsync(Q.p, A[j].d, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
     cx.tic(&h->st.ms_orth_svd);
-    orth_columns(h, Q.p, rows, ar, 4);
+    orth_columns(h, Q.p, rows, ar, 5);
     cx.toc();
     gemm_rm(h, true, false, ar, ar, (int)rows, Q.p, ar, A[j].d, ar, Rf.p, ar);
     TN_CUDA(cudaMemcpyAsync(A[j].d, Q.p, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
@@ -415,7 +415,7 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
           apply_T(cx, op, Renv[j], Z.p, s);
           if (j + 1 < n) {
             cx.tic(&h->st.ms_orth_svd);
-            orth_columns(h, Z.p, op.n, s, 4);
+            orth_columns(h, Z.p, op.n, s, 5);
             cx.toc();
             if (Lenv[j + 1]) h->dfree(Lenv[j + 1]);
             Lenv[j + 1] = h->dalloc<double>((size_t)op.m * s);
@@ -437,7 +437,7 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
           apply_T(cx, op, Lenv[j], Z.p, s);
           if (j > 0) {
             cx.tic(&h->st.ms_orth_svd);
-            orth_columns(h, Z.p, op.n, s, 4);
+            orth_columns(h, Z.p, op.n, s, 5);
             cx.toc();
             h->dfree(Renv[j - 1]);
             Renv[j - 1] = h->dalloc<double>((size_t)op.m * s);

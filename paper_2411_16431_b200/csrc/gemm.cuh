@@ -154,6 +154,10 @@ struct GemmDesc {
 };
 // kernels.cu
 void gemm_general(tn_handle* h, const GemmDesc& g);
+// tsgemm.cu: streaming tall x skinny GEMM (N <= 96).  trans = false: C[M x N] = A[M x K] B[K x N];
+// trans = true: C[K x N] = A[M x K]^T B[M x N].  Returns false if shape / alignment do not fit.
+bool tsgemm(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb, double* C,
+            i64 ldc);
 // plain row-major helpers: C[M,N] = op(A) op(B)
 void gemm_rm(tn_handle* h, bool ta, bool tb, int M, int N, int K, const double* A, int lda, const double* B,
              int ldb, double* C, int ldc, double alpha = 1.0, double beta = 0.0);

@@ -70,6 +70,11 @@ void gemm_general(tn_handle* h, const GemmDesc& g) {
 
 void gemm_rm(tn_handle* h, bool ta, bool tb, int M, int N, int K, const double* A, int lda, const double* B,
              int ldb, double* C, int ldc, double alpha, double beta) {
+  if (M <= 0 || N <= 0) return;
+  if (!tb && alpha == 1.0 && beta == 0.0 && K > 0) {   // tall x skinny: streaming cp.async kernel (tsgemm.cu)
+    if (!ta && tsgemm(h, false, M, N, K, A, lda, B, ldb, C, ldc)) return;
+    if (ta && tsgemm(h, true, K, N, M, A, lda, B, ldb, C, ldc)) return;
+  }
   GemmDesc g;
   g.M = M; g.N = N; g.K = K;
   g.A = A; g.a_i = ta ? 1 : lda; g.a_k = ta ? lda : 1;

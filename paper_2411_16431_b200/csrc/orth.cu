@@ -5,7 +5,7 @@
 // One launch per round does  [apply the previous round's T] -> [Gram of the result with DMMA] ->
 // [last CTA: ordered reduction of the per-CTA partial Grams, test ||G - I||, Cholesky, triangular
 // inverse], so a round costs one kernel instead of (split-K GEMM, reduce, Jacobi, scale, GEMM, copy).
-// Pivots below 1e-13 max_i G_ii are replaced by that floor (reading S6): a rank-deficient or
+// Pivots below ~1e-11 max_i G_ii are replaced by that floor (reading S6): a rank-deficient or
 // exactly-zero direction is scaled by a bounded factor instead of breaking the factorisation, and the
 // next round (conditioning improved by ~1e6.5) finishes the job; exactly-zero columns stay zero.
 // Rounds stop early (device flag) once ||G - I||_max is at rounding level.
@@ -35,7 +35,7 @@ __device__ __forceinline__ double block_max256(double v, double* sh) {
 template <int KT>
 __global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y, i64 m, int k, const double* __restrict__ Tin,
                                                           double* __restrict__ Tout, double* __restrict__ part, OrthCtl* ctl,
-                                                          int do_gram, double tol) {
+                                                          int do_gram, double tol, double frel) {
   constexpr int KP = 8 * KT, LD = smem_ld(KP), NQ = (KT + 7) / 8;
   extern __shared__ double sm[];
   __shared__ double s_red[OR_THREADS];
@@ -165,16 +165,23 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y
     if (tid == 0) ctl->done = 1;
     return;
   }
-  const double floor_ = 1e-13 * md;
-  // ---- Cholesky G = L L^T (lower triangle of sG, in place), pivots floored
+  const double floor_ = frel * md;
+  // ---- Cholesky G = L L^T (lower triangle of sG, in place).  A pivot at or below the floor (rounding noise of
+  // the Gram matrix, c * eps * md) is replaced by the floor and its sub-column is dropped: noise directions
+  // are scaled up by a bounded factor and are NOT used to "orthogonalise" later columns -- dividing noise by
+  // noise gives O(1) multipliers and an exponentially ill-conditioned L.  The next round sees them at a
+  // resolvable size.
   for (int j = 0; j < k; j++) {
     __syncthreads();
     double d = sG[j * LG + j];
-    if (!(d > floor_)) d = floor_;
+    const bool floored = !(d > floor_);
+    if (floored) d = floor_;
     const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;
     __syncthreads();
-    for (int i = j + tid; i < k; i += OR_THREADS) sG[i * LG + j] = (i == j) ? d * inv : sG[i * LG + j] * inv;
+    for (int i = j + tid; i < k; i += OR_THREADS)
+      sG[i * LG + j] = (i == j) ? d * inv : (floored ? 0.0 : sG[i * LG + j] * inv);
     __syncthreads();
+    if (floored) continue;
     const int n = k - j - 1;
     for (int idx = tid; idx < n * n; idx += OR_THREADS) {
       int i = j + 1 + idx / n, c = j + 1 + idx % n;
@@ -217,10 +224,11 @@ void run_orth(tn_handle* h, double* Y, i64 m, int k, int passes) {
   DBuf<OrthCtl> ctl(h, 1);
   TN_CUDA(cudaMemsetAsync(ctl.p, 0, sizeof(OrthCtl), h->stream));
   const double tol = 1e-15 * (32.0 + std::sqrt((double)m));
+  const double frel = 1e-11 * std::max(1.0, std::sqrt((double)m) / 128.0);   // pivot floor relative to max_i G_ii
   for (int p = 0; p <= passes; p++) {
     const double* Tin = p > 0 ? T.p + (size_t)((p - 1) & 1) * KP * KP : nullptr;
     double* Tout = T.p + (size_t)(p & 1) * KP * KP;
-    k_orth_pass<KT><<<nb, OR_THREADS, smem, h->stream>>>(Y, m, k, Tin, Tout, part.p, ctl.p, p < passes ? 1 : 0, tol);
+    k_orth_pass<KT><<<nb, OR_THREADS, smem, h->stream>>>(Y, m, k, Tin, Tout, part.p, ctl.p, p < passes ? 1 : 0, tol, frel);
     TN_LAUNCH_CHECK(h);
   }
 }
@@ -231,6 +239,36 @@ void orth_columns_jacobi(tn_handle* h, double* Y, i64 m, int k, int passes);   /
 
 void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes) {
   if (m <= 0 || k <= 0) return;
+  if (getenv("ORTH_OLD")) { orth_columns_jacobi(h, Y, m, k, passes); return; }
+  std::vector<double> dbg_in;
+  if (getenv("ORTH_DEBUG")) {
+    dbg_in.resize((size_t)m * k);
+    cudaMemcpyAsync(dbg_in.data(), Y, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream);
+    cudaStreamSynchronize(h->stream);
+  }
+  struct Dbg {
+    tn_handle* h; double* Y; i64 m; int k; std::vector<double>& in;
+    ~Dbg() {
+      if (in.empty()) return;
+      std::vector<double> out((size_t)m * k);
+      cudaMemcpyAsync(out.data(), Y, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream);
+      cudaStreamSynchronize(h->stream);
+      bool bi = false, bo = false;
+      for (double v : in) if (!std::isfinite(v)) bi = true;
+      for (double v : out) if (!std::isfinite(v)) bo = true;
+      static int ncall = 0;
+      ncall++;
+      if (bo || bi) {
+        fprintf(stderr, "ORTH_DEBUG call %d m=%lld k=%d bad_in=%d bad_out=%d\n", ncall, (long long)m, k, (int)bi, (int)bo);
+        if (bo && !bi) {
+          FILE* f = fopen("gpurun_out/orth_bad.bin", "wb");
+          long long hdr[2] = {m, k};
+          fwrite(hdr, 8, 2, f); fwrite(in.data(), 8, in.size(), f); fwrite(out.data(), 8, out.size(), f); fclose(f);
+          exit(3);
+        }
+      }
+    }
+  } dbg{h, Y, m, k, dbg_in};
   if (k <= 16) run_orth<2>(h, Y, m, k, passes);
   else if (k <= 32) run_orth<4>(h, Y, m, k, passes);
   else if (k <= 48) run_orth<6>(h, Y, m, k, passes);
@@ -245,7 +283,7 @@ void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A
   if (op == TN_CHECK_ORTH) {
     DBuf<double> Y(h, (size_t)m * k);
     TN_CUDA(cudaMemcpyAsync(Y.p, A, sizeof(double) * m * k, cudaMemcpyHostToDevice, h->stream));
-    orth_columns(h, Y.p, m, k, 4);
+    orth_columns(h, Y.p, m, k, 5);
     TN_CUDA(cudaMemcpyAsync(C, Y.p, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream));
     TN_CUDA(cudaStreamSynchronize(h->stream));
   } else if (op == TN_CHECK_GEMM_N || op == TN_CHECK_GEMM_T) {
@@ -262,4 +300,46 @@ void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A
   } else {
     tn_throw(TN_ERR_ARG, "unknown op %d", op);
   }
+}
+
+// ---- tn_kernel_bench: device time of one building block on device-resident random data -----------
+void kernel_bench_run(tn_handle* h, int op, i64 m, int n, i64 k, int iters, double* ms_per_call) {
+  if (iters < 1) iters = 1;
+  cudaEvent_t e0, e1;
+  TN_CUDA(cudaEventCreate(&e0)); TN_CUDA(cudaEventCreate(&e1));
+  float ms = 0;
+  if (op == TN_CHECK_ORTH) {
+    DBuf<double> Y(h, (size_t)m * n), Y0(h, (size_t)m * n);
+    fill_random(h, Y0.p, m * n, 7);
+    double tot = 0;
+    for (int it = -1; it < iters; it++) {
+      TN_CUDA(cudaMemcpyAsync(Y.p, Y0.p, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, h->stream));
+      TN_CUDA(cudaEventRecord(e0, h->stream));
+      orth_columns(h, Y.p, m, n, 5);
+      TN_CUDA(cudaEventRecord(e1, h->stream));
+      TN_CUDA(cudaEventSynchronize(e1));
+      TN_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+      if (it >= 0) tot += ms;
+    }
+    *ms_per_call = tot / iters;
+  } else if (op == TN_CHECK_GEMM_N || op == TN_CHECK_GEMM_T) {
+    const bool t = op == TN_CHECK_GEMM_T;
+    const i64 nb = t ? m * n : k * n, nc = t ? k * n : m * n;
+    DBuf<double> dA(h, (size_t)m * k), dB(h, (size_t)nb), dC(h, (size_t)nc);
+    fill_random(h, dA.p, m * k, 1);
+    fill_random(h, dB.p, nb, 2);
+    for (int it = -1; it < iters; it++) {
+      if (it == 0) TN_CUDA(cudaEventRecord(e0, h->stream));
+      if (t) gemm_rm(h, true, false, (int)k, n, (int)m, dA.p, (int)k, dB.p, n, dC.p, n);
+      else gemm_rm(h, false, false, (int)m, n, (int)k, dA.p, (int)k, dB.p, n, dC.p, n);
+    }
+    TN_CUDA(cudaEventRecord(e1, h->stream));
+    TN_CUDA(cudaEventSynchronize(e1));
+    TN_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    *ms_per_call = ms / iters;
+  } else {
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    tn_throw(TN_ERR_ARG, "unknown op %d", op);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
 }

@@ -140,3 +140,4 @@ void search_run(tn_handle* h, int M, int* n_out, int8_t* states, double* energie
 void energy_run(tn_handle* h, int n, const int8_t* states, double* energies);
 // ---- orth.cu
 void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A, const double* B, double* C);
+void kernel_bench_run(tn_handle* h, int op, i64 m, int n, i64 k, int iters, double* ms_per_call);

@@ -1,0 +1,221 @@
+// Streaming tall x skinny FP64 tensor-core GEMMs: the "Theta-core x skinny" applies of a2/a3 (Fig. 7
+// the O(chi^3 d) batched products are, with the explicit Theta-core, plain GEMMs with one
+// huge operand read once from HBM and a skinny operand of <= 96 columns).
+//
+//   N:  C[M x N] = A[M x K]   . B[K x N]      A row-major (lda), streamed by row blocks
+//   T:  C[K x N] = A[M x K]^T . B[M x N]      A row-major (lda), streamed by column blocks, reduced over rows
+//
+// Both: N <= 96 (all columns in one CTA), operands move global -> shared with 16-byte cp.async in a 3-stage
+// ring (zero-filled at the ragged edges), fragments for mma.sync.m8n8k4.f64 (SASS DMMA) are read from
+// shared memory with conflict-free strides (== 4 mod 16 doubles), 8 warps x (16 rows x N) register tiles.
+// Arithmetic intensity is N/4 FLOP/B, so the kernel is DMMA-bound for N >= 24 and HBM-bound below.
+// Small row counts use narrower CTAs and a split over the reduction (ordered workspace reduce: deterministic).
+#include "kernels.cuh"
+
+namespace {
+
+constexpr int TS_BK = 16, TS_STAGES = 3;
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+// TRANS = false: CTA owns rows [m0, m0+BM) of A / C, reduction index = columns of A.
+// TRANS = true : CTA owns columns [m0, m0+BM) of A (= rows of C), reduction index = rows of A.
+// In both cases "i" is the output row (BM per CTA, 16 per warp) and "kk" the reduction index.
+template <int NT, int WARPS, bool TRANS>
+__global__ void __launch_bounds__(WARPS * 32, (NT <= 10 || WARPS < 8) ? 2 : 1)
+k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i64 ldb, double* __restrict__ C, i64 ldc,
+         i64 Mout, int N, i64 Kred, i64 kper, double* __restrict__ ws) {
+  constexpr int BM = 16 * WARPS, NTH = 32 * WARPS, NP = 8 * NT;
+  constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK);   // doubles
+  constexpr int LDB = smem_ld(NP);
+  constexpr int A_ELEMS = TRANS ? TS_BK * LDA : BM * LDA;
+  constexpr int B_ELEMS = TS_BK * LDB;
+  extern __shared__ __align__(16) double smem[];
+  double* sA = smem;
+  double* sB = smem + TS_STAGES * A_ELEMS;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const i64 m0 = (i64)blockIdx.x * BM;
+  const int split = blockIdx.y, nsplit = gridDim.y;
+  const i64 k0 = (i64)split * kper, k1 = min(Kred, k0 + kper);
+  const int nkt = k1 > k0 ? (int)((k1 - k0 + TS_BK - 1) / TS_BK) : 0;
+
+  auto load_stage = [&](int stage, int kt) {
+    const i64 kb = k0 + (i64)kt * TS_BK;
+    double* a = sA + stage * A_ELEMS;
+    double* b = sB + stage * B_ELEMS;
+    if (!TRANS) {
+      constexpr int G = TS_BK / 2;                      // 16-byte granules per row
+      for (int idx = tid; idx < BM * G; idx += NTH) {
+        const int r = idx / G, g = idx % G;
+        const i64 gr = m0 + r, gk = kb + 2 * g;
+        i64 rem = gr < Mout ? (k1 - gk) : 0;
+        int bytes = rem >= 2 ? 16 : rem == 1 ? 8 : 0;
+        const double* src = bytes ? A + gr * lda + gk : A;
+        cp_async16(a + r * LDA + 2 * g, src, bytes);
+      }
+    } else {
+      constexpr int G = BM / 2;
+      for (int idx = tid; idx < TS_BK * G; idx += NTH) {
+        const int r = idx / G, g = idx % G;
+        const i64 gk = kb + r, gc = m0 + 2 * g;
+        i64 rem = gk < k1 ? (Mout - gc) : 0;
+        int bytes = rem >= 2 ? 16 : rem == 1 ? 8 : 0;
+        const double* src = bytes ? A + gk * lda + gc : A;
+        cp_async16(a + r * LDA + 2 * g, src, bytes);
+      }
+    }
+    {
+      constexpr int G = NP / 2;
+      for (int idx = tid; idx < TS_BK * G; idx += NTH) {
+        const int r = idx / G, g = idx % G;
+        const i64 gk = kb + r;
+        const int gc = 2 * g;
+        int rem = gk < k1 ? (N - gc) : 0;
+        int bytes = rem >= 2 ? 16 : rem == 1 ? 8 : 0;
+        const double* src = bytes ? B + gk * ldb + gc : B;
+        cp_async16(b + r * LDB + 2 * g, src, bytes);
+      }
+    }
+  };
+
+  double acc[2][NT][2];
+#pragma unroll
+  for (int i = 0; i < 2; i++)
+#pragma unroll
+    for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+#pragma unroll
+  for (int s = 0; s < TS_STAGES - 1; s++) {
+    if (s < nkt) load_stage(s, s);
+    cp_async_commit();
+  }
+  for (int kt = 0; kt < nkt; kt++) {
+    cp_async_wait<TS_STAGES - 2>();
+    __syncthreads();
+    if (kt + TS_STAGES - 1 < nkt) load_stage((kt + TS_STAGES - 1) % TS_STAGES, kt + TS_STAGES - 1);
+    cp_async_commit();
+    const double* a = sA + (kt % TS_STAGES) * A_ELEMS;
+    const double* b = sB + (kt % TS_STAGES) * B_ELEMS;
+#pragma unroll
+    for (int kk = 0; kk < TS_BK; kk += 4) {
+      double fa[2];
+#pragma unroll
+      for (int i = 0; i < 2; i++)
+        fa[i] = TRANS ? a[(kk + (lane & 3)) * LDA + 16 * warp + 8 * i + (lane >> 2)]
+                      : a[(16 * warp + 8 * i + (lane >> 2)) * LDA + kk + (lane & 3)];
+      const double* brow = b + (kk + (lane & 3)) * LDB + (lane >> 2);
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const double fb = brow[8 * j];
+        dmma884(acc[0][j][0], acc[0][j][1], fa[0], fb);
+        dmma884(acc[1][j][0], acc[1][j][1], fa[1], fb);
+      }
+    }
+  }
+  cp_async_wait<0>();
+  // ---- epilogue
+  double* out = nsplit > 1 ? ws + (size_t)split * Mout * N : C;
+  const i64 ldo = nsplit > 1 ? N : ldc;
+#pragma unroll
+  for (int i = 0; i < 2; i++) {
+    const i64 row = m0 + 16 * warp + 8 * i + (lane >> 2);
+    if (row < Mout) {
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const int col = 8 * j + 2 * (lane & 3);
+        if (col < N) out[row * ldo + col] = acc[i][j][0];
+        if (col + 1 < N) out[row * ldo + col + 1] = acc[i][j][1];
+      }
+    }
+  }
+}
+
+// C[i][j] = sum_s ws[s][i][j]  (fixed order)
+__global__ void k_ts_reduce(const double* __restrict__ ws, int nsplit, i64 M, int N, double* __restrict__ C, i64 ldc) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= M * N) return;
+  double s = 0.0;
+  for (int sp = 0; sp < nsplit; sp++) s += ws[(size_t)sp * M * N + t];
+  C[(t / N) * ldc + t % N] = s;
+}
+
+template <int NT, int WARPS, bool TRANS>
+void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
+               i64 Kred, int nsplit) {
+  constexpr int BM = 16 * WARPS, NP = 8 * NT;
+  constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK), LDB = smem_ld(NP);
+  constexpr size_t smem = sizeof(double) * TS_STAGES * ((TRANS ? TS_BK * LDA : BM * LDA) + TS_BK * LDB);
+  static bool attr = false;
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_tsgemm<NT, WARPS, TRANS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr = true;
+  }
+  i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
+  nsplit = (int)((Kred + kper - 1) / kper);
+  double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nsplit * Mout * N) : nullptr;
+  dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit);
+  k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws);
+  TN_LAUNCH_CHECK(h);
+  if (nsplit > 1) {
+    k_ts_reduce<<<cdiv(Mout * N, 256), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc);
+    TN_LAUNCH_CHECK(h);
+    h->dfree(ws);
+  }
+}
+
+// CTA width and reduction split: minimise  waves x (per-CTA work + fixed cost) + split-workspace traffic.
+// Measured on B200 (profiles/): wide CTAs win everywhere; the split mostly repairs wave quantisation when the
+// output has fewer row blocks than 2 x 148 CTA slots.
+template <int NT, bool TRANS>
+void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
+                i64 Kred) {
+  int warps = Mout > 64 ? 8 : Mout > 32 ? 4 : 2;
+  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps);
+  const int slots = 148 * ((NT <= 10 || warps < 8) ? 2 : 1);
+  const double t_k = 2.0 * 16 * warps * (8 * NT) * slots / 37e12;      // seconds per reduction index per CTA
+  const double t_ws = (double)Mout * N * 16.0 / 6e12 + 2e-7;           // seconds per extra split (write + read)
+  int best = 1;
+  double best_t = 1e30;
+  const int smax = (int)std::max<i64>(1, std::min<i64>(64, Kred / 128));
+  for (int sp = 1; sp <= smax; sp++) {
+    const i64 waves = (tiles * sp + slots - 1) / slots;
+    const double t = waves * ((double)((Kred + sp - 1) / sp) + 96.0) * t_k + (sp > 1 ? sp * t_ws + 3e-6 : 0.0);
+    if (t < best_t) { best_t = t; best = sp; }
+  }
+  if (warps == 8) launch_ts<NT, 8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
+  else if (warps == 4) launch_ts<NT, 4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
+  else launch_ts<NT, 2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
+}
+
+template <bool TRANS>
+void pick_nt(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
+             i64 Kred) {
+  if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  else if (N <= 32) pick_warps<4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  else if (N <= 48) pick_warps<6, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  else if (N <= 64) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  else if (N <= 80) pick_warps<10, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  else pick_warps<12, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+}
+
+bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
+
+}  // namespace
+
+// Returns false when the shapes / alignment do not fit (the caller falls back to the generic k_gemm).
+bool tsgemm(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb, double* C,
+            i64 ldc) {
+  if (N < 1 || N > 96 || M < 1 || K < 1) return false;
+  if (getenv("TS_DISABLE")) return false;
+  if ((lda & 1) || (ldb & 1) || !aligned16(A) || !aligned16(B)) return false;
+  if (trans) pick_nt<true>(h, A, lda, B, ldb, C, ldc, K, N, M);    // output rows = K (columns of A), reduce over M
+  else pick_nt<false>(h, A, lda, B, ldb, C, ldc, M, N, K);
+  return true;
+}
