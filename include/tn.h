@@ -67,7 +67,10 @@ enum {
                              (default 1e-11; reading S1)            */
   TN_OPT_SVD_MAXIT = 3,   /* max block-subspace iterations per zipper step (default 40)       */
   TN_OPT_OVERSAMPLE = 4,  /* extra block columns of the subspace iteration (default 16)       */
-  TN_OPT_EXACT_CAP = 5    /* largest bond allowed when D <= 0 (default 512)                   */
+  TN_OPT_EXACT_CAP = 5,   /* largest bond allowed when D <= 0 (default 512)                   */
+  TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
+                             all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
+                             key first and one prefilter pass compacts the survivors (default 2^22)  */
 };
 
 /* Counters and timers filled by tn_get_stats (all since the last tn_set_beta). */

@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
                     "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
-OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP = 1, 2, 3, 4, 5
+OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX = 1, 2, 3, 4, 5, 6
 
 
 class TnError(RuntimeError):

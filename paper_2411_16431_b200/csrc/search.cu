@@ -197,13 +197,28 @@ struct SelArgs {
 __device__ __forceinline__ double sel_fcd(const SelArgs& a, int m, int cl, int ch) {
   return a.wC[cl * a.nCh + ch] * a.Bd[a.drow_x[a.slot[m]] * a.n_i + a.Pi[ch]];
 }
-__global__ void k_sel_hist(SelArgs a, const SelState* st, int shift, int nbits, int first, unsigned* hist) {
+__device__ __forceinline__ unsigned long long sel_mix(unsigned long long z) {
+  z += 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+// Histogram of one radix digit of the keys.  sample_log2 > 0: only one hashed element of every
+// 2^sample_log2 consecutive entries of V is looked at (a SUBSET of the candidates: its (M+1)-th largest key is a
+// guaranteed lower bound of the true (M+1)-th largest, used as a prefilter threshold).
+__global__ void k_sel_hist(SelArgs a, const SelState* st, int shift, int nbits, int first, int sample_log2, unsigned* hist) {
   __shared__ unsigned sh[4096];
   for (int i = threadIdx.x; i < 4096; i += blockDim.x) sh[i] = 0;
   __syncthreads();
   const unsigned long long prefix = st->prefix;
   const i64 total = (i64)a.nb * a.per_m;
-  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+  const i64 nq = sample_log2 ? ((total + (1ll << sample_log2) - 1) >> sample_log2) : total;
+  for (i64 q = (i64)blockIdx.x * blockDim.x + threadIdx.x; q < nq; q += (i64)gridDim.x * blockDim.x) {
+    i64 t = q;
+    if (sample_log2) {
+      t = (q << sample_log2) + (i64)(sel_mix((unsigned long long)q) & ((1ull << sample_log2) - 1));
+      if (t >= total) continue;
+    }
     double v = a.V[t];
     if (!(v > 0.0)) continue;
     int m = (int)(t / a.per_m);
@@ -221,28 +236,55 @@ __global__ void k_sel_hist(SelArgs a, const SelState* st, int shift, int nbits, 
   for (int i = threadIdx.x; i < 4096; i += blockDim.x)
     if (sh[i]) atomicAdd(&hist[i], sh[i]);
 }
-__global__ void k_sel_resolve(SelState* st, unsigned* hist, int shift, int nbits, int first, unsigned long long cap) {
-  if (threadIdx.x || blockIdx.x) return;
-  const int nbin = 1 << nbits;
-  unsigned long long cum = 0;
-  int found = -1;
-  for (int b = nbin - 1; b >= 0; b--) {
-    unsigned long long hb = hist[b];
-    if (cum + hb >= st->want) { found = b; break; }
-    cum += hb;
+// Locates the bin (scanning from the top) that holds the `want`-th largest key.  One CTA of 1024 threads,
+// 4 bins per thread in descending order, block-wide inclusive scan.
+__global__ void __launch_bounds__(1024) k_sel_resolve(SelState* st, unsigned* hist, int shift, int nbits, int first,
+                                                      unsigned long long cap) {
+  __shared__ unsigned long long sc[1024];
+  __shared__ int s_found;
+  __shared__ unsigned long long s_cum, s_inbin;
+  const int tid = threadIdx.x, nbin = 1 << nbits;
+  if (tid == 0) s_found = -1;
+  unsigned hb[4];
+  unsigned long long sum = 0;
+#pragma unroll
+  for (int j = 0; j < 4; j++) {
+    int b = nbin - 1 - (4 * tid + j);
+    hb[j] = b >= 0 ? hist[b] : 0u;
+    sum += hb[j];
   }
+  sc[tid] = sum;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    unsigned long long v = tid >= o ? sc[tid - o] : 0ull;
+    __syncthreads();
+    sc[tid] += v;
+    __syncthreads();
+  }
+  const unsigned long long want = st->want;
+  unsigned long long cum = sc[tid] - sum;
+#pragma unroll
+  for (int j = 0; j < 4; j++) {
+    int b = nbin - 1 - (4 * tid + j);
+    if (b >= 0 && cum < want && cum + hb[j] >= want) { s_found = b; s_cum = cum; s_inbin = hb[j]; }
+    cum += hb[j];
+  }
+  const unsigned long long totalc = sc[1023];
+  __syncthreads();
+  for (int b = tid; b < 4096; b += 1024) hist[b] = 0;
+  if (tid) return;
+  const int found = s_found;
   if (found < 0) {            // fewer candidates than wanted: take everything positive
     st->takeall = 1; st->done = 1; st->thresh = 1ull;
-    st->inbin = 0; st->above += cum;
+    st->inbin = 0; st->above += totalc;
   } else {
     st->prefix = first ? (unsigned long long)found : ((st->prefix << nbits) | (unsigned long long)found);
-    st->want -= cum;
-    st->above += cum;
-    st->inbin = hist[found];
+    st->want -= s_cum;
+    st->above += s_cum;
+    st->inbin = s_inbin;
     st->thresh = st->prefix << shift;
     if (st->above + st->inbin <= cap || shift == 0) st->done = 1;
   }
-  for (int b = 0; b < 4096; b++) hist[b] = 0;
 }
 struct Raw { int m; int i; int a; int ch; };
 __global__ void k_sel_collect(SelArgs a, const SelState* st, Raw* out, unsigned* count, unsigned cap) {
@@ -263,6 +305,65 @@ __global__ void k_sel_collect(SelArgs a, const SelState* st, Raw* out, unsigned*
         unsigned idx = atomicAdd(count, 1u);
         if (idx < cap) out[idx] = Raw{m, i, aa, ch};
       }
+    }
+  }
+}
+// fmx[m][cl] = max_ch fcd(m, cl, ch): upper bound used to reject whole (m,i,a) entries with one compare
+__global__ void k_sel_fmax(SelArgs a, double* fmx) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= a.nb * a.nCl) return;
+  int m = t / a.nCl, cl = t % a.nCl;
+  double mx = 0.0;
+  for (int ch = 0; ch < a.nCh; ch++) mx = fmax(mx, sel_fcd(a, m, cl, ch));
+  fmx[t] = mx;
+}
+// Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).
+__global__ void k_sel_prefilter(SelArgs a, const SelState* st, const double* fmx, double* keys, Raw* out, unsigned* count,
+                                unsigned cap) {
+  double thr = __longlong_as_double((long long)st->thresh);
+  thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
+  const i64 total = (i64)a.nb * a.per_m;
+  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+    double v = a.V[t];
+    if (!(v > 0.0)) continue;
+    int m = (int)(t / a.per_m);
+    i64 rem = t % a.per_m;
+    int i = (int)(rem / a.nA), aa = (int)(rem % a.nA);
+    int cl = i % a.nCl;
+    double vs = v * a.scale[m];
+    if (!(vs * fmx[m * a.nCl + cl] >= thr)) continue;
+    for (int ch = 0; ch < a.nCh; ch++) {
+      double r = vs * sel_fcd(a, m, cl, ch);
+      if (r > 0.0 && r >= thr) {
+        unsigned idx = atomicAdd(count, 1u);
+        if (idx < cap) { keys[idx] = r; out[idx] = Raw{m, i, aa, ch}; }
+      }
+    }
+  }
+}
+// radix digit histogram / final compaction on the compact key list
+__global__ void k_csel_hist(const double* keys, unsigned n, const SelState* st, int shift, int nbits, int first, unsigned* hist) {
+  __shared__ unsigned sh[4096];
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sh[i] = 0;
+  __syncthreads();
+  const unsigned long long prefix = st->prefix;
+  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x) {
+    unsigned long long key = (unsigned long long)__double_as_longlong(keys[t]);
+    if (!first && (key >> (shift + nbits)) != prefix) continue;
+    atomicAdd(&sh[(key >> shift) & ((1u << nbits) - 1)], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x)
+    if (sh[i]) atomicAdd(&hist[i], sh[i]);
+}
+__global__ void k_csel_compact(const double* keys, const Raw* in, unsigned n, const SelState* st, Raw* out, unsigned* count,
+                               unsigned cap) {
+  double thr = __longlong_as_double((long long)st->thresh);
+  thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
+  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x) {
+    if (keys[t] >= thr) {
+      unsigned idx = atomicAdd(count, 1u);
+      if (idx < cap) out[idx] = in[t];
     }
   }
 }
@@ -430,6 +531,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   DBuf<SelState> sel(h, 1);
   DBuf<unsigned> hist(h, 4096), count(h, 1);
   DBuf<Raw> raw(h, cap);
+  const unsigned ccap = 1u << 22;                   // compact candidate list of the prefilter pass
+  DBuf<double> ckeys(h, ccap), fmx(h, (size_t)M * 16);
+  DBuf<Raw> craw(h, ccap);
   DBuf<Cand> cand(h, npad);
   unsigned* st_cur = stA.p; unsigned* st_nxt = stB.p;
   double* lp_cur = lpA.p; double* lp_nxt = lpB.p;
@@ -558,18 +662,62 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       const int shifts[6] = {52, 40, 28, 16, 4, 0}, nbitsv[6] = {12, 12, 12, 12, 12, 4};
       const i64 total = (i64)nb * per_m;
       const int gsel = (int)std::min<i64>(148 * 8, (total + 255) / 256);
-      for (int pass = 0; pass < 6; pass++) {
-        k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, hist.p);
+      unsigned ncand = 0;
+      bool direct = total * c.nCh <= (i64)h->select_direct_max;       // few candidates: radix passes straight on V
+      if (!direct) {
+        // (1) lower bound of the (M+1)-th largest key from a hashed 1/64 sample of V (two radix digits)
+        for (int pass = 0; pass < 2; pass++) {
+          k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
+          TN_LAUNCH_CHECK(h);
+          k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, 0ull);
+          TN_LAUNCH_CHECK(h);
+        }
+        // (2) one pass over V: everything at or above the bound goes to the compact list
+        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
         TN_LAUNCH_CHECK(h);
-        k_sel_resolve<<<1, 32, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, cap);
+        TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+        k_sel_prefilter<<<gsel, 256, 0, h->stream>>>(sa, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap);
         TN_LAUNCH_CHECK(h);
-        SelState cur = d2h(h, sel.p);
-        if (cur.done) break;
+        const unsigned n1 = d2h(h, count.p);
+        if (n1 > ccap) {
+          direct = true;                              // massive ties at the bound: fall back to the direct passes
+        } else if (n1 <= cap) {
+          ncand = n1;
+          TN_CUDA(cudaMemcpyAsync(raw.p, craw.p, sizeof(Raw) * n1, cudaMemcpyDeviceToDevice, h->stream));
+        } else {
+          // (3) exact radix selection on the compact keys
+          TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
+          const int gc = (int)std::min<i64>(148 * 4, ((i64)n1 + 255) / 256);
+          for (int pass = 0; pass < 6; pass++) {
+            k_csel_hist<<<gc, 256, 0, h->stream>>>(ckeys.p, n1, sel.p, shifts[pass], nbitsv[pass], pass == 0, hist.p);
+            TN_LAUNCH_CHECK(h);
+            k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, cap);
+            TN_LAUNCH_CHECK(h);
+            SelState cur = d2h(h, sel.p);
+            if (cur.done) break;
+          }
+          TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+          k_csel_compact<<<gc, 256, 0, h->stream>>>(ckeys.p, craw.p, n1, sel.p, raw.p, count.p, cap);
+          TN_LAUNCH_CHECK(h);
+          ncand = std::min(d2h(h, count.p), cap);
+        }
       }
-      TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
-      k_sel_collect<<<gsel, 256, 0, h->stream>>>(sa, sel.p, raw.p, count.p, cap);
-      TN_LAUNCH_CHECK(h);
-      unsigned ncand = std::min(d2h(h, count.p), cap);
+      if (direct) {
+        TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
+        TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
+        for (int pass = 0; pass < 6; pass++) {
+          k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 0, hist.p);
+          TN_LAUNCH_CHECK(h);
+          k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, cap);
+          TN_LAUNCH_CHECK(h);
+          SelState cur = d2h(h, sel.p);
+          if (cur.done) break;
+        }
+        TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+        k_sel_collect<<<gsel, 256, 0, h->stream>>>(sa, sel.p, raw.p, count.p, cap);
+        TN_LAUNCH_CHECK(h);
+        ncand = std::min(d2h(h, count.p), cap);
+      }
       if (ncand == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
       unsigned np2 = 2;
       while (np2 < ncand + 1) np2 <<= 1;   // at least one sentinel so that cand[M] exists when ncand <= M

@@ -84,6 +84,7 @@ struct tn_handle {
   // options
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512;
   double svd_tol = 1e-11;
+  i64 select_direct_max = 1ll << 22;
   // runtime
   cudaStream_t stream = nullptr;
   void* (*alloc_cb)(size_t, void*) = nullptr;

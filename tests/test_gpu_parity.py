@@ -34,9 +34,11 @@ def run_oracle(inst, beta, D, sweeps, M):
     return m, R, ln, out
 
 
-def compare(inst, beta, D, sweeps, M, tol, check_rows=True):
+def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=()):
     m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M)
     with _tn(inst) as t:
+        for key, val in options:
+            t.set_option(key, val)
         t.set_beta(beta)
         t.contract(D, sweeps)
         if check_rows:
@@ -105,6 +107,15 @@ TRUNC = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M)
 def test_truncated_contraction_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M):
     inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
     compare(inst, beta, D, sweeps, M, 1e-6)
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,D,sweeps,M", [TRUNC[3], TRUNC[4], TRUNC[6]])
+def test_sampled_prefilter_selection_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M):
+    """Top-M through the hashed-sample lower bound + prefilter + compact radix passes (the route taken at the
+    BASELINE.json sizes), forced here by TN_OPT_SELECT_DIRECT_MAX = 0."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    compare(inst, beta, D, sweeps, M, 1e-6, check_rows=False, options=[(tnb.OPT_SELECT_DIRECT_MAX, 0)])
 
 
 def test_zero_field_z2_instance():
