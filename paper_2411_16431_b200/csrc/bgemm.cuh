@@ -1,0 +1,119 @@
+// Batched small-K FP64 tensor-core GEMM with a fused weight epilogue.
+//
+//   C(batch; i, j) = weight(batch, i, j) * sum_{k < K} A(batch; i, k) * B(batch; k, j),      K <= 64 (a bond dimension)
+//
+// This is the shape of the two "project -> batched D x D product -> Boltzmann factor" diagrams of Fig. 7
+// once the cell weight is factorised: the Theta-core build (batch = MPO-bond state k, rows
+// (x, b), K = old bond) and the search conditionals (batch = beam element, rows (b, c_lo), columns a, K = bond
+// of R_{y+1}).  With K <= 64 each output costs <= 128 FLOP, i.e. <= 16 FLOP per byte written: the kernel is bound
+// by the HBM WRITE of C, so the whole K extent of both operands is staged in shared memory once per CTA (no k
+// pipeline), rows of A are gathered through the projector tables by a row-pointer functor, and all weights are
+// applied in registers before the only global store.
+//
+//   AR: const double* operator()(int batch, int i)      -> pointer to the K contiguous doubles of row i
+//   BE: double operator()(int batch, int k, int j)      -> element of B
+//   EP: Row row(int batch, int i);  put(const Row&, batch, j, v);  put2(const Row&, batch, j, v0, v1) (columns j, j+1)
+#pragma once
+#include "gemm.cuh"
+
+// A_SHARED: the rows of A do not depend on the batch -> one CTA keeps its A tile in shared memory and walks
+// over `bg` consecutive batches (cuts the L2 -> SM read traffic, which otherwise equals the write traffic).
+// Every CTA also walks over all column tiles of its rows with the same A tile.
+template <int KP, int NT, bool A_SHARED, class AR, class BE, class EP>
+__global__ void __launch_bounds__(256, 2) k_bgemm(int batches, int bg, int M, int N, int K, AR ar, BE be, EP ep) {
+  constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
+  extern __shared__ __align__(16) double bg_smem[];
+  double* sA = bg_smem;
+  double* sB = bg_smem + BM * LDA;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int m0 = blockIdx.y * BM;
+  const int b0 = blockIdx.x * bg, b1 = min(batches, b0 + bg);
+  for (int batch = b0; batch < b1; batch++) {
+    if (!A_SHARED || batch == b0) {
+      __syncthreads();
+      for (int r = warp; r < BM; r += 8) {
+        const int gi = m0 + r;
+        const double* src = gi < M ? ar(batch, gi) : nullptr;
+#pragma unroll
+        for (int k = lane; k < KP; k += 32) sA[r * LDA + k] = (src && k < K) ? __ldg(src + k) : 0.0;
+      }
+    }
+    for (int n0 = 0; n0 < N; n0 += BN) {
+      __syncthreads();
+      for (int idx = tid; idx < KP * BN; idx += 256) {
+        const int k = idx / BN, j = idx % BN;
+        sB[k * LDB + j] = (k < K && n0 + j < N) ? be(batch, k, n0 + j) : 0.0;
+      }
+      __syncthreads();
+      double acc[2][NT][2];
+#pragma unroll
+      for (int i = 0; i < 2; i++)
+#pragma unroll
+        for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+      for (int kk = 0; kk < KP; kk += 4) {
+        const double fa0 = sA[(16 * warp + (lane >> 2)) * LDA + kk + (lane & 3)];
+        const double fa1 = sA[(16 * warp + 8 + (lane >> 2)) * LDA + kk + (lane & 3)];
+        const double* brow = sB + (kk + (lane & 3)) * LDB + (lane >> 2);
+#pragma unroll
+        for (int j = 0; j < NT; j++) {
+          const double fb = brow[8 * j];
+          dmma884(acc[0][j][0], acc[0][j][1], fa0, fb);
+          dmma884(acc[1][j][0], acc[1][j][1], fa1, fb);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < 2; i++) {
+        const int row = m0 + 16 * warp + 8 * i + (lane >> 2);
+        if (row < M) {
+          const typename EP::Row rc = ep.row(batch, row);
+#pragma unroll
+          for (int j = 0; j < NT; j++) {
+            const int col = n0 + 8 * j + 2 * (lane & 3);
+            if (col + 1 < N) ep.put2(rc, batch, col, acc[i][j][0], acc[i][j][1]);
+            else if (col < N) ep.put(rc, batch, col, acc[i][j][0]);
+          }
+        }
+      }
+    }
+  }
+}
+
+template <int KP, int NT, bool A_SHARED, class AR, class BE, class EP>
+void launch_bgemm_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BE& be, const EP& ep) {
+  constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
+  constexpr int smem = (int)sizeof(double) * (BM * LDA + KP * LDB);
+  static bool attr = false;
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_bgemm<KP, NT, A_SHARED, AR, BE, EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    attr = true;
+  }
+  const int mt = (M + BM - 1) / BM;
+  int bg = 1;
+  if (A_SHARED) {   // as many batches per CTA as still leave >= 4 waves of CTAs
+    bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (4 * 296)));
+  }
+  dim3 grid((unsigned)((batches + bg - 1) / bg), (unsigned)mt);
+  k_bgemm<KP, NT, A_SHARED, AR, BE, EP><<<grid, 256, smem, h->stream>>>(batches, bg, M, N, K, ar, be, ep);
+  h->st.kernel_launches++;
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) tn_throw(TN_ERR_CUDA, "k_bgemm launch failed: %s", cudaGetErrorString(e));
+}
+
+template <int KP, bool A_SHARED, class AR, class BE, class EP>
+void launch_bgemm_k(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BE& be, const EP& ep) {
+  if (N <= 16) launch_bgemm_knt<KP, 2, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  else if (N <= 32) launch_bgemm_knt<KP, 4, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  else launch_bgemm_knt<KP, 8, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+}
+
+// K <= 64 only (returns false otherwise: the caller keeps its generic k_gemm path for exact-mode bonds).
+template <bool A_SHARED, class AR, class BE, class EP>
+bool launch_bgemm(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BE& be, const EP& ep) {
+  if (K < 1 || K > 64 || batches < 1 || M < 1 || N < 1 || (M + 127) / 128 > 65535) return false;
+  if (K <= 16) launch_bgemm_k<16, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  else if (K <= 32) launch_bgemm_k<32, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  else if (K <= 48) launch_bgemm_k<48, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  else launch_bgemm_k<64, A_SHARED>(h, batches, M, N, K, ar, be, ep);
+  return true;
+}

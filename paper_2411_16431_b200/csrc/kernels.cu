@@ -1,5 +1,6 @@
 // Shared device kernels: GEMM launchers, Jacobi, orthonormalisation, projector maps, Theta-core.
 #include "kernels.cuh"
+#include "bgemm.cuh"
 #include <cstdarg>
 
 // ============================================================================================
@@ -196,6 +197,20 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
   __syncthreads();
   const int ce = c + (c & 1);
   const double tol = 1e-15;
+  // ||M||_F^2 (invariant under the rotations): rows below 1e-33 of it (norm < 3e-17 sigma_1, far under the rank
+  // cut of reading S6) are left alone -- pairs of noise rows would otherwise keep rotating for all 60 sweeps.
+  for (int p = warp; p < c; p += nwarp) {
+    double a = 0;
+    for (int i = lane; i < r; i += 32) { double u = Mw[(size_t)p * r + i]; a += u * u; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (lane == 0) s_norm[p] = a;
+  }
+  __syncthreads();
+  double fro2 = 0.0;
+  for (int p = 0; p < c; p++) fro2 += s_norm[p];
+  const double negl = 1e-33 * fro2;
+  __syncthreads();
   if (c > 1) {
     for (int sweep = 0; sweep < 60; sweep++) {
       if (tid == 0) s_rot = 0;
@@ -220,7 +235,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
             b += __shfl_xor_sync(0xffffffffu, b, o);
             g += __shfl_xor_sync(0xffffffffu, g, o);
           }
-          if (fabs(g) > tol * sqrt(a * b) && a > 0.0 && b > 0.0) {
+          if (fmin(a, b) > negl && fabs(g) > tol * sqrt(a) * sqrt(b)) {
             double zeta = (b - a) / (2.0 * g);
             double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
             double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
@@ -483,13 +498,43 @@ static void launch_theta(tn_handle* h, const CellDev& c, const double* A, int dx
   k_gemm<64, BN, 16, 4, 1, true, true, LdThA, LdThE, StTh><<<grid, 128, 0, h->stream>>>(M, g, dy, 1, a, b, e);
   TN_LAUNCH_CHECK(h);
 }
+// small-K route (bgemm.cuh): rows gathered through Pd by pointer, weight hoisted to one product per output row
+struct ArTh {
+  const double* A;
+  const int* Pd;
+  int nB, pd, dy;
+  __device__ __forceinline__ const double* operator()(int, int i) const {
+    return A + ((i64)(i / nB) * pd + Pd[i % nB]) * dy;
+  }
+};
+struct EpTh {
+  double* Tc;
+  const double *wA, *X, *Yc;
+  int nK, nB, nCl, tshift, g;
+  struct Row { double* p; double w; };
+  __device__ __forceinline__ Row row(int k, int i) const {
+    const int x = i / nB, b = i % nB, a = k / nCl, cl = k % nCl;
+    return Row{Tc + (((i64)x * nK + k) * nB + b) * g, wA[a] * X[(a >> tshift) * nB + b] * Yc[b * nCl + cl]};
+  }
+  __device__ __forceinline__ void put(const Row& r, int, int j, double v) const { r.p[j] = v * r.w; }
+  __device__ __forceinline__ void put2(const Row& r, int, int j, double v0, double v1) const {
+    if (((g | j) & 1) == 0) *reinterpret_cast<double2*>(r.p + j) = make_double2(v0 * r.w, v1 * r.w);   // 16-byte store
+    else { r.p[j] = v0 * r.w; r.p[j + 1] = v1 * r.w; }
+  }
+};
 void theta_core(tn_handle* h, const CellDev& c, const double* A, int dx, int dy, const double* Ek, int g,
                 double* Tc) {
+  h->st.flop_theta_build += 2.0 * dx * c.nB * (double)c.nK * dy * g;
+  {
+    ArTh ar{A, c.Pd, c.nB, c.n_d, dy};
+    LdThE be{Ek, c.nK, g};
+    EpTh ep{Tc, c.wA, c.X, c.Yc, c.nK, c.nB, c.nCl, c.tshift, g};
+    if (launch_bgemm<true>(h, c.nK, dx * c.nB, g, dy, ar, be, ep)) return;
+  }
   if (g <= 16) launch_theta<16>(h, c, A, dx, dy, Ek, g, Tc);
   else if (g <= 32) launch_theta<32>(h, c, A, dx, dy, Ek, g, Tc);
   else if (g <= 48) launch_theta<48>(h, c, A, dx, dy, Ek, g, Tc);
   else launch_theta<64>(h, c, A, dx, dy, Ek, g, Tc);
-  h->st.flop_theta_build += 2.0 * dx * c.nB * (double)c.nK * dy * g;
 }
 
 // ============================================================================================

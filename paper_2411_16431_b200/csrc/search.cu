@@ -9,6 +9,7 @@
 //                    * sum_{b''} LG_m[(Pd b, Po cl)][b''] RM_{m,x}[b''][Pr a],     LG_m = Lv_m . (S Q)
 //   hS = BhS_x[Pr(a of the cell on the left)], vS = BvS_x[Pd(b of the cell above)], dvec = Bd_x[Po(c_lo of upper-left)].
 #include "kernels.cuh"
+#include "bgemm.cuh"
 #include <algorithm>
 #include <cfloat>
 
@@ -51,6 +52,37 @@ struct StPV {
     V[(i64)m * per_m + (i64)i * nA + a] = acc * w;
   }
 };
+// small-K route (bgemm.cuh) for the conditionals: row pointer into LG, column weights cs[m][a] = hS wA precomputed
+struct ArPV {
+  const double* LG; const int *Pd, *Po; int nCl, n_o, npp, Dr;
+  __device__ __forceinline__ const double* operator()(int m, int i) const {
+    return LG + ((i64)m * npp + Pd[i / nCl] * n_o + Po[i % nCl]) * Dr;
+  }
+};
+struct EpPV {
+  double* V; const double *cs, *X, *vS, *Yc; const int *vrow, *slot;
+  int nA, nB, nCl, tshift; i64 per_m;
+  struct Row { double* p; const double* x; const double* c; double w; };
+  __device__ __forceinline__ Row row(int m, int i) const {
+    const int b = i / nCl, cl = i % nCl;
+    return Row{V + (i64)m * per_m + (i64)i * nA, X + b, cs + (i64)m * nA, vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl]};
+  }
+  __device__ __forceinline__ void put(const Row& r, int, int a, double v) const {
+    r.p[a] = v * r.w * r.c[a] * r.x[(a >> tshift) * nB];
+  }
+  __device__ __forceinline__ void put2(const Row& r, int, int a, double v0, double v1) const {
+    const double x0 = r.x[(a >> tshift) * nB], x1 = r.x[((a + 1) >> tshift) * nB];
+    if (((nA | a) & 1) == 0) *reinterpret_cast<double2*>(r.p + a) = make_double2(v0 * r.w * r.c[a] * x0, v1 * r.w * r.c[a + 1] * x1);
+    else { r.p[a] = v0 * r.w * r.c[a] * x0; r.p[a + 1] = v1 * r.w * r.c[a + 1] * x1; }
+  }
+};
+// cs[m][a] = hS[hrow[m]][a] * wA[a]
+__global__ void k_colscale(const double* hS, const double* wA, const int* hrow, int nb, int nA, double* cs) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nb * nA) return;
+  int m = t / nA, a = t % nA;
+  cs[t] = hS[(i64)hrow[m] * nA + a] * wA[a];
+}
 struct LdHA {   // A(i=(b',b''), kk=(b,cl)) = G[(Pd b * n_o + Po cl)][i]
   const double* G; const int *Pd, *Po; int nCl, n_o; i64 DD;
   __device__ __forceinline__ double operator()(int, int i, int kk) const {
@@ -143,20 +175,31 @@ __global__ void k_norm_rm(double* RM, int per_m, const double* ls_in, double* ls
     for (int i = threadIdx.x; i < per_m; i += blockDim.x) p[i] /= mx;
   if (threadIdx.x == 0) ls_out[m] = ls_in[m] + (mx > 0.0 ? log(mx) : 0.0);
 }
-// Z[m] = sum max(v,0) fc[m][cl]; negatives counted and clamped in place (reading S7)
-__global__ void k_beam_Z(double* V, i64 per_m, int nA, int nCl, const double* fc, double* Z, unsigned long long* nneg) {
+// Z[m] = sum max(v,0) fc[m][cl]; negatives / NaNs counted and clamped in place (reading S7).  Grid (chunk, m):
+// every CTA streams one contiguous chunk of V[m] with 16-byte loads; nA, nCl are powers of two (2^n_s, 2^(n_s/2)).
+// Partial sums go to part[m][chunk]; k_beam_Z_final adds them in chunk order (deterministic).
+__global__ void __launch_bounds__(256) k_beam_Z(double* V, i64 per_m, int lgA, int nCl, const double* fc, double* part,
+                                                unsigned long long* nneg) {
   __shared__ double sh[256];
-  __shared__ unsigned long long shn[256];
-  int m = blockIdx.x;
-  double* v = V + (i64)m * per_m;
+  __shared__ unsigned shn[256];
+  const int m = blockIdx.y, nchunk = gridDim.x;
+  const i64 per2 = per_m >> 1;                          // per_m is even (a power of two >= 4)
+  const i64 c0 = per2 * blockIdx.x / nchunk, c1 = per2 * (blockIdx.x + 1) / nchunk;
+  double2* v2 = reinterpret_cast<double2*>(V + (i64)m * per_m);
+  const double* fcm = fc + (i64)m * nCl;
   double s = 0.0;
-  unsigned long long neg = 0;
-  for (i64 i = threadIdx.x; i < per_m; i += blockDim.x) {
-    double x = v[i];
-    if (x < 0.0) { neg++; x = 0.0; v[i] = 0.0; }
-    if (!(x == x)) { x = 0.0; v[i] = 0.0; }
-    int cl = (int)((i / nA) % nCl);
-    s += x * fc[(i64)m * nCl + cl];
+  unsigned neg = 0;
+  for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
+    double2 x = v2[q];
+    const bool bad0 = !(x.x >= 0.0), bad1 = !(x.y >= 0.0);
+    if (bad0 | bad1) {
+      neg += (x.x < 0.0) + (x.y < 0.0);
+      if (bad0) x.x = 0.0;
+      if (bad1) x.y = 0.0;
+      v2[q] = x;
+    }
+    const int cl = (int)(((2 * q) >> lgA) & (nCl - 1));   // both entries share (b, cl): nA is even
+    s += (x.x + x.y) * fcm[cl];
   }
   sh[threadIdx.x] = s; shn[threadIdx.x] = neg;
   __syncthreads();
@@ -164,7 +207,14 @@ __global__ void k_beam_Z(double* V, i64 per_m, int nA, int nCl, const double* fc
     if (threadIdx.x < o) { sh[threadIdx.x] += sh[threadIdx.x + o]; shn[threadIdx.x] += shn[threadIdx.x + o]; }
     __syncthreads();
   }
-  if (threadIdx.x == 0) { Z[m] = sh[0]; if (shn[0]) atomicAdd(nneg, shn[0]); }
+  if (threadIdx.x == 0) { part[(i64)m * nchunk + blockIdx.x] = sh[0]; if (shn[0]) atomicAdd(nneg, (unsigned long long)shn[0]); }
+}
+__global__ void k_beam_Z_final(const double* part, int nb, int nchunk, double* Z) {
+  int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= nb) return;
+  double s = 0.0;
+  for (int c = 0; c < nchunk; c++) s += part[(i64)m * nchunk + c];
+  Z[m] = s;
 }
 // scale[m] = exp(logp[m] - max logp) / Z[m]
 __global__ void k_beam_scale(const double* logp, const double* Z, int nb, double* scale) {
@@ -317,26 +367,35 @@ __global__ void k_sel_fmax(SelArgs a, double* fmx) {
   for (int ch = 0; ch < a.nCh; ch++) mx = fmax(mx, sel_fcd(a, m, cl, ch));
   fmx[t] = mx;
 }
-// Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).
-__global__ void k_sel_prefilter(SelArgs a, const SelState* st, const double* fmx, double* keys, Raw* out, unsigned* count,
-                                unsigned cap) {
+// Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).  Grid (chunk, m),
+// 16-byte loads, shifts instead of divisions (nA, nCl powers of two); survivors are rare.
+__global__ void __launch_bounds__(256) k_sel_prefilter(SelArgs a, int lgA, const SelState* st, const double* fmx, double* keys,
+                                                       Raw* out, unsigned* count, unsigned cap) {
   double thr = __longlong_as_double((long long)st->thresh);
   thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
-  const i64 total = (i64)a.nb * a.per_m;
-  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
-    double v = a.V[t];
-    if (!(v > 0.0)) continue;
-    int m = (int)(t / a.per_m);
-    i64 rem = t % a.per_m;
-    int i = (int)(rem / a.nA), aa = (int)(rem % a.nA);
-    int cl = i % a.nCl;
-    double vs = v * a.scale[m];
-    if (!(vs * fmx[m * a.nCl + cl] >= thr)) continue;
-    for (int ch = 0; ch < a.nCh; ch++) {
-      double r = vs * sel_fcd(a, m, cl, ch);
-      if (r > 0.0 && r >= thr) {
-        unsigned idx = atomicAdd(count, 1u);
-        if (idx < cap) { keys[idx] = r; out[idx] = Raw{m, i, aa, ch}; }
+  const int m = blockIdx.y, nchunk = gridDim.x;
+  const i64 per2 = a.per_m >> 1;
+  const i64 c0 = per2 * blockIdx.x / nchunk, c1 = per2 * (blockIdx.x + 1) / nchunk;
+  const double2* v2 = reinterpret_cast<const double2*>(a.V + (i64)m * a.per_m);
+  const double sc = a.scale[m];
+  const double* fm = fmx + (i64)m * a.nCl;
+  for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
+    const double2 x = v2[q];
+    const int i = (int)((2 * q) >> lgA), cl = i & (a.nCl - 1);
+    const double bound = fmax(x.x, x.y) * sc * fm[cl];
+    if (!(bound >= thr) || !(bound > 0.0)) continue;
+#pragma unroll
+    for (int e = 0; e < 2; e++) {
+      const double v = e ? x.y : x.x;
+      if (!(v > 0.0)) continue;
+      const double vs = v * sc;
+      const int aa = (int)((2 * q + e) & (a.nA - 1));
+      for (int ch = 0; ch < a.nCh; ch++) {
+        double r = vs * sel_fcd(a, m, cl, ch);
+        if (r > 0.0 && r >= thr) {
+          unsigned idx = atomicAdd(count, 1u);
+          if (idx < cap) { keys[idx] = r; out[idx] = Raw{m, i, aa, ch}; }
+        }
       }
     }
   }
@@ -626,17 +685,32 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         h->st.flop_search += 2.0 * nb * (double)Ng * Dl;
       }
       {   // V[m][(b,cl)][a]
-        LdPA a{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
-        LdPB b{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r};
-        StPV e{V.p, c.BhS, c.wA, c.X, c.BvS, c.Yc, hrow.p, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
         int Mg = c.nB * c.nCl, Ng = c.nA;
-        dim3 grid(nb, cdiv(Mg, 64), cdiv(Ng, 64));
-        k_gemm<64, 64, 16, 2, 2, true, true, LdPA, LdPB, StPV><<<grid, 128, 0, h->stream>>>(Mg, Ng, Dr, 1, a, b, e);
-        TN_LAUNCH_CHECK(h);
         h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
+        DBuf<double> cs(h, (size_t)nb * c.nA);
+        k_colscale<<<cdiv((i64)nb * c.nA, 256), 256, 0, h->stream>>>(c.BhS, c.wA, hrow.p, nb, c.nA, cs.p);
+        TN_LAUNCH_CHECK(h);
+        ArPV ar{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
+        LdPB be{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r};
+        EpPV ep{V.p, cs.p, c.X, c.BvS, c.Yc, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
+        if (!launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
+          LdPA a{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
+          StPV e{V.p, c.BhS, c.wA, c.X, c.BvS, c.Yc, hrow.p, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
+          dim3 grid(nb, cdiv(Mg, 64), cdiv(Ng, 64));
+          k_gemm<64, 64, 16, 2, 2, true, true, LdPA, LdPB, StPV><<<grid, 128, 0, h->stream>>>(Mg, Ng, Dr, 1, a, be, e);
+          TN_LAUNCH_CHECK(h);
+        }
       }
-      k_beam_Z<<<nb, 256, 0, h->stream>>>(V.p, per_m, c.nA, c.nCl, fc.p, Z.p, nneg.p);
-      TN_LAUNCH_CHECK(h);
+      {
+        int lgA = 0;
+        while ((1 << lgA) < c.nA) lgA++;
+        const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
+        DBuf<double> zpart(h, (size_t)nb * nchunk);
+        k_beam_Z<<<dim3(nchunk, nb), 256, 0, h->stream>>>(V.p, per_m, lgA, c.nCl, fc.p, zpart.p, nneg.p);
+        TN_LAUNCH_CHECK(h);
+        k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, nchunk, Z.p);
+        TN_LAUNCH_CHECK(h);
+      }
       t_c.stop();
       if (y == 0 && x == 0) {
         double z0 = d2h(h, Z.p), ls0 = d2h(h, rt[0].ls);
@@ -676,7 +750,12 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
         TN_LAUNCH_CHECK(h);
         TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
-        k_sel_prefilter<<<gsel, 256, 0, h->stream>>>(sa, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap);
+        {
+          int lgA = 0;
+          while ((1 << lgA) < c.nA) lgA++;
+          const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
+          k_sel_prefilter<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap);
+        }
         TN_LAUNCH_CHECK(h);
         const unsigned n1 = d2h(h, count.p);
         if (n1 > ccap) {
