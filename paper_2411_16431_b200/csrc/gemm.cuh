@@ -158,6 +158,8 @@ void gemm_general(tn_handle* h, const GemmDesc& g);
 // trans = true: C[K x N] = A[M x K]^T B[M x N].  Returns false if shape / alignment do not fit.
 bool tsgemm(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb, double* C,
             i64 ldc);
+bool tsgemm_batched(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb,
+                    i64 sB, double* C, i64 ldc, i64 sC, int nbatch);
 // plain row-major helpers: C[M,N] = op(A) op(B)
 void gemm_rm(tn_handle* h, bool ta, bool tb, int M, int N, int K, const double* A, int lda, const double* B,
              int ldb, double* C, int ldc, double alpha = 1.0, double beta = 0.0);

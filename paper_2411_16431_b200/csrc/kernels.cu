@@ -69,12 +69,29 @@ void gemm_general(tn_handle* h, const GemmDesc& g) {
   }
 }
 
+// out[k][j] = in[j][k] (j < N), zero in the pad column
+__global__ void k_transpose_pad(double* out, const double* in, int K, int N, int ldt, int ldb) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= K * ldt) return;
+  int k = t / ldt, j = t % ldt;
+  out[t] = j < N ? in[(i64)j * ldb + k] : 0.0;
+}
+
 void gemm_rm(tn_handle* h, bool ta, bool tb, int M, int N, int K, const double* A, int lda, const double* B,
              int ldb, double* C, int ldc, double alpha, double beta) {
   if (M <= 0 || N <= 0) return;
-  if (!tb && alpha == 1.0 && beta == 0.0 && K > 0) {   // tall x skinny: streaming cp.async kernel (tsgemm.cu)
-    if (!ta && tsgemm(h, false, M, N, K, A, lda, B, ldb, C, ldc)) return;
-    if (ta && tsgemm(h, true, K, N, M, A, lda, B, ldb, C, ldc)) return;
+  if (alpha == 1.0 && beta == 0.0 && K > 0) {   // streaming cp.async kernel (tsgemm.cu)
+    if (!tb) {
+      if (!ta && tsgemm(h, false, M, N, K, A, lda, B, ldb, C, ldc)) return;
+      if (ta && tsgemm(h, true, K, N, M, A, lda, B, ldb, C, ldc)) return;
+    } else if ((i64)N * K <= 65536) {             // small B given transposed: transpose it first
+      const int ldt = (N + 1) & ~1;
+      DBuf<double> Bt(h, (size_t)K * ldt);
+      k_transpose_pad<<<cdiv((i64)K * ldt, 256), 256, 0, h->stream>>>(Bt.p, B, K, N, ldt, ldb);
+      TN_LAUNCH_CHECK(h);
+      if (!ta && tsgemm(h, false, M, N, K, A, lda, Bt.p, ldt, C, ldc)) return;
+      if (ta && tsgemm(h, true, K, N, M, A, lda, Bt.p, ldt, C, ldc)) return;
+    }
   }
   GemmDesc g;
   g.M = M; g.N = N; g.K = K;
@@ -418,6 +435,7 @@ __global__ void k_map_RT(CellDev c, const double* Yk, double* Y, int outer, int 
 
 void map_L(tn_handle* h, const CellDev& c, bool fold, const double* Y, double* Yk, int outer, int s) {
   if (fold) {   // Yk[o][a][s] = sum_r BhS[r][a] Y[o][r][s]
+    if (tsgemm_batched(h, true, c.bh_rows, s, c.nA, c.BhS, c.nA, Y, s, (i64)c.bh_rows * s, Yk, s, (i64)c.nA * s, outer)) return;
     GemmDesc g;
     g.M = c.nA; g.N = s; g.K = c.bh_rows; g.B1 = outer;
     g.A = c.BhS; g.a_i = 1; g.a_k = c.nA;
@@ -433,6 +451,7 @@ void map_L(tn_handle* h, const CellDev& c, bool fold, const double* Y, double* Y
 }
 void map_LT(tn_handle* h, const CellDev& c, bool fold, const double* Yk, double* Y, int outer, int s) {
   if (fold) {   // Y[o][r][s] = sum_a BhS[r][a] Yk[o][a][s]
+    if (tsgemm_batched(h, false, c.bh_rows, s, c.nA, c.BhS, c.nA, Yk, s, (i64)c.nA * s, Y, s, (i64)c.bh_rows * s, outer)) return;
     GemmDesc g;
     g.M = c.bh_rows; g.N = s; g.K = c.nA; g.B1 = outer;
     g.A = c.BhS; g.a_i = c.nA; g.a_k = 1;

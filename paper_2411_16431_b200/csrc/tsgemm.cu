@@ -30,7 +30,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int NT, int WARPS, bool TRANS>
 __global__ void __launch_bounds__(WARPS * 32, (NT <= 10 || WARPS < 8) ? 2 : 1)
 k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i64 ldb, double* __restrict__ C, i64 ldc,
-         i64 Mout, int N, i64 Kred, i64 kper, double* __restrict__ ws) {
+         i64 Mout, int Nfull, i64 Kred, i64 kper, double* __restrict__ ws, int nz, i64 sBz, i64 sCz) {
   constexpr int BM = 16 * WARPS, NTH = 32 * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK);   // doubles
   constexpr int LDB = smem_ld(NP);
@@ -43,6 +43,10 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const i64 m0 = (i64)blockIdx.x * BM;
   const int split = blockIdx.y, nsplit = gridDim.y;
+  const int bz = blockIdx.z / nz;                    // batch (A shared, B and C strided)
+  const int n_off = (blockIdx.z % nz) * NP;          // column chunk (N > 96 is cut into chunks of NP columns)
+  const int N = min(NP, Nfull - n_off);
+  B += n_off + (i64)bz * sBz;
   const i64 k0 = (i64)split * kper, k1 = min(Kred, k0 + kper);
   const int nkt = k1 > k0 ? (int)((k1 - k0 + TS_BK - 1) / TS_BK) : 0;
 
@@ -121,8 +125,8 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
   }
   cp_async_wait<0>();
   // ---- epilogue
-  double* out = nsplit > 1 ? ws + (size_t)split * Mout * N : C;
-  const i64 ldo = nsplit > 1 ? N : ldc;
+  double* out = (nsplit > 1 ? ws + ((size_t)bz * nsplit + split) * Mout * Nfull : C + (i64)bz * sCz) + n_off;
+  const i64 ldo = nsplit > 1 ? Nfull : ldc;
 #pragma unroll
   for (int i = 0; i < 2; i++) {
     const i64 row = m0 + 16 * warp + 8 * i + (lane >> 2);
@@ -138,13 +142,18 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
 }
 
 // C[i][j] = sum_s ws[s][i][j]  (fixed order)
-__global__ void k_ts_reduce(const double* __restrict__ ws, int nsplit, i64 M, int N, double* __restrict__ C, i64 ldc) {
+__global__ void k_ts_reduce(const double* __restrict__ ws, int nsplit, i64 M, int N, double* __restrict__ C, i64 ldc,
+                            i64 sCz) {
   i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= M * N) return;
+  const int bz = blockIdx.y;
   double s = 0.0;
-  for (int sp = 0; sp < nsplit; sp++) s += ws[(size_t)sp * M * N + t];
-  C[(t / N) * ldc + t % N] = s;
+  for (int sp = 0; sp < nsplit; sp++) s += ws[((size_t)bz * nsplit + sp) * M * N + t];
+  C[(i64)bz * sCz + (t / N) * ldc + t % N] = s;
 }
+
+struct TsBatch { int n = 1; i64 sB = 0, sC = 0; };
+TsBatch g_tsb;   // set by tsgemm_batched around the dispatch (host-side, single-threaded per handle)
 
 template <int NT, int WARPS, bool TRANS>
 void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
@@ -159,12 +168,14 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
   }
   i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
   nsplit = (int)((Kred + kper - 1) / kper);
-  double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nsplit * Mout * N) : nullptr;
-  dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit);
-  k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws);
+  const int nbz = g_tsb.n, nz = (N + NP - 1) / NP;
+  double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nbz * nsplit * Mout * N) : nullptr;
+  dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit, (unsigned)(nz * nbz));
+  k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws, nz,
+                                                                     g_tsb.sB, g_tsb.sC);
   TN_LAUNCH_CHECK(h);
   if (nsplit > 1) {
-    k_ts_reduce<<<cdiv(Mout * N, 256), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc);
+    k_ts_reduce<<<dim3(cdiv(Mout * N, 256), nbz), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc, g_tsb.sC);
     TN_LAUNCH_CHECK(h);
     h->dfree(ws);
   }
@@ -177,7 +188,7 @@ template <int NT, bool TRANS>
 void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
                 i64 Kred) {
   int warps = Mout > 64 ? 8 : Mout > 32 ? 4 : 2;
-  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps);
+  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps) * ((N + 8 * NT - 1) / (8 * NT)) * g_tsb.n;
   const int slots = 148 * ((NT <= 10 || warps < 8) ? 2 : 1);
   const double t_k = 2.0 * 16 * warps * (8 * NT) * slots / 37e12;      // seconds per reduction index per CTA
   const double t_ws = (double)Mout * N * 16.0 / 6e12 + 2e-7;           // seconds per extra split (write + read)
@@ -197,7 +208,8 @@ void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb
 template <bool TRANS>
 void pick_nt(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
              i64 Kred) {
-  if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+  if (N > 96) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);          // chunks of 64 columns
+  else if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
   else if (N <= 32) pick_warps<4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
   else if (N <= 48) pick_warps<6, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
   else if (N <= 64) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
@@ -212,10 +224,25 @@ bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 // Returns false when the shapes / alignment do not fit (the caller falls back to the generic k_gemm).
 bool tsgemm(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb, double* C,
             i64 ldc) {
-  if (N < 1 || N > 96 || M < 1 || K < 1) return false;
-  if (getenv("TS_DISABLE")) return false;
+  if (N < 1 || M < 1 || K < 1) return false;
   if ((lda & 1) || (ldb & 1) || !aligned16(A) || !aligned16(B)) return false;
   if (trans) pick_nt<true>(h, A, lda, B, ldb, C, ldc, K, N, M);    // output rows = K (columns of A), reduce over M
   else pick_nt<false>(h, A, lda, B, ldb, C, ldc, M, N, K);
   return true;
+}
+
+// nbatch independent products with a shared A: B_z = B + z sB, C_z = C + z sC.
+bool tsgemm_batched(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb,
+                    i64 sB, double* C, i64 ldc, i64 sC, int nbatch) {
+  if (nbatch < 1 || nbatch > 16384 || (sB & 1)) return false;
+  g_tsb.n = nbatch; g_tsb.sB = sB; g_tsb.sC = sC;
+  bool ok = false;
+  try {
+    ok = tsgemm(h, trans, M, N, K, A, lda, B, ldb, C, ldc);
+  } catch (...) {
+    g_tsb = TsBatch();
+    throw;
+  }
+  g_tsb = TsBatch();
+  return ok;
 }
