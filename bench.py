@@ -83,6 +83,30 @@ def oracle_sample(inst, run, beta, rows=2):
     return t3 - t0, est, desc
 
 
+# ----------------------------------------------------------------------------------------------------
+# multi-rank plumbing (replicas only); backend-agnostic so that the gloo tests cover it
+# ----------------------------------------------------------------------------------------------------
+def replica_instance(config_index, rank):
+    """Rank r solves its own instance of the config: same shape, generator seed r."""
+    import instances
+    return instances.config(config_index, seed=rank)
+
+
+def max_over_ranks(v, world, device="cuda"):
+    if world == 1:
+        return float(v)
+    import torch
+    import torch.distributed as dist
+    x = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(x, op=dist.ReduceOp.MAX)
+    return float(x.item())
+
+
+def whole_job_value(ms_total, steps, world):
+    """Seconds per instance over the whole job: every rank solves `steps` instances in ms_total (max over ranks)."""
+    return ms_total / steps * 1e-3 / world
+
+
 def host_threads():
     try:
         from threadpoolctl import threadpool_info
@@ -184,15 +208,27 @@ def measured_peaks():
 
 
 STAGES = [  # (stats ms key, label, kernel, flop key, bytes key, bound)
-    ("ms_theta_apply", "theta_apply", "k_gemm<Tc x skinny> (zipper SVD / variational / env applies)", "flop_theta_apply",
-     "bytes_theta_apply", "tensor"),
-    ("ms_theta_build", "theta_build", "k_gemm<theta_core> + projector maps", "flop_theta_build", None, "tensor"),
-    ("ms_orth_svd", "orth_svd", "Gram GEMM + k_jacobi_rows (orthonormalisation, Rayleigh-Ritz)", None, None, "alu"),
-    ("ms_search_rblocks", "search_rblocks", "k_gemm<H> + k_rs (right blocks)", None, None, "tensor"),
-    ("ms_search_cond", "search_cond", "k_gemm<LG>, k_gemm<V> + k_beam_Z (conditionals)", None, None, "tensor"),
-    ("ms_search_select", "search_select", "k_sel_hist/collect + bitonic (top-M)", None, None, "alu"),
+    ("ms_theta_apply", "theta_apply", "k_tsgemm<NT,8,N|T> (Theta-core x skinny: zipper SVD / variational / env applies)",
+     "flop_theta_apply", "bytes_theta_apply", "tensor"),
+    ("ms_theta_build", "theta_build", "k_bgemm<.., ArTh, LdThE, EpTh> (Theta-core build) + projector maps", "flop_theta_build",
+     None, "tensor"),
+    ("ms_orth_svd", "orth_svd", "k_orth_pass (Cholesky-QR rounds) + k_jacobi_rows (Rayleigh-Ritz)", None, None, "alu"),
+    ("ms_search_rblocks", "search_rblocks", "k_gemm<LdHA,LdHB> + k_rs (right blocks)", None, None, "tensor"),
+    ("ms_search_cond", "search_cond", "k_bgemm<.., ArPV, LdPB, EpPV> + k_beam_Z (conditionals)", None, None, "tensor"),
+    ("ms_search_select", "search_select", "k_sel_hist (sample) + k_sel_prefilter + k_csel_* + bitonic (top-M)", None, None,
+     "hbm"),
     ("ms_tables", "tables", "k_tables", None, None, "hbm"),
 ]
+
+
+def stored_traffic(workload_key):
+    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get(workload_key)
+    except (OSError, ValueError):
+        return None
 
 
 def run_ours(args):
@@ -218,7 +254,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    inst, run = instances.config(args.config, seed=rank)      # one independent replica per rank
+    inst, run = replica_instance(args.config, rank)           # one independent replica per rank
     beta = run["beta"][args.beta_index]
     D, sweeps, M = run["D"], run["sweeps"], run["M"]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -252,6 +288,18 @@ def run_ours(args):
     ms_total, outs = timed(lambda: step(t), args.steps)
     barrier()
     st = t.stats()                                               # stage timers of the last timed step
+    # the dominant kernel timed alone at this workload's largest apply shape (burst figure, warm L2 for small shapes)
+    alone = None
+    if rank == 0:
+        c0 = 1 << inst.n_s
+        nK = c0 * ((1 << (inst.n_s // 2)) if inst.S == 3 else 1)
+        mk, nk, sk = D * nK, c0 * D, min(D + 16, 96)
+        alone = {"shape": "Tc[%d x %d] x [%d x %d]" % (mk, nk, nk, sk)}
+        for op, nm in ((tnb.CHECK_GEMM_N, "N"), (tnb.CHECK_GEMM_T, "T")):
+            ms1 = tnb.tn_kernel_bench(t.handle, op, mk, sk, nk, 5)
+            alone[nm] = {"ms": round(ms1, 4), "tflops": round(2.0 * mk * nk * sk / ms1 * 1e-9, 2),
+                         "frac_fp64_tensor": round(2.0 * mk * nk * sk / ms1 * 1e-9 / fp64_peak, 4),
+                         "gbs": round(8.0 * mk * nk / ms1 * 1e-6, 1)}
     t.close()
 
     # ---- e2e: host buffers in, host buffers out, tn_create / tn_destroy inside the timed region
@@ -268,11 +316,7 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
 
     def maxr(v):
-        if world == 1:
-            return v
-        x = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(x, op=dist.ReduceOp.MAX)
-        return float(x.item())
+        return max_over_ranks(v, world, device="cuda")
 
     ms_total = maxr(ms_total)
     if e2e_ms is not None:
@@ -284,7 +328,7 @@ def run_ours(args):
     states, E, logp, pd = outs
     K = args.steps
     ms_step = ms_total / K
-    value = ms_step * 1e-3 / world                               # seconds per instance over the whole job
+    value = whole_job_value(ms_total, K, world)                  # seconds per instance over the whole job
     h2d = int(inst.edge_u.nbytes + inst.edge_v.nbytes + inst.J.nbytes + inst.h.nbytes + inst.cell_y.nbytes
               + inst.cell_x.nbytes + inst.sub.nbytes + inst.pos.nbytes)
     d2h = int(M * inst.n_spins + 2 * 8 * M + 8 + 4)
@@ -309,12 +353,17 @@ def run_ours(args):
     dom = max((s for s in STAGES if s[3]), key=lambda s: st[s[0]])
     ms_dom = st[dom[0]]
     achieved = st[dom[3]] / ms_dom * 1e-9 if ms_dom > 0 else 0.0
+    tr = stored_traffic("configs[%d]" % args.config)
     roofline = {"bound": "tensor", "achieved": round(achieved, 3), "peak": round(fp64_peak, 2), "unit": "TFLOP/s",
-                "frac": round(achieved / fp64_peak, 4), "traffic": None, "kernel": dom[2], "stage": dom[1],
-                "share_of_step": stages[dom[1]]["share"],
-                "peak_source": "tn_fp64_peak(): mma.sync m8n8k4 f64 chain measured in this run (MEASURED_PEAKS.json "
-                               "has no FP64 entry); HBM peak %s = %.1f GB/s" % (peak_src, peaks["hbm_gbs"]),
-                "algorithmic_flop_per_step": st[dom[3]]}
+                "frac": round(achieved / fp64_peak, 4), "traffic": tr["dram_bytes_per_launch"] if tr else None,
+                "kernel": dom[2], "stage": dom[1], "share_of_step": stages[dom[1]]["share"],
+                "launches_per_step": int(st["theta_apply_calls"]),
+                "peak_source": "tn_fp64_peak(): mma.sync m8n8k4 f64 (SASS DMMA) chain measured in this run "
+                               "(MEASURED_PEAKS.json has no FP64 entry; profiles/r01_fp64_peak.md); HBM peak %s = %.1f GB/s"
+                               % (peak_src, peaks["hbm_gbs"]),
+                "algorithmic_flop_per_step": st[dom[3]], "algorithmic_bytes_per_step": st["bytes_theta_apply"],
+                "achieved_gbs": round(st["bytes_theta_apply"] / ms_dom * 1e-6, 1) if ms_dom > 0 else None,
+                "kernel_alone": alone}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "l2": "flushed (256 MiB fill) between timed steps",
@@ -326,7 +375,7 @@ def run_ours(args):
             "gpu_launches": int(st["kernel_launches"]) * K, "stages": stages, "roofline": roofline, "clocks": clocks,
             "fp64_tensor_peak_tflops": round(fp64_peak, 2)}
     if e2e_ms is not None:
-        line["e2e"] = {"value": e2e_ms / K * 1e-3 / world, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        line["e2e"] = {"value": whole_job_value(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h}
     if world == 1 and not args.no_cpu_baseline:
         tm, est, desc = oracle_sample(inst, run, beta)

@@ -97,6 +97,7 @@ typedef struct {
   int64_t bytes_device;      /* device bytes currently held                                  */
   int64_t jacobi_calls;      /* one-sided Jacobi kernel launches                             */
   int64_t jacobi_sweeps;     /* total Jacobi sweeps over all calls                           */
+  int64_t theta_apply_calls; /* Theta-core x skinny GEMM calls (launches of the dominant kernel)  */
 } tn_stats;
 
 /* tn_create: validates the geometry and copies the instance to the device.

@@ -27,7 +27,7 @@ class TnStats(C.Structure):
         "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
         "bytes_theta_apply", "flop_search", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
-            "jacobi_sweeps")]
+            "jacobi_sweeps", "theta_apply_calls")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

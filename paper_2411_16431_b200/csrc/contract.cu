@@ -91,6 +91,7 @@ void tc_apply_N(Ctx& cx, const ThetaOp& op, const double* X, double* Y, int s) {
   cx.toc();
   cx.h->st.flop_theta_apply += 2.0 * op.mk * op.nk * s;
   cx.h->st.bytes_theta_apply += 8.0 * op.mk * op.nk;
+  cx.h->st.theta_apply_calls++;
 }
 void tc_apply_T(Ctx& cx, const ThetaOp& op, const double* Y, double* Z, int s) {   // Z[nk x s] = Tc^T Y[mk x s]
   cx.tic(&cx.h->st.ms_theta_apply);
@@ -98,6 +99,7 @@ void tc_apply_T(Ctx& cx, const ThetaOp& op, const double* Y, double* Z, int s) {
   cx.toc();
   cx.h->st.flop_theta_apply += 2.0 * op.mk * op.nk * s;
   cx.h->st.bytes_theta_apply += 8.0 * op.mk * op.nk;
+  cx.h->st.theta_apply_calls++;
 }
 
 // Y[m x s] = Theta X[n x s]
@@ -233,17 +235,30 @@ __global__ void k_ls_step(const double* s, const double* ls_in, double* ls_out, 
   *safe = v;
   *ls_out = (ls_in ? *ls_in : 0.0) + log(v);
 }
-// partial column sums of squares of (P - Q), both [m x k]
-__global__ void k_coldiff_part(const double* P, const double* Q, i64 m, int k, int rows_per_block, double* part) {
-  int col = threadIdx.x;
-  if (col >= k) return;
-  i64 r0 = (i64)blockIdx.x * rows_per_block, r1 = min(m, r0 + rows_per_block);
-  double s = 0.0;
-  for (i64 r = r0; r < r1; r++) {
-    double d = P[r * k + col] - Q[r * k + col];
-    s += d * d;
+// partial column sums of squares of (P - Q), both [m x k]: block (32 columns x 8 row lanes), fixed reduction order
+__global__ void __launch_bounds__(256) k_coldiff_part(const double* P, const double* Q, i64 m, int k, int rows_per_block,
+                                                      double* part) {
+  __shared__ double sh[8][33];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const i64 r0 = (i64)blockIdx.x * rows_per_block, r1 = min(m, r0 + rows_per_block);
+  for (int c0 = 0; c0 < k; c0 += 32) {
+    const int col = c0 + tx;
+    double s = 0.0;
+    if (col < k)
+      for (i64 r = r0 + ty; r < r1; r += 8) {
+        double d = P[r * k + col] - Q[r * k + col];
+        s += d * d;
+      }
+    sh[ty][tx] = s;
+    __syncthreads();
+    if (ty == 0 && col < k) {
+      double t = 0.0;
+#pragma unroll
+      for (int y = 0; y < 8; y++) t += sh[y][tx];
+      part[(i64)blockIdx.x * k + col] = t;
+    }
+    __syncthreads();
   }
-  part[(i64)blockIdx.x * k + col] = s;
 }
 __global__ void k_resid_flag(const double* part, int nblk, int k, const int* keep, const double* sig, double tol,
                              int* flag) {
@@ -273,7 +288,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
   cx.tic(&h->st.ms_orth_svd);
   orth_columns(h, Om.p, n, ks, 3);
   cx.toc();
-  const int rpb = 512;
+  const int rpb = (int)std::max<i64>(64, (m + 255) / 256);
   const int nblk = cdiv(m, rpb);
   DBuf<double> part(h, (size_t)nblk * ks);
   bool prev = false;
@@ -282,7 +297,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     if (prev) {
       gemm_rm(h, false, true, (int)m, ks, ks, Yn, ks, Wt.p, ks, TV.p, ks);
       gemm_rm(h, false, true, (int)m, ks, ks, Y, ks, Bo.p, ks, US.p, ks);
-      k_coldiff_part<<<nblk, std::max(32, (ks + 31) / 32 * 32), 0, h->stream>>>(TV.p, US.p, m, ks, rpb, part.p);
+      k_coldiff_part<<<nblk, 256, 0, h->stream>>>(TV.p, US.p, m, ks, rpb, part.p);
       TN_LAUNCH_CHECK(h);
       k_resid_flag<<<1, std::max(32, (ks + 31) / 32 * 32), 0, h->stream>>>(part.p, nblk, ks, cx.d_keep, sig.p,
                                                                         h->svd_tol, cx.d_flag);
