@@ -199,6 +199,19 @@ void frob_norm(tn_handle* h, const double* X, i64 n, double* out) {
 // one-sided Jacobi on rows (single CTA; working set in shared memory when it fits)
 // ============================================================================================
 // Working storage: Mw [c x r] (ldm), Ww [c x c].  Round-robin pair ordering; each warp owns a pair.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  y = y * (2.0 - x * y);
+  return y * (2.0 - x * y);
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double hx = 0.5 * x;
+  y = y * (1.5 - hx * y * y);
+  return y * (1.5 - hx * y * y);
+}
 __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld, int c, int r, double* Mout,
                                                       double* Wt, double* sig, double* gwork, int use_smem,
                                                       unsigned long long* cnt) {
@@ -226,7 +239,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
   __syncthreads();
   double fro2 = 0.0;
   for (int p = 0; p < c; p++) fro2 += s_norm[p];
-  const double negl = 1e-33 * fro2;
+  const double sinv = fro2 > 0.0 ? 1.0 / fro2 : 0.0;
   __syncthreads();
   if (c > 1) {
     for (int sweep = 0; sweep < 60; sweep++) {
@@ -252,10 +265,14 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
             b += __shfl_xor_sync(0xffffffffu, b, o);
             g += __shfl_xor_sync(0xffffffffu, g, o);
           }
-          if (fmin(a, b) > negl && fabs(g) > tol * sqrt(a) * sqrt(b)) {
-            double zeta = (b - a) / (2.0 * g);
-            double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-            double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
+          // scaled by 1 / ||M||_F^2: a, b in (1e-33, 1], so neither the test nor q below can under- or overflow
+          a *= sinv; b *= sinv; g *= sinv;
+          if (fmin(a, b) > 1e-33 && g * g > tol * tol * a * b) {
+            // tan of the rotation angle, t = 2 g sign(d) / (|d| + sqrt(d^2 + 4 g^2)), d = b - a, from approximate
+            // reciprocal / reciprocal square root + two Newton steps each (full precision, no IEEE division)
+            const double d = b - a, q2 = d * d + 4.0 * g * g;
+            const double t = 2.0 * (d >= 0.0 ? g : -g) * rcp_fast(fabs(d) + q2 * rsqrt_fast(q2));
+            const double cs = rsqrt_fast(1.0 + t * t), sn = cs * t;
             for (int i = lane; i < r; i += 32) {
               double u = xp[i], v = xq[i];
               xp[i] = cs * u - sn * v;
