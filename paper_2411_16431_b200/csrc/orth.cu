@@ -239,36 +239,6 @@ void orth_columns_jacobi(tn_handle* h, double* Y, i64 m, int k, int passes);   /
 
 void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes) {
   if (m <= 0 || k <= 0) return;
-  if (getenv("ORTH_OLD")) { orth_columns_jacobi(h, Y, m, k, passes); return; }
-  std::vector<double> dbg_in;
-  if (getenv("ORTH_DEBUG")) {
-    dbg_in.resize((size_t)m * k);
-    cudaMemcpyAsync(dbg_in.data(), Y, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream);
-    cudaStreamSynchronize(h->stream);
-  }
-  struct Dbg {
-    tn_handle* h; double* Y; i64 m; int k; std::vector<double>& in;
-    ~Dbg() {
-      if (in.empty()) return;
-      std::vector<double> out((size_t)m * k);
-      cudaMemcpyAsync(out.data(), Y, sizeof(double) * m * k, cudaMemcpyDeviceToHost, h->stream);
-      cudaStreamSynchronize(h->stream);
-      bool bi = false, bo = false;
-      for (double v : in) if (!std::isfinite(v)) bi = true;
-      for (double v : out) if (!std::isfinite(v)) bo = true;
-      static int ncall = 0;
-      ncall++;
-      if (bo || bi) {
-        fprintf(stderr, "ORTH_DEBUG call %d m=%lld k=%d bad_in=%d bad_out=%d\n", ncall, (long long)m, k, (int)bi, (int)bo);
-        if (bo && !bi) {
-          FILE* f = fopen("gpurun_out/orth_bad.bin", "wb");
-          long long hdr[2] = {m, k};
-          fwrite(hdr, 8, 2, f); fwrite(in.data(), 8, in.size(), f); fwrite(out.data(), 8, out.size(), f); fclose(f);
-          exit(3);
-        }
-      }
-    }
-  } dbg{h, Y, m, k, dbg_in};
   if (k <= 16) run_orth<2>(h, Y, m, k, passes);
   else if (k <= 32) run_orth<4>(h, Y, m, k, passes);
   else if (k <= 48) run_orth<6>(h, Y, m, k, passes);
