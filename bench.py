@@ -107,6 +107,40 @@ def whole_job_value(ms_total, steps, world):
     return ms_total / steps * 1e-3 / world
 
 
+def diversity_report(inst, states, E, frac=0.01, R=0.25, restarts=100, seed=0):
+    """Config-5 harness metrics: gap to the planted E0, states within `frac` of E0 by both
+    (E - E0)/|E0| and Eq. (14) d_E = (E - E0)/(2|E0|), and the size of the largest set of those states
+    that are pairwise >= R*N Hamming apart (Eq. (15)), found by a randomised greedy clique heuristic
+    (footnote [58] PAPER.md:418) after flipping every state to s_0 = +1 (h = 0)."""
+    import numpy as np
+    E0 = float(inst.E0)
+    rel = (E - E0) / abs(E0)
+    near = np.flatnonzero(rel <= frac)
+    out = {"E0": E0, "gap_to_E0": float(E.min() - E0), "n_within_1pct": int(near.size),
+           "n_within_dE_1pct": int(np.count_nonzero(rel / 2.0 <= frac))}
+    s = states[near].astype(np.int8)
+    s = s * s[:, :1]                                           # Z2 gauge: s_0 = +1
+    s = np.unique(s, axis=0)
+    n, N = s.shape[0], inst.n_spins
+    if n == 0:
+        out["diversity"] = 0
+        return out
+    ham = (N - s.astype(np.int32) @ s.astype(np.int32).T) // 2
+    ok = ham >= R * N
+    rng = np.random.default_rng(seed)
+    best = 1
+    for _ in range(restarts):
+        order = rng.permutation(n)
+        chosen = []
+        for i in order:
+            if all(ok[i, j] for j in chosen):
+                chosen.append(i)
+        best = max(best, len(chosen))
+    out["diversity"] = int(best)
+    out["distinct_up_to_Z2"] = int(n)
+    return out
+
+
 def host_threads():
     try:
         from threadpoolctl import threadpool_info
@@ -374,6 +408,8 @@ def run_ours(args):
             "best_energy": float(E.min()), "n_states": int(len(E)), "log_p_discarded": float(pd),
             "gpu_launches": int(st["kernel_launches"]) * K, "stages": stages, "roofline": roofline, "clocks": clocks,
             "fp64_tensor_peak_tflops": round(fp64_peak, 2)}
+    if "E0" in inst:
+        line["planted"] = diversity_report(inst, states, E)
     if e2e_ms is not None:
         line["e2e"] = {"value": whole_job_value(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h}
