@@ -82,7 +82,7 @@ struct tn_handle {
   bool have_logz = false;
   int D = 0, sweeps = 0;
   // options
-  int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1;
+  int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
   double svd_tol = 1e-11;
   i64 select_direct_max = 1ll << 22;
   // runtime
