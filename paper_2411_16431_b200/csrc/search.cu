@@ -97,6 +97,22 @@ struct LdHB {   // B(kk=(b,cl), j=(m,t)) = X[t][b] vS[vrow m][b] Yc[b][cl] fc[m]
     return X[t * nB + b] * vS[(i64)vrow[m] * nB + b] * Yc[b * nCl + cl] * fc[(i64)m * nCl + cl];
   }
 };
+// materialised operands of the right-block GEMM
+__global__ void k_gather_G(const double* G, const int* Pd, const int* Po, int nCl, int n_o, i64 DD, int Kg, double* out) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)Kg * DD) return;
+  const int kk = (int)(t / DD);
+  const i64 i = t % DD;
+  out[t] = G[(i64)(Pd[kk / nCl] * n_o + Po[kk % nCl]) * DD + i];
+}
+__global__ void k_coef(const double* X, const double* vS, const double* Yc, const double* fc, const int* vrow, int nB, int nCl,
+                       int nT, int Kg, int Ng, double* out) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)Kg * Ng) return;
+  const int kk = (int)(t / Ng), j = (int)(t % Ng);
+  const int b = kk / nCl, cl = kk % nCl, m = j / nT, tt = j % nT;
+  out[t] = X[tt * nB + b] * vS[(i64)vrow[m] * nB + b] * Yc[b * nCl + cl] * fc[(i64)m * nCl + cl];
+}
 struct StH { double* H; i64 DD; __device__ __forceinline__ void operator()(int, int, int i, int j, double v) const { H[(i64)j * DD + i] = v; } };
 
 // ---- small kernels -------------------------------------------------------------------------------
@@ -636,15 +652,28 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       DBuf<double> fcx(h, (size_t)nb * c.nCl), H(h, (size_t)nb * c.nT * DD), RS(h, (size_t)nb * Dl * c.nA);
       k_fc<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(c, drow.p + (size_t)x * nb, nullptr, nb, fcx.p);
       TN_LAUNCH_CHECK(h);
-      {
-        LdHA a{rt[x].G, c.Pd, c.Po, c.nCl, c.n_o, DD};
-        LdHB b{c.X, c.BvS, c.Yc, fcx.p, vrow.p + (size_t)x * nb, c.nB, c.nCl, c.nT};
-        StH e{H.p, DD};
-        int Mg = (int)DD, Ng = nb * c.nT, Kg = c.nB * c.nCl;
-        dim3 grid(1, cdiv(Mg, 64), cdiv(Ng, 64));
-        k_gemm<64, 64, 16, 2, 2, false, true, LdHA, LdHB, StH><<<grid, 128, 0, h->stream>>>(Mg, Ng, Kg, 1, a, b, e);
-        TN_LAUNCH_CHECK(h);
+      {   // H[(m,t)][(b',b'')] = sum_{(b,cl)} coef[(b,cl)][(m,t)] G[(Pd b, Po cl)][(b',b'')]
+        const int Mg = (int)DD, Ng = nb * c.nT, Kg = c.nB * c.nCl;
         h->st.flop_search += 2.0 * Mg * (double)Ng * Kg;
+        bool done = false;
+        if ((DD & 1) == 0 && (Ng & 1) == 0) {
+          // both operands materialised row-major in the reduction index, then the streaming GEMM (tsgemm.cu)
+          DBuf<double> Gg(h, (size_t)Kg * DD), cf(h, (size_t)Kg * Ng);
+          k_gather_G<<<cdiv((i64)Kg * DD, 256), 256, 0, h->stream>>>(rt[x].G, c.Pd, c.Po, c.nCl, c.n_o, DD, Kg, Gg.p);
+          TN_LAUNCH_CHECK(h);
+          k_coef<<<cdiv((i64)Kg * Ng, 256), 256, 0, h->stream>>>(c.X, c.BvS, c.Yc, fcx.p, vrow.p + (size_t)x * nb, c.nB, c.nCl,
+                                                               c.nT, Kg, Ng, cf.p);
+          TN_LAUNCH_CHECK(h);
+          done = tsgemm(h, true, Kg, Mg, Ng, cf.p, Ng, Gg.p, DD, H.p, DD);
+        }
+        if (!done) {
+          LdHA a{rt[x].G, c.Pd, c.Po, c.nCl, c.n_o, DD};
+          LdHB b{c.X, c.BvS, c.Yc, fcx.p, vrow.p + (size_t)x * nb, c.nB, c.nCl, c.nT};
+          StH e{H.p, DD};
+          dim3 grid(1, cdiv(Mg, 64), cdiv(Ng, 64));
+          k_gemm<64, 64, 16, 2, 2, false, true, LdHA, LdHB, StH><<<grid, 128, 0, h->stream>>>(Mg, Ng, Kg, 1, a, b, e);
+          TN_LAUNCH_CHECK(h);
+        }
       }
       {
         i64 total = (i64)nb * Dl * c.nA;

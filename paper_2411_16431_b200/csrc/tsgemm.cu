@@ -152,12 +152,11 @@ __global__ void k_ts_reduce(const double* __restrict__ ws, int nsplit, i64 M, in
   C[(i64)bz * sCz + (t / N) * ldc + t % N] = s;
 }
 
-struct TsBatch { int n = 1; i64 sB = 0, sC = 0; };
-TsBatch g_tsb;   // set by tsgemm_batched around the dispatch (host-side, single-threaded per handle)
+struct TsBatch { int n = 1; i64 sB = 0, sC = 0; };   // independent products sharing A: B_z = B + z sB, C_z = C + z sC
 
 template <int NT, int WARPS, bool TRANS>
 void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
-               i64 Kred, int nsplit) {
+               i64 Kred, int nsplit, const TsBatch& tsb) {
   constexpr int BM = 16 * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK), LDB = smem_ld(NP);
   constexpr size_t smem = sizeof(double) * TS_STAGES * ((TRANS ? TS_BK * LDA : BM * LDA) + TS_BK * LDB);
@@ -168,14 +167,14 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
   }
   i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
   nsplit = (int)((Kred + kper - 1) / kper);
-  const int nbz = g_tsb.n, nz = (N + NP - 1) / NP;
+  const int nbz = tsb.n, nz = (N + NP - 1) / NP;
   double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nbz * nsplit * Mout * N) : nullptr;
   dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit, (unsigned)(nz * nbz));
   k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws, nz,
-                                                                     g_tsb.sB, g_tsb.sC);
+                                                                     tsb.sB, tsb.sC);
   TN_LAUNCH_CHECK(h);
   if (nsplit > 1) {
-    k_ts_reduce<<<dim3(cdiv(Mout * N, 256), nbz), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc, g_tsb.sC);
+    k_ts_reduce<<<dim3(cdiv(Mout * N, 256), nbz), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc, tsb.sC);
     TN_LAUNCH_CHECK(h);
     h->dfree(ws);
   }
@@ -186,9 +185,9 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
 // output has fewer row blocks than 2 x 148 CTA slots.
 template <int NT, bool TRANS>
 void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
-                i64 Kred) {
+                i64 Kred, const TsBatch& tsb) {
   int warps = Mout > 64 ? 8 : Mout > 32 ? 4 : 2;
-  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps) * ((N + 8 * NT - 1) / (8 * NT)) * g_tsb.n;
+  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps) * ((N + 8 * NT - 1) / (8 * NT)) * tsb.n;
   const int slots = 148 * ((NT <= 10 || warps < 8) ? 2 : 1);
   const double t_k = 2.0 * 16 * warps * (8 * NT) * slots / 37e12;      // seconds per reduction index per CTA
   const double t_ws = (double)Mout * N * 16.0 / 6e12 + 2e-7;           // seconds per extra split (write + read)
@@ -200,49 +199,47 @@ void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb
     const double t = waves * ((double)((Kred + sp - 1) / sp) + 96.0) * t_k + (sp > 1 ? sp * t_ws + 3e-6 : 0.0);
     if (t < best_t) { best_t = t; best = sp; }
   }
-  if (warps == 8) launch_ts<NT, 8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
-  else if (warps == 4) launch_ts<NT, 4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
-  else launch_ts<NT, 2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best);
+  if (warps == 8) launch_ts<NT, 8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);
+  else if (warps == 4) launch_ts<NT, 4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);
+  else launch_ts<NT, 2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);
 }
 
 template <bool TRANS>
 void pick_nt(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
-             i64 Kred) {
-  if (N > 96) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);          // chunks of 64 columns
-  else if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
-  else if (N <= 32) pick_warps<4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
-  else if (N <= 48) pick_warps<6, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
-  else if (N <= 64) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
-  else if (N <= 80) pick_warps<10, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
-  else pick_warps<12, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred);
+             i64 Kred, const TsBatch& tsb) {
+  if (N > 96) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);          // chunks of 64 columns
+  else if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  else if (N <= 32) pick_warps<4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  else if (N <= 48) pick_warps<6, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  else if (N <= 64) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  else if (N <= 80) pick_warps<10, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  else pick_warps<12, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
 }
 
 bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 
 }  // namespace
 
+static bool tsgemm_impl(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb,
+                        double* C, i64 ldc, const TsBatch& tsb) {
+  if (N < 1 || M < 1 || K < 1) return false;
+  if ((lda & 1) || (ldb & 1) || !aligned16(A) || !aligned16(B)) return false;
+  if (trans) pick_nt<true>(h, A, lda, B, ldb, C, ldc, K, N, M, tsb);    // output rows = K (columns of A), reduce over M
+  else pick_nt<false>(h, A, lda, B, ldb, C, ldc, M, N, K, tsb);
+  return true;
+}
+
 // Returns false when the shapes / alignment do not fit (the caller falls back to the generic k_gemm).
 bool tsgemm(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb, double* C,
             i64 ldc) {
-  if (N < 1 || M < 1 || K < 1) return false;
-  if ((lda & 1) || (ldb & 1) || !aligned16(A) || !aligned16(B)) return false;
-  if (trans) pick_nt<true>(h, A, lda, B, ldb, C, ldc, K, N, M);    // output rows = K (columns of A), reduce over M
-  else pick_nt<false>(h, A, lda, B, ldb, C, ldc, M, N, K);
-  return true;
+  return tsgemm_impl(h, trans, M, N, K, A, lda, B, ldb, C, ldc, TsBatch());
 }
 
 // nbatch independent products with a shared A: B_z = B + z sB, C_z = C + z sC.
 bool tsgemm_batched(tn_handle* h, bool trans, i64 M, int N, i64 K, const double* A, i64 lda, const double* B, i64 ldb,
                     i64 sB, double* C, i64 ldc, i64 sC, int nbatch) {
   if (nbatch < 1 || nbatch > 16384 || (sB & 1)) return false;
-  g_tsb.n = nbatch; g_tsb.sB = sB; g_tsb.sC = sC;
-  bool ok = false;
-  try {
-    ok = tsgemm(h, trans, M, N, K, A, lda, B, ldb, C, ldc);
-  } catch (...) {
-    g_tsb = TsBatch();
-    throw;
-  }
-  g_tsb = TsBatch();
-  return ok;
+  TsBatch tsb;
+  tsb.n = nbatch; tsb.sB = sB; tsb.sC = sC;
+  return tsgemm_impl(h, trans, M, N, K, A, lda, B, ldb, C, ldc, tsb);
 }
