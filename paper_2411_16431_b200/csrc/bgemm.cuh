@@ -79,6 +79,119 @@ __global__ void __launch_bounds__(256, 2) k_bgemm(int batches, int bg, int M, in
   }
 }
 
+// Pipelined variant for a batch-independent A and a B whose rows are contiguous in memory (Theta-core build):
+// the B tile of batch i+1 is fetched with 16-byte cp.async into the second shared buffer while batch i is
+// multiplied and stored, so the only exposed latencies are the first fetch and the barriers.
+//   BR: const double* operator()(int batch, int k) -> pointer to the N contiguous doubles of row k of B (16-byte aligned)
+template <int KP, int NT, class AR, class BR, class EP>
+__global__ void __launch_bounds__(256) k_bgemm_pipe(int batches, int bg, int M, int N, int K, AR ar, BR br, EP ep) {
+  constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
+  extern __shared__ __align__(16) double bg_smem[];
+  double* sA = bg_smem;
+  double* sB = bg_smem + BM * LDA;            // two buffers of KP * LDB
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int m0 = blockIdx.y * BM;
+  const int b0 = blockIdx.x * bg, b1 = min(batches, b0 + bg);
+  auto fetch = [&](int batch, int buf) {
+    double* dst = sB + buf * (KP * LDB);
+    constexpr int G = BN / 2;
+    for (int idx = tid; idx < KP * G; idx += 256) {
+      const int k = idx / G, g2 = 2 * (idx % G);
+      const int rem = k < K ? N - g2 : 0;
+      const int bytes = rem >= 2 ? 16 : rem == 1 ? 8 : 0;
+      const double* src = bytes ? br(batch, k) + g2 : br(batch, 0);
+      unsigned sa = (unsigned)__cvta_generic_to_shared(dst + k * LDB + g2);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(src), "r"(bytes));
+    }
+    asm volatile("cp.async.commit_group;");
+  };
+  fetch(b0, 0);
+  for (int r = warp; r < BM; r += 8) {
+    const int gi = m0 + r;
+    const double* src = gi < M ? ar(b0, gi) : nullptr;
+#pragma unroll
+    for (int k = lane; k < KP; k += 32) sA[r * LDA + k] = (src && k < K) ? __ldg(src + k) : 0.0;
+  }
+  for (int batch = b0; batch < b1; batch++) {
+    const int buf = (batch - b0) & 1;
+    if (batch + 1 < b1) {
+      fetch(batch + 1, buf ^ 1);
+      asm volatile("cp.async.wait_group 1;");
+    } else {
+      asm volatile("cp.async.wait_group 0;");
+    }
+    __syncthreads();
+    const double* sb = sB + buf * (KP * LDB);
+    double acc[2][NT][2];
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+      for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+    for (int kk = 0; kk < KP; kk += 4) {
+      const double fa0 = sA[(16 * warp + (lane >> 2)) * LDA + kk + (lane & 3)];
+      const double fa1 = sA[(16 * warp + 8 + (lane >> 2)) * LDA + kk + (lane & 3)];
+      const double* brow = sb + (kk + (lane & 3)) * LDB + (lane >> 2);
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const double fb = brow[8 * j];
+        dmma884(acc[0][j][0], acc[0][j][1], fa0, fb);
+        dmma884(acc[1][j][0], acc[1][j][1], fa1, fb);
+      }
+    }
+    __syncthreads();      // everyone is done with sb before the fetch of batch + 2 overwrites it
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+      const int row = m0 + 16 * warp + 8 * i + (lane >> 2);
+      if (row < M) {
+        const typename EP::Row rc = ep.row(batch, row);
+#pragma unroll
+        for (int j = 0; j < NT; j++) {
+          const int col = 8 * j + 2 * (lane & 3);
+          if (col + 1 < N) ep.put2(rc, batch, col, acc[i][j][0], acc[i][j][1]);
+          else if (col < N) ep.put(rc, batch, col, acc[i][j][0]);
+        }
+      }
+    }
+  }
+}
+
+template <int KP, int NT, class AR, class BR, class EP>
+void launch_bgemm_pipe_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BR& br, const EP& ep) {
+  constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
+  constexpr int smem = (int)sizeof(double) * (BM * LDA + 2 * KP * LDB);
+  static bool attr = false;
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_bgemm_pipe<KP, NT, AR, BR, EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    attr = true;
+  }
+  const int mt = (M + BM - 1) / BM;
+  const int bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (4 * 296)));
+  dim3 grid((unsigned)((batches + bg - 1) / bg), (unsigned)mt);
+  k_bgemm_pipe<KP, NT, AR, BR, EP><<<grid, 256, smem, h->stream>>>(batches, bg, M, N, K, ar, br, ep);
+  h->st.kernel_launches++;
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) tn_throw(TN_ERR_CUDA, "k_bgemm_pipe launch failed: %s", cudaGetErrorString(e));
+}
+
+// K <= 64, N <= 64 and even (16-byte rows); returns false otherwise.
+template <class AR, class BR, class EP>
+bool launch_bgemm_pipe(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BR& br, const EP& ep) {
+  if (K < 1 || K > 64 || N < 2 || N > 64 || (N & 1) || batches < 1 || M < 1 || (M + 127) / 128 > 65535) return false;
+#define TN_PIPE_N(KP_)                                                                   \
+  do {                                                                                   \
+    if (N <= 16) launch_bgemm_pipe_knt<KP_, 2>(h, batches, M, N, K, ar, br, ep);         \
+    else if (N <= 32) launch_bgemm_pipe_knt<KP_, 4>(h, batches, M, N, K, ar, br, ep);    \
+    else launch_bgemm_pipe_knt<KP_, 8>(h, batches, M, N, K, ar, br, ep);                 \
+  } while (0)
+  if (K <= 16) TN_PIPE_N(16);
+  else if (K <= 32) TN_PIPE_N(32);
+  else if (K <= 48) TN_PIPE_N(48);
+  else TN_PIPE_N(64);
+#undef TN_PIPE_N
+  return true;
+}
+
 template <int KP, int NT, bool A_SHARED, class AR, class BE, class EP>
 void launch_bgemm_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BE& be, const EP& ep) {
   constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);

@@ -543,6 +543,11 @@ struct ArTh {
     return A + ((i64)(i / nB) * pd + Pd[i % nB]) * dy;
   }
 };
+struct BrTh {   // row y of B for batch k: Ek[(y, k)][0..g)
+  const double* Ek;
+  int nK, g;
+  __device__ __forceinline__ const double* operator()(int k, int y) const { return Ek + ((i64)y * nK + k) * g; }
+};
 struct EpTh {
   double* Tc;
   const double *wA, *X, *Yc;
@@ -565,6 +570,8 @@ void theta_core(tn_handle* h, const CellDev& c, const double* A, int dx, int dy,
     ArTh ar{A, c.Pd, c.nB, c.n_d, dy};
     LdThE be{Ek, c.nK, g};
     EpTh ep{Tc, c.wA, c.X, c.Yc, c.nK, c.nB, c.nCl, c.tshift, g};
+    BrTh br{Ek, c.nK, g};
+    if ((((uintptr_t)Ek) & 15) == 0 && launch_bgemm_pipe(h, c.nK, dx * c.nB, g, dy, ar, br, ep)) return;
     if (launch_bgemm<true>(h, c.nK, dx * c.nB, g, dy, ar, be, ep)) return;
   }
   if (g <= 16) launch_theta<16>(h, c, A, dx, dy, Ek, g, Tc);
