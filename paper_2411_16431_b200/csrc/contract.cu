@@ -358,6 +358,7 @@ void svd_trunc_locked(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, d
   std::vector<double> res(128, 0.0);
   int L = 0, sa = ks;
   bool have_rr = false;
+  const bool skip_first_rr = ks < std::min(m, n);
   for (int it = 0;; it++) {
     apply_N(cx, op, Om.p, Yn, sa);
     if (have_rr) {
@@ -399,13 +400,17 @@ void svd_trunc_locked(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, d
     TN_CUDA(cudaMemcpyAsync(Om.p, Z.p, sizeof(double) * n * sa, cudaMemcpyDeviceToDevice, h->stream));
     cx.tic(&h->st.ms_orth_svd);
     orth_columns(h, Om.p, n, sa, 5);
+    h->st.svd_iterations++;
+    if (it == 0 && skip_first_rr) {   // a random start block is never converged after one step: no Rayleigh-Ritz, no test
+      cx.toc();
+      continue;
+    }
     gemm_rm(h, true, false, sa, sa, (int)n, Om.p, sa, Z.p, sa, B.p, sa);
     jacobi_rows(h, B.p, sa, sa, sa, Bo.p, Wt.p, sigfull.p + L);
     k_rank_decide<<<1, 32, 0, h->stream>>>(sigfull.p, L + sa, chi, h->gap_guard, cx.d_keep, cx.d_stat);
     TN_LAUNCH_CHECK(h);
     cx.toc();
     have_rr = true;
-    h->st.svd_iterations++;
   }
   k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
   TN_LAUNCH_CHECK(h);
@@ -508,13 +513,17 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     TN_CUDA(cudaMemcpyAsync(Om.p, Z.p, sizeof(double) * n * ks, cudaMemcpyDeviceToDevice, h->stream));
     cx.tic(&h->st.ms_orth_svd);
     orth_columns(h, Om.p, n, ks, 5);
+    h->st.svd_iterations++;
+    if (it == 0 && ks < std::min(m, n)) {   // random start block: skip the first Rayleigh-Ritz step and its test
+      cx.toc();
+      continue;
+    }
     gemm_rm(h, true, false, ks, ks, (int)n, Om.p, ks, Z.p, ks, B.p, ks);
     jacobi_rows(h, B.p, ks, ks, ks, Bo.p, Wt.p, sig.p);
     k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, ks, chi, h->gap_guard, cx.d_keep, cx.d_stat);
     TN_LAUNCH_CHECK(h);
     cx.toc();
     prev = true;
-    h->st.svd_iterations++;
   }
   k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
   TN_LAUNCH_CHECK(h);
