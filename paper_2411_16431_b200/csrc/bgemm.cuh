@@ -12,7 +12,9 @@
 //
 //   AR: const double* operator()(int batch, int i)      -> pointer to the K contiguous doubles of row i
 //   BE: double operator()(int batch, int k, int j)      -> element of B
-//   EP: Row row(int batch, int i);  put(const Row&, batch, j, v);  put2(const Row&, batch, j, v0, v1) (columns j, j+1)
+//   EP: Row row(int batch, int i);  put(Row&, batch, j, v);  put2(Row&, batch, j, v0, v1) (columns j, j+1);
+//       static constexpr bool kReduce: if set, collect(Row&, double&, unsigned&) after each row and
+//       tile_done(batch, row_tile, sum, count) once per (batch, row tile) with the CTA-reduced values (fixed order)
 #pragma once
 #include "gemm.cuh"
 
@@ -28,7 +30,11 @@ __global__ void __launch_bounds__(256, 2) k_bgemm(int batches, int bg, int M, in
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int m0 = blockIdx.y * BM;
   const int b0 = blockIdx.x * bg, b1 = min(batches, b0 + bg);
+  __shared__ double s_rz[8];
+  __shared__ unsigned s_rn[8];
   for (int batch = b0; batch < b1; batch++) {
+    double tz = 0.0;     // EP::kReduce: per-thread sum / count collected by the epilogue rows of this batch
+    unsigned tn = 0;
     if (!A_SHARED || batch == b0) {
       __syncthreads();
       for (int r = warp; r < BM; r += 8) {
@@ -66,14 +72,31 @@ __global__ void __launch_bounds__(256, 2) k_bgemm(int batches, int bg, int M, in
       for (int i = 0; i < 2; i++) {
         const int row = m0 + 16 * warp + 8 * i + (lane >> 2);
         if (row < M) {
-          const typename EP::Row rc = ep.row(batch, row);
+          typename EP::Row rc = ep.row(batch, row);
 #pragma unroll
           for (int j = 0; j < NT; j++) {
             const int col = n0 + 8 * j + 2 * (lane & 3);
             if (col + 1 < N) ep.put2(rc, batch, col, acc[i][j][0], acc[i][j][1]);
             else if (col < N) ep.put(rc, batch, col, acc[i][j][0]);
           }
+          if constexpr (EP::kReduce) ep.collect(rc, tz, tn);
         }
+      }
+    }
+    if constexpr (EP::kReduce) {   // ordered CTA reduction of the epilogue sums -> one partial per (batch, row tile)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        tz += __shfl_xor_sync(0xffffffffu, tz, o);
+        tn += __shfl_xor_sync(0xffffffffu, tn, o);
+      }
+      __syncthreads();
+      if (lane == 0) { s_rz[warp] = tz; s_rn[warp] = tn; }
+      __syncthreads();
+      if (tid == 0) {
+        double z = 0.0;
+        unsigned nn = 0;
+        for (int w = 0; w < 8; w++) { z += s_rz[w]; nn += s_rn[w]; }
+        ep.tile_done(batch, blockIdx.y, z, nn);
       }
     }
   }
@@ -144,7 +167,7 @@ __global__ void __launch_bounds__(256) k_bgemm_pipe(int batches, int bg, int M, 
     for (int i = 0; i < 2; i++) {
       const int row = m0 + 16 * warp + 8 * i + (lane >> 2);
       if (row < M) {
-        const typename EP::Row rc = ep.row(batch, row);
+        typename EP::Row rc = ep.row(batch, row);
 #pragma unroll
         for (int j = 0; j < NT; j++) {
           const int col = 8 * j + 2 * (lane & 3);

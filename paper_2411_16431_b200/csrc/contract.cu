@@ -358,7 +358,11 @@ void svd_trunc_locked(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, d
   std::vector<double> res(128, 0.0);
   int L = 0, sa = ks;
   bool have_rr = false;
-  const bool skip_first_rr = ks < std::min(m, n);
+  // skip the first Rayleigh-Ritz step / test when the previous SVD of this contraction did not converge at its
+  // first test (a random start block needs >= 2 power steps unless Theta is rank-deficient below ks, config 5)
+  const bool skip_first_rr = h->svd_skip_first && ks < std::min(m, n);
+  int n_rr = 0;
+  double last_res = 1.0;
   for (int it = 0;; it++) {
     apply_N(cx, op, Om.p, Yn, sa);
     if (have_rr) {
@@ -373,6 +377,7 @@ void svd_trunc_locked(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, d
       TN_CUDA(cudaMemcpyAsync(&info, dinfo.p, sizeof(info), cudaMemcpyDeviceToHost, h->stream));
       TN_CUDA(cudaMemcpyAsync(res.data(), dres.p, sizeof(double) * sa, cudaMemcpyDeviceToHost, h->stream));
       TN_CUDA(cudaStreamSynchronize(h->stream));
+      last_res = info.res;
       if (info.flag) break;
       if (it >= h->svd_maxit) { h->st.svd_unconverged++; break; }
       int c = 0;
@@ -411,7 +416,10 @@ void svd_trunc_locked(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, d
     TN_LAUNCH_CHECK(h);
     cx.toc();
     have_rr = true;
+    n_rr++;
   }
+  if (!skip_first_rr) h->svd_skip_first = n_rr >= 2;
+  else if (n_rr == 1 && last_res < 1e-3) h->svd_skip_first = 0;
   k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
   TN_LAUNCH_CHECK(h);
   gemm_rm(h, false, true, (int)n, sa, sa, Om.p, sa, Wt.p, sa, Vrot.p, sa);          // V_a = Om W
@@ -447,6 +455,9 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
   DBuf<double> part(h, (size_t)nblk * ks);
   DBuf<SvdInfo> dinfo(h, 1);
   bool prev = false;
+  const bool skip_first_rr = h->svd_skip_first && ks < std::min(m, n);
+  int n_rr = 0;
+  double last_res = 1.0;
   for (int it = 0;; it++) {
     apply_N(cx, op, Om.p, Yn, ks);
     if (prev) {
@@ -460,6 +471,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
       SvdInfo info;
       TN_CUDA(cudaMemcpyAsync(&info, dinfo.p, sizeof(info), cudaMemcpyDeviceToHost, h->stream));
       TN_CUDA(cudaStreamSynchronize(h->stream));
+      last_res = info.res;
       if (info.flag) break;
       if (it >= h->svd_maxit) { h->st.svd_unconverged++; break; }
       // ---- Chebyshev-filtered step: when the worst residual is still far from the tolerance
@@ -514,7 +526,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     cx.tic(&h->st.ms_orth_svd);
     orth_columns(h, Om.p, n, ks, 5);
     h->st.svd_iterations++;
-    if (it == 0 && ks < std::min(m, n)) {   // random start block: skip the first Rayleigh-Ritz step and its test
+    if (it == 0 && skip_first_rr) {   // random start block: skip the first Rayleigh-Ritz step and its test
       cx.toc();
       continue;
     }
@@ -524,7 +536,10 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     TN_LAUNCH_CHECK(h);
     cx.toc();
     prev = true;
+    n_rr++;
   }
+  if (!skip_first_rr) h->svd_skip_first = n_rr >= 2;
+  else if (n_rr == 1 && last_res < 1e-3) h->svd_skip_first = 0;
   k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
   TN_LAUNCH_CHECK(h);
   gemm_rm(h, false, true, (int)n, ks, ks, Om.p, ks, Wt.p, ks, Z.p, ks);        // V = Omega W
@@ -706,6 +721,7 @@ void mps_free(tn_handle* h) {
 
 void contract_run(tn_handle* h, int D, int sweeps) {
   mps_free(h);
+  h->svd_skip_first = 0;
   Ctx cx;
   cx.h = h;
   DBuf<int> ints(h, 4);

@@ -552,13 +552,14 @@ struct EpTh {
   double* Tc;
   const double *wA, *X, *Yc;
   int nK, nB, nCl, tshift, g;
+  static constexpr bool kReduce = false;
   struct Row { double* p; double w; };
   __device__ __forceinline__ Row row(int k, int i) const {
     const int x = i / nB, b = i % nB, a = k / nCl, cl = k % nCl;
     return Row{Tc + (((i64)x * nK + k) * nB + b) * g, wA[a] * X[(a >> tshift) * nB + b] * Yc[b * nCl + cl]};
   }
-  __device__ __forceinline__ void put(const Row& r, int, int j, double v) const { r.p[j] = v * r.w; }
-  __device__ __forceinline__ void put2(const Row& r, int, int j, double v0, double v1) const {
+  __device__ __forceinline__ void put(Row& r, int, int j, double v) const { r.p[j] = v * r.w; }
+  __device__ __forceinline__ void put2(Row& r, int, int j, double v0, double v1) const {
     if (((g | j) & 1) == 0) *reinterpret_cast<double2*>(r.p + j) = make_double2(v0 * r.w, v1 * r.w);   // 16-byte store
     else { r.p[j] = v0 * r.w; r.p[j + 1] = v1 * r.w; }
   }

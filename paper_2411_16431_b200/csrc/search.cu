@@ -59,21 +59,37 @@ struct ArPV {
     return LG + ((i64)m * npp + Pd[i / nCl] * n_o + Po[i % nCl]) * Dr;
   }
 };
-struct EpPV {
-  double* V; const double *cs, *X, *vS, *Yc; const int *vrow, *slot;
-  int nA, nB, nCl, tshift; i64 per_m;
-  struct Row { double* p; const double* x; const double* c; double w; };
+struct EpPV {   // stores V and, fused, collects Z_m = sum max(v, 0) fc[m][cl] and the count of negative entries
+  double* V; const double *cs, *X, *vS, *Yc, *fc; const int *vrow, *slot;
+  double* zpart; unsigned long long* nneg;
+  int nA, nB, nCl, tshift, ntile; i64 per_m;
+  static constexpr bool kReduce = true;
+  struct Row { double* p; const double* x; const double* c; double w, f, z; unsigned neg; };
   __device__ __forceinline__ Row row(int m, int i) const {
     const int b = i / nCl, cl = i % nCl;
-    return Row{V + (i64)m * per_m + (i64)i * nA, X + b, cs + (i64)m * nA, vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl]};
+    return Row{V + (i64)m * per_m + (i64)i * nA, X + b, cs + (i64)m * nA, vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl],
+               fc[(i64)m * nCl + cl], 0.0, 0u};
   }
-  __device__ __forceinline__ void put(const Row& r, int, int a, double v) const {
-    r.p[a] = v * r.w * r.c[a] * r.x[(a >> tshift) * nB];
+  __device__ __forceinline__ void tally(Row& r, double v) const {
+    if (v > 0.0) r.z += v * r.f;
+    else if (v < 0.0) r.neg++;
   }
-  __device__ __forceinline__ void put2(const Row& r, int, int a, double v0, double v1) const {
-    const double x0 = r.x[(a >> tshift) * nB], x1 = r.x[((a + 1) >> tshift) * nB];
-    if (((nA | a) & 1) == 0) *reinterpret_cast<double2*>(r.p + a) = make_double2(v0 * r.w * r.c[a] * x0, v1 * r.w * r.c[a + 1] * x1);
-    else { r.p[a] = v0 * r.w * r.c[a] * x0; r.p[a + 1] = v1 * r.w * r.c[a + 1] * x1; }
+  __device__ __forceinline__ void put(Row& r, int, int a, double v) const {
+    const double o = v * r.w * r.c[a] * r.x[(a >> tshift) * nB];
+    r.p[a] = o;
+    tally(r, o);
+  }
+  __device__ __forceinline__ void put2(Row& r, int, int a, double v0, double v1) const {
+    const double o0 = v0 * r.w * r.c[a] * r.x[(a >> tshift) * nB], o1 = v1 * r.w * r.c[a + 1] * r.x[((a + 1) >> tshift) * nB];
+    if (((nA | a) & 1) == 0) *reinterpret_cast<double2*>(r.p + a) = make_double2(o0, o1);
+    else { r.p[a] = o0; r.p[a + 1] = o1; }
+    tally(r, o0);
+    tally(r, o1);
+  }
+  __device__ __forceinline__ void collect(const Row& r, double& z, unsigned& n) const { z += r.z; n += r.neg; }
+  __device__ __forceinline__ void tile_done(int m, int tile, double z, unsigned n) const {
+    zpart[(i64)m * ntile + tile] = z;
+    if (n) atomicAdd(nneg, (unsigned long long)n);
   }
 };
 // cs[m][a] = hS[hrow[m]][a] * wA[a]
@@ -721,24 +737,28 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         TN_LAUNCH_CHECK(h);
         ArPV ar{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
         LdPB be{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r};
-        EpPV ep{V.p, cs.p, c.X, c.BvS, c.Yc, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
-        if (!launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
+        const int ntile = (Mg + 127) / 128;
+        DBuf<double> zpart(h, (size_t)nb * std::max(ntile, 64));
+        EpPV ep{V.p, cs.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
+                c.nA, c.nB, c.nCl, c.tshift, ntile, per_m};
+        if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
+          // Z and the negative count came out of the GEMM epilogue: no extra pass over V
+          k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
+          TN_LAUNCH_CHECK(h);
+        } else {
           LdPA a{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
           StPV e{V.p, c.BhS, c.wA, c.X, c.BvS, c.Yc, hrow.p, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
           dim3 grid(nb, cdiv(Mg, 64), cdiv(Ng, 64));
           k_gemm<64, 64, 16, 2, 2, true, true, LdPA, LdPB, StPV><<<grid, 128, 0, h->stream>>>(Mg, Ng, Dr, 1, a, be, e);
           TN_LAUNCH_CHECK(h);
+          int lgA = 0;
+          while ((1 << lgA) < c.nA) lgA++;
+          const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
+          k_beam_Z<<<dim3(nchunk, nb), 256, 0, h->stream>>>(V.p, per_m, lgA, c.nCl, fc.p, zpart.p, nneg.p);
+          TN_LAUNCH_CHECK(h);
+          k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, nchunk, Z.p);
+          TN_LAUNCH_CHECK(h);
         }
-      }
-      {
-        int lgA = 0;
-        while ((1 << lgA) < c.nA) lgA++;
-        const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
-        DBuf<double> zpart(h, (size_t)nb * nchunk);
-        k_beam_Z<<<dim3(nchunk, nb), 256, 0, h->stream>>>(V.p, per_m, lgA, c.nCl, fc.p, zpart.p, nneg.p);
-        TN_LAUNCH_CHECK(h);
-        k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, nchunk, Z.p);
-        TN_LAUNCH_CHECK(h);
       }
       t_c.stop();
       if (y == 0 && x == 0) {

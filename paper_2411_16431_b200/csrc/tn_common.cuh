@@ -83,6 +83,7 @@ struct tn_handle {
   int D = 0, sweeps = 0;
   // options
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
+  int svd_skip_first = 0;   // predictor (contract.cu): skip the first Rayleigh-Ritz step of the next truncated SVD
   double svd_tol = 1e-11;
   i64 select_direct_max = 1ll << 22;
   // runtime
