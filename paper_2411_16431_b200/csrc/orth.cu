@@ -10,6 +10,9 @@
 // next round (conditioning improved by ~1e6.5) finishes the job; exactly-zero columns stay zero.
 // Rounds stop early (device flag) once ||G - I||_max is at rounding level.
 #include "kernels.cuh"
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -30,6 +33,69 @@ __device__ __forceinline__ double block_max256(double v, double* sh) {
   double r = sh[0];
   __syncthreads();
   return r;
+}
+
+// Last stage of a round, run by ONE CTA on the reduced Gram matrix in shared memory (sG [k x k], ld KP + 1):
+// test ||G - I||, pivot-floored Cholesky, triangular inverse, T = L^-T to global memory (zero-padded KP x KP).
+// Returns true (to all threads) when Y is already orthonormal to rounding.
+template <int KP>
+__device__ bool orth_factor(double* sG, double* sX, double* s_red, int k, double tol, double frel, double* Tout) {
+  constexpr int LG = KP + 1;
+  const int tid = threadIdx.x;
+  double dev = 0.0, md = 0.0;
+  for (int idx = tid; idx < k * k; idx += OR_THREADS) {
+    int i = idx / k, j = idx % k;
+    double v = sG[i * LG + j];
+    dev = fmax(dev, fabs(v - (i == j ? 1.0 : 0.0)));
+    if (i == j) md = fmax(md, v);
+  }
+  dev = block_max256(dev, s_red);
+  md = block_max256(md, s_red);
+  if (dev <= tol) return true;
+  const double floor_ = frel * md;
+  // ---- Cholesky G = L L^T (lower triangle of sG, in place).  A pivot at or below the floor (rounding noise of
+  // the Gram matrix, c * eps * md) is replaced by the floor and its sub-column is dropped: noise directions
+  // are scaled up by a bounded factor and are NOT used to "orthogonalise" later columns -- dividing noise by
+  // noise gives O(1) multipliers and an exponentially ill-conditioned L.  The next round sees them at a
+  // resolvable size.
+  for (int j = 0; j < k; j++) {
+    __syncthreads();
+    double d = sG[j * LG + j];
+    const bool floored = !(d > floor_);
+    if (floored) d = floor_;
+    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;
+    __syncthreads();
+    for (int i = j + tid; i < k; i += OR_THREADS)
+      sG[i * LG + j] = (i == j) ? d * inv : (floored ? 0.0 : sG[i * LG + j] * inv);
+    __syncthreads();
+    if (floored) continue;
+    const int n = k - j - 1;
+    for (int idx = tid; idx < n * n; idx += OR_THREADS) {
+      int i = j + 1 + idx / n, c = j + 1 + idx % n;
+      if (c <= i) sG[i * LG + c] -= sG[i * LG + j] * sG[c * LG + j];
+    }
+  }
+  // ---- X = L^-1 (lower triangular) by a column sweep of rank-1 updates
+  for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
+  for (int p = 0; p < k; p++) {
+    __syncthreads();
+    const double lp = sG[p * LG + p];
+    const double ip = lp > 0.0 ? 1.0 / lp : 0.0;
+    for (int c = tid; c <= p; c += OR_THREADS) sX[p * LG + c] *= ip;
+    __syncthreads();
+    const int n = k - p - 1, w = p + 1;
+    for (int idx = tid; idx < n * w; idx += OR_THREADS) {
+      int i = p + 1 + idx / w, c = idx % w;
+      sX[i * LG + c] -= sG[i * LG + p] * sX[p * LG + c];
+    }
+  }
+  __syncthreads();
+  // T = L^-T (upper triangular), zero-padded to KP x KP
+  for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
+    int c = idx / KP, j = idx % KP;
+    Tout[idx] = (c <= j && j < k) ? sX[j * LG + c] : 0.0;
+  }
+  return false;
 }
 
 template <int KT>
@@ -150,63 +216,132 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y
     sG[(idx / KP) * LG + idx % KP] = s;
   }
   __syncthreads();
-  double dev = 0.0, md = 0.0;
-  for (int idx = tid; idx < k * k; idx += OR_THREADS) {
-    int i = idx / k, j = idx % k;
-    double v = sG[i * LG + j];
-    dev = fmax(dev, fabs(v - (i == j ? 1.0 : 0.0)));
-    if (i == j) md = fmax(md, v);
-  }
-  dev = block_max256(dev, s_red);
-  md = block_max256(md, s_red);
-  if (tid == 0) { ctl->top = 0; ctl->rounds++; }
+  const bool ortho = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
+  if (tid == 0) { ctl->top = 0; ctl->rounds++; if (ortho) ctl->done = 1; }
   if (tid < OR_MAXG) ctl->grp[tid] = 0;
-  if (dev <= tol) {
-    if (tid == 0) ctl->done = 1;
-    return;
-  }
-  const double floor_ = frel * md;
-  // ---- Cholesky G = L L^T (lower triangle of sG, in place).  A pivot at or below the floor (rounding noise of
-  // the Gram matrix, c * eps * md) is replaced by the floor and its sub-column is dropped: noise directions
-  // are scaled up by a bounded factor and are NOT used to "orthogonalise" later columns -- dividing noise by
-  // noise gives O(1) multipliers and an exponentially ill-conditioned L.  The next round sees them at a
-  // resolvable size.
-  for (int j = 0; j < k; j++) {
+}
+
+// All rounds of one orthonormalisation in ONE cooperative launch (grid <= resident CTAs): the rounds are separated
+// by grid-wide barriers instead of kernel boundaries, which removes ~5 launches and their gaps from every call.
+// Same arithmetic and the same reduction order as k_orth_pass (bit-identical results).
+template <int KT>
+__global__ void __launch_bounds__(OR_THREADS) k_orth_coop(double* __restrict__ Y, i64 m, int k, double* __restrict__ Tbuf,
+                                                          double* __restrict__ part, OrthCtl* ctl, int passes, double tol,
+                                                          double frel) {
+  constexpr int KP = 8 * KT, LD = smem_ld(KP), NQ = (KT + 7) / 8, LG = KP + 1;
+  extern __shared__ double sm[];
+  __shared__ double s_red[OR_THREADS];
+  cg::grid_group grid = cg::this_grid();
+  double* sT = sm;
+  double* sIn = sT + KP * LD;
+  double* sOut = sIn + OR_ROWS * LD;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nb = gridDim.x, ngrp = (nb + OR_GS - 1) / OR_GS;
+  double* gpart = part + (size_t)nb * KP * KP;
+  const i64 ntile = (m + OR_ROWS - 1) / OR_ROWS;
+  for (int p = 0; p <= passes; p++) {
+    const bool has_T = p > 0, do_gram = p < passes;
+    const double* Tin = Tbuf + (size_t)((p - 1) & 1) * KP * KP;
+    double* Tout = Tbuf + (size_t)(p & 1) * KP * KP;
     __syncthreads();
-    double d = sG[j * LG + j];
-    const bool floored = !(d > floor_);
-    if (floored) d = floor_;
-    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;
-    __syncthreads();
-    for (int i = j + tid; i < k; i += OR_THREADS)
-      sG[i * LG + j] = (i == j) ? d * inv : (floored ? 0.0 : sG[i * LG + j] * inv);
-    __syncthreads();
-    if (floored) continue;
-    const int n = k - j - 1;
-    for (int idx = tid; idx < n * n; idx += OR_THREADS) {
-      int i = j + 1 + idx / n, c = j + 1 + idx % n;
-      if (c <= i) sG[i * LG + c] -= sG[i * LG + j] * sG[c * LG + j];
+    if (has_T)
+      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) sT[(idx / KP) * LD + idx % KP] = __ldcg(Tin + idx);
+    double g[NQ][KT][2];
+#pragma unroll
+    for (int q = 0; q < NQ; q++)
+#pragma unroll
+      for (int j = 0; j < KT; j++) g[q][j][0] = g[q][j][1] = 0.0;
+    for (i64 tile = blockIdx.x; tile < ntile; tile += nb) {
+      const i64 r0 = tile * OR_ROWS;
+      __syncthreads();
+      for (int idx = tid; idx < OR_ROWS * KP; idx += OR_THREADS) {
+        int r = idx / KP, c = idx % KP;
+        i64 gr = r0 + r;
+        sIn[r * LD + c] = (gr < m && c < k) ? Y[gr * k + c] : 0.0;
+      }
+      __syncthreads();
+      const double* src = sIn;
+      if (has_T) {
+        double o[KT][2];
+#pragma unroll
+        for (int j = 0; j < KT; j++) o[j][0] = o[j][1] = 0.0;
+#pragma unroll 4
+        for (int kk = 0; kk < KP; kk += 4) {
+          double a = sIn[(8 * warp + (lane >> 2)) * LD + kk + (lane & 3)];
+#pragma unroll
+          for (int j = 0; j < KT; j++) dmma884(o[j][0], o[j][1], a, sT[(kk + (lane & 3)) * LD + 8 * j + (lane >> 2)]);
+        }
+#pragma unroll
+        for (int j = 0; j < KT; j++) {
+          int row = 8 * warp + (lane >> 2), col = 8 * j + 2 * (lane & 3);
+          sOut[row * LD + col] = o[j][0];
+          sOut[row * LD + col + 1] = o[j][1];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < OR_ROWS * KP; idx += OR_THREADS) {
+          int r = idx / KP, c = idx % KP;
+          i64 gr = r0 + r;
+          if (gr < m && c < k) Y[gr * k + c] = sOut[r * LD + c];
+        }
+        src = sOut;
+      }
+      if (do_gram) {
+#pragma unroll
+        for (int q = 0; q < NQ; q++) {
+          const int ti = warp + 8 * q;
+          if (ti < KT) {
+#pragma unroll 4
+            for (int rr = 0; rr < OR_ROWS; rr += 4) {
+              const double* row = src + (rr + (lane & 3)) * LD + (lane >> 2);
+              double a = row[8 * ti];
+#pragma unroll
+              for (int j = 0; j < KT; j++) dmma884(g[q][j][0], g[q][j][1], a, row[8 * j]);
+            }
+          }
+        }
+      }
     }
-  }
-  // ---- X = L^-1 (lower triangular) by a column sweep of rank-1 updates
-  for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
-  for (int p = 0; p < k; p++) {
-    __syncthreads();
-    const double lp = sG[p * LG + p];
-    const double ip = lp > 0.0 ? 1.0 / lp : 0.0;
-    for (int c = tid; c <= p; c += OR_THREADS) sX[p * LG + c] *= ip;
-    __syncthreads();
-    const int n = k - p - 1, w = p + 1;
-    for (int idx = tid; idx < n * w; idx += OR_THREADS) {
-      int i = p + 1 + idx / w, c = idx % w;
-      sX[i * LG + c] -= sG[i * LG + p] * sX[p * LG + c];
+    if (!do_gram) break;
+    double* mine = part + (size_t)blockIdx.x * KP * KP;
+#pragma unroll
+    for (int q = 0; q < NQ; q++) {
+      const int ti = warp + 8 * q;
+      if (ti < KT) {
+#pragma unroll
+        for (int j = 0; j < KT; j++) {
+          int row = 8 * ti + (lane >> 2), col = 8 * j + 2 * (lane & 3);
+          mine[row * KP + col] = g[q][j][0];
+          mine[row * KP + col + 1] = g[q][j][1];
+        }
+      }
     }
-  }
-  __syncthreads();
-  // T = L^-T (upper triangular), zero-padded to KP x KP
-  for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
-    int c = idx / KP, j = idx % KP;
-    Tout[idx] = (c <= j && j < k) ? sX[j * LG + c] : 0.0;
+    grid.sync();
+    if ((int)blockIdx.x < ngrp) {          // level 1: CTA g reduces group g in CTA order
+      const int g0 = blockIdx.x * OR_GS, g1 = min(nb, g0 + OR_GS);
+      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
+        double s = 0.0;
+#pragma unroll 4
+        for (int b = g0; b < g1; b++) s += __ldcg(part + (size_t)b * KP * KP + idx);
+        gpart[(size_t)blockIdx.x * KP * KP + idx] = s;
+      }
+    }
+    grid.sync();
+    if (blockIdx.x == 0) {                 // level 2 + factorisation
+      double* sG = sm;
+      double* sX = sm + KP * LG;
+      __syncthreads();
+      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
+        double s = 0.0;
+#pragma unroll 4
+        for (int b = 0; b < ngrp; b++) s += __ldcg(gpart + (size_t)b * KP * KP + idx);
+        sG[(idx / KP) * LG + idx % KP] = s;
+      }
+      __syncthreads();
+      const bool ortho = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
+      if (tid == 0) { ctl->rounds++; if (ortho) ctl->done = 1; }
+    }
+    grid.sync();
+    if (*(volatile int*)&ctl->done) break;
   }
 }
 
@@ -219,12 +354,33 @@ void run_orth(tn_handle* h, double* Y, i64 m, int k, int passes) {
     TN_CUDA(cudaFuncSetAttribute(k_orth_pass<KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr = true;
   }
-  const int nb = (int)std::min<i64>(148, (m + OR_ROWS - 1) / OR_ROWS);
+  int nb = (int)std::min<i64>(148, (m + OR_ROWS - 1) / OR_ROWS);
   DBuf<double> part(h, (size_t)(nb + OR_MAXG) * KP * KP), T(h, 2 * (size_t)KP * KP);
   DBuf<OrthCtl> ctl(h, 1);
   TN_CUDA(cudaMemsetAsync(ctl.p, 0, sizeof(OrthCtl), h->stream));
-  const double tol = 1e-15 * (32.0 + std::sqrt((double)m));
-  const double frel = 1e-11 * std::max(1.0, std::sqrt((double)m) / 128.0);   // pivot floor relative to max_i G_ii
+  double tol = 1e-15 * (32.0 + std::sqrt((double)m));
+  double frel = 1e-11 * std::max(1.0, std::sqrt((double)m) / 128.0);   // pivot floor relative to max_i G_ii
+  // ---- one cooperative launch for all rounds when the device supports it and the grid is co-resident
+  static int coop_slots = -1;
+  if (coop_slots < 0) {
+    int dev = 0, coop = 0, sms = 0, occ = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    TN_CUDA(cudaFuncSetAttribute(k_orth_coop<KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_orth_coop<KT>, OR_THREADS, smem);
+    coop_slots = coop ? sms * occ : 0;
+  }
+  if (coop_slots > 0 && nb <= coop_slots) {
+    double* Yp = Y;
+    double* Tp = T.p;
+    double* pp = part.p;
+    OrthCtl* cp = ctl.p;
+    void* args[] = {&Yp, &m, &k, &Tp, &pp, &cp, &passes, &tol, &frel};
+    TN_CUDA(cudaLaunchCooperativeKernel((const void*)k_orth_coop<KT>, dim3(nb), dim3(OR_THREADS), args, smem, h->stream));
+    TN_LAUNCH_CHECK(h);
+    return;
+  }
   for (int p = 0; p <= passes; p++) {
     const double* Tin = p > 0 ? T.p + (size_t)((p - 1) & 1) * KP * KP : nullptr;
     double* Tout = T.p + (size_t)(p & 1) * KP * KP;
