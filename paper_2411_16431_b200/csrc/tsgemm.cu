@@ -207,13 +207,14 @@ void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb
 template <bool TRANS>
 void pick_nt(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
              i64 Kred, const TsBatch& tsb) {
-  if (N > 96) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);          // chunks of 64 columns
-  else if (N <= 16) pick_warps<2, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
-  else if (N <= 32) pick_warps<4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
-  else if (N <= 48) pick_warps<6, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
-  else if (N <= 64) pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
-  else if (N <= 80) pick_warps<10, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
-  else pick_warps<12, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb);
+  if (N > 96) { pick_warps<8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb); return; }   // chunks of 64 columns
+  switch ((N + 7) / 8) {   // one 8-column register tile per 8 columns: no padding beyond the last tile
+#define TN_TS_CASE(NT_) case NT_: pick_warps<NT_, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, tsb); break;
+    TN_TS_CASE(1) TN_TS_CASE(2) TN_TS_CASE(3) TN_TS_CASE(4) TN_TS_CASE(5) TN_TS_CASE(6)
+    TN_TS_CASE(7) TN_TS_CASE(8) TN_TS_CASE(9) TN_TS_CASE(10) TN_TS_CASE(11) TN_TS_CASE(12)
+#undef TN_TS_CASE
+    default: break;
+  }
 }
 
 bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
