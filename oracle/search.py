@@ -94,9 +94,56 @@ def _above_vectors(model, y, x, above):
     return uvec, dvec
 
 
-def branch_and_bound(model, R, lognorm, M, stats=None):
+def _forward_legs(model, y, x, n_last):
+    """Directions of cell (x, y) that lead to a cell visited AFTER cell index n_last (row-major order)."""
+    out = []
+    for d, (dy, dx) in (("right", (0, 1)), ("down", (1, 0)), ("dout", (1, 1))):
+        yy, xx = y + dy, x + dx
+        if yy < model.Ly and xx < model.Lx and yy * model.Lx + xx > n_last:
+            out.append(d)
+    return out
+
+
+def boundary_codes(model, y, x, beam_states):
+    """Boundary of every candidate (parent m, new state X of cell (x, y)), Eq. (8): the
+    sub-configuration of the visited spins that couple to not yet visited cells, as
+    (id of the parent's part, integer code of the new cell's part [d]).  Only rows y-1 and y can contribute."""
+    Lx = model.Lx
+    n = y * Lx + x
+    ids, keys = {}, []
+    for st in beam_states:
+        key = []
+        for yy in (y - 1, y):
+            if yy < 0:
+                continue
+            for xx in range(Lx):
+                idx = yy * Lx + xx
+                if idx >= n:
+                    break
+                c = model.cells[yy][xx]
+                for d in _forward_legs(model, yy, xx, n):
+                    key.append(int(c.P[d][st[idx]]))
+        keys.append(ids.setdefault(tuple(key), len(ids)))
+    c = model.cells[y][x]
+    code = np.zeros(c.d, dtype=np.int64)
+    for d in _forward_legs(model, y, x, n):
+        code = code * c.n[d] + c.P[d]
+    return np.asarray(keys, dtype=np.int64), code
+
+
+def merge_by_boundary(score, parent, state, parent_key, state_code):
+    """Fig. 3(d): among candidates with the same boundary keep the most probable one
+    (ties by the S8 order).  Returns the indices of the survivors."""
+    key = parent_key[parent] * (int(state_code.max()) + 1) + state_code[state]
+    order = np.lexsort((state, parent, -score, key))
+    first = np.r_[True, key[order][1:] != key[order][:-1]]
+    return np.sort(order[first])
+
+
+def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
     """Returns dict(states [n, N] int8 +-1, energies [n], logp [n] (descending), log_pd, log_z,
-    cell_states [n, Ly*Lx])."""
+    cell_states [n, Ly*Lx]).  merge=True adds the paper's merge-by-boundary step (Fig. 3(d)) before the bound
+    (reading S11: off by default; the CUDA path does not have it yet)."""
     Ly, Lx = model.Ly, model.Lx
     beam_states = [[]]                  # per element: list of chosen cell states (row-major)
     beam_logp = np.zeros(1)
@@ -140,6 +187,12 @@ def branch_and_bound(model, R, lognorm, M, stats=None):
             score = np.concatenate(cand_score)
             parent = np.concatenate(cand_parent)
             state = np.concatenate(cand_state)
+            if merge:
+                pk, sc = boundary_codes(model, y, x, beam_states)
+                surv = merge_by_boundary(score, parent, state, pk, sc)
+                score, parent, state = score[surv], parent[surv], state[surv]
+                if stats is not None:
+                    stats["merged_away"] = stats.get("merged_away", 0) + int(pk.size * sc.size - surv.size)
             keep, disc = select_top(score, parent, state, M)
             keep = keep[np.isfinite(score[keep])]                          # never keep p = 0
             log_pd = max(log_pd, disc)

@@ -355,3 +355,52 @@ def test_truncated_marginals_close_to_exact():
     assert abs(tr["log_z"] - ex["log_z"]) < 1e-3 * abs(ex["log_z"])
     assert tr["energies"].min() == ex["energies"].min()
     assert max(st["min_sigma"]) < 1.0
+
+
+# ---------------------------------------------------------------- merge by boundary (Fig. 3(d))
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta", MINIS)
+def test_merge_by_boundary_never_loses_the_most_probable_state(Ly, Lx, S, ns, p, seed, beta):
+    """Two prefixes with the same boundary have identical futures (Eqs. (8)-(9) PAPER.md:100-107), so dropping the
+    less probable one cannot lose the most probable full state: with merging on and no pruning by the bound
+    (M >= number of boundaries) the first returned state is the brute-force ground state with its exact logp,
+    while the number of kept prefixes stays far below the unmerged beam."""
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    E = brute.all_energies(inst)
+    m = model.Model(inst).set_beta(beta)
+    R, ln = mps.contract(m, 0, 0)
+    M = 1 << 14
+    st = {}
+    out = search.branch_and_bound(m, R, ln, M, stats=st, merge=True)
+    idx, El = brute.lowest(E, 1)
+    gs = brute.index_to_spins(idx, inst.n_spins)[0]
+    assert np.array_equal(out["states"][0], gs)
+    lz = brute.log_z(E, beta)
+    assert abs(out["logp"][0] - (-beta * El[0] - lz)) <= 1e-10 * abs(lz)
+    assert st["merged_away"] > 0
+    # every survivor is exact too, and no two survivors share a boundary with a better twin: logp = -beta E - log Z
+    assert np.allclose(out["logp"], -beta * out["energies"] - lz, rtol=0, atol=1e-9 * abs(lz))
+    # without merging the same M gives the same best state (pruning never triggers on these sizes or keeps it)
+    ref = search.branch_and_bound(m, R, ln, M)
+    assert np.array_equal(ref["states"][0], gs)
+    assert out["logp"].size < ref["logp"].size or ref["logp"].size < M
+
+
+def test_merge_groups_are_boundaries():
+    """Survivors of one merge step have pairwise different boundaries; a merged-away candidate has a survivor
+    with the same boundary and a score at least as large."""
+    inst = instances.lattice(2, 3, 2, 2, p_keep=0.9, seed=7)
+    m = model.Model(inst).set_beta(0.9)
+    beam = [[3, 1, 0], [5, 1, 0], [3, 9, 2]]                     # three prefixes covering row 0
+    pk, sc = search.boundary_codes(m, 1, 0, beam)
+    d = m.cells[1][0].d
+    rng = np.random.default_rng(3)
+    score = rng.standard_normal(len(beam) * d)
+    parent = np.repeat(np.arange(len(beam)), d)
+    state = np.tile(np.arange(d), len(beam))
+    surv = search.merge_by_boundary(score, parent, state, pk, sc)
+    key = pk[parent] * (sc.max() + 1) + sc[state]
+    assert np.unique(key[surv]).size == surv.size == np.unique(key).size
+    best = {}
+    for k, s_ in zip(key.tolist(), score.tolist()):
+        best[k] = max(best.get(k, -np.inf), s_)
+    assert all(score[i] == best[key[i]] for i in surv)
