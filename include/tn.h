@@ -72,6 +72,8 @@ enum {
                              block's Ritz values decay slowly (same converged subspace, fewer Theta applies)  */
   TN_OPT_SVD_LOCK = 8,    /* 1 (default) / 0: freeze converged leading Ritz triplets of the truncated SVD and apply
                              Theta only to the remaining columns (deflation; same converged subspace)          */
+  TN_OPT_MERGE = 9,       /* 0 (default) / 1: merge candidates with the same boundary before the bound, keeping the
+                             most probable one (Fig. 3(d); reading S11)                 */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */
@@ -104,6 +106,7 @@ typedef struct {
   int64_t theta_apply_calls; /* Theta-core x skinny GEMM calls (launches of the dominant kernel)  */
   int64_t cheb_steps;        /* total Chebyshev degrees spent in filtered subspace steps           */
   int64_t svd_locked_cols;   /* Ritz triplets frozen by the locked subspace iteration (summed over all SVDs)        */
+  int64_t merged_away;       /* candidates removed by TN_OPT_MERGE among those above the selection threshold        */
   int64_t svd_unconverged;   /* truncated SVDs stopped by TN_OPT_SVD_MAXIT with a residual above tolerance:
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
 } tn_stats;

@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
                     "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
-OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 
 
 class TnError(RuntimeError):
@@ -27,7 +27,7 @@ class TnStats(C.Structure):
         "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
         "bytes_theta_apply", "flop_search", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
-            "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "svd_unconverged")]
+            "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -215,6 +215,7 @@ int tn_set_option(tn_handle* h, int32_t key, double v) {
       h->exact_cap = (int)v; break;
     case TN_OPT_SVD_CHEB: h->svd_cheb = v != 0.0; break;
     case TN_OPT_SVD_LOCK: h->svd_lock = v != 0.0; break;
+    case TN_OPT_MERGE: h->merge = v != 0.0; break;
     case TN_OPT_SELECT_DIRECT_MAX:
       if (v < 0) tn_throw(TN_ERR_ARG, "select direct max must be >= 0");
       h->select_direct_max = (i64)v; break;

@@ -12,6 +12,7 @@
 #include "bgemm.cuh"
 #include <algorithm>
 #include <cfloat>
+#include <map>
 
 namespace {
 
@@ -505,6 +506,113 @@ __global__ void __launch_bounds__(1024) k_bitonic_smem(Cand* c, unsigned n) {
     }
   for (unsigned i = threadIdx.x; i < n; i += blockDim.x) c[i] = sc[i];
 }
+// ---- merge by boundary (Fig. 3(d), Eq. (8)) ------------------------------------------
+// Candidates with the same boundary (the projected legs of visited cells towards not yet visited cells) have
+// identical futures; only the most probable one is kept.  The boundary of candidate (m, a, b, c_lo, c_hi) is
+// (pid[m], P_right a, P_down b, P_dout c_lo): c_hi never appears (its only neighbour, up-left, is visited), so the
+// prefilter already keeps one c_hi per V entry; pid[m] = dense id of the parent's part (host, from the beam states).
+struct MCand { unsigned long long g; double score; int parent; unsigned state; };
+__device__ __forceinline__ bool mcand_before(const MCand& x, const MCand& y) {
+  if (x.g != y.g) return x.g < y.g;
+  if (x.score != y.score) return x.score > y.score;
+  if (x.parent != y.parent) return x.parent < y.parent;
+  return x.state < y.state;
+}
+__global__ void __launch_bounds__(256) k_sel_prefilter_merge(SelArgs a, int lgA, double thr, const double* fmx, Raw* out,
+                                                             unsigned* count, unsigned cap) {
+  const int m = blockIdx.y, nchunk = gridDim.x;
+  const i64 per2 = a.per_m >> 1;
+  const i64 c0 = per2 * blockIdx.x / nchunk, c1 = per2 * (blockIdx.x + 1) / nchunk;
+  const double2* v2 = reinterpret_cast<const double2*>(a.V + (i64)m * a.per_m);
+  const double sc = a.scale[m];
+  const double* fm = fmx + (i64)m * a.nCl;
+  for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
+    const double2 x = v2[q];
+    const int i = (int)((2 * q) >> lgA), cl = i & (a.nCl - 1);
+    const double bound = fmax(x.x, x.y) * sc * fm[cl];
+    if (!(bound >= thr) || !(bound > 0.0)) continue;
+#pragma unroll
+    for (int e = 0; e < 2; e++) {
+      const double v = e ? x.y : x.x;
+      if (!(v > 0.0) || !(v * sc * fm[cl] >= thr)) continue;
+      int best = 0;
+      double rb = -1.0;
+      for (int ch = 0; ch < a.nCh; ch++) {
+        const double r = sel_fcd(a, m, cl, ch);
+        if (r > rb) { rb = r; best = ch; }
+      }
+      if (!(rb > 0.0)) continue;
+      unsigned idx = atomicAdd(count, 1u);
+      if (idx < cap) out[idx] = Raw{m, i, (int)((2 * q + e) & (a.nA - 1)), best};
+    }
+  }
+}
+struct MergeLegs { const int *Pr, *Pd, *Po; int n_r, n_d, n_o, use_r, use_d, use_o; };
+__global__ void k_merge_score(SelArgs a, const Raw* raw, unsigned n, unsigned npad, const double* logp, const double* Z,
+                              int ns, int S, const int* pid, MergeLegs lg, MCand* out) {
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= npad) return;
+  if (t >= n) { out[t] = MCand{~0ull, -INFINITY, 0x7fffffff, 0xffffffffu}; return; }
+  Raw q = raw[t];
+  int b = q.i / a.nCl, cl = q.i % a.nCl;
+  double u = a.V[(i64)q.m * a.per_m + (i64)q.i * a.nA + q.a] * sel_fcd(a, q.m, cl, q.ch);
+  unsigned state = (unsigned)q.a;
+  if (S >= 2) state |= (unsigned)b << ns;
+  if (S == 3) state |= ((unsigned)cl | ((unsigned)q.ch << (ns / 2))) << (2 * ns);
+  // for S == 1 the vertical sub-cluster IS sub-cluster 0: b == a there (i = b * nCl + cl with nCl = 1)
+  unsigned long long g = (unsigned long long)pid[q.m];
+  g = g * (unsigned long long)(lg.use_r ? lg.n_r : 1) + (unsigned long long)(lg.use_r ? lg.Pr[q.a] : 0);
+  g = g * (unsigned long long)(lg.use_d ? lg.n_d : 1) + (unsigned long long)(lg.use_d ? lg.Pd[b] : 0);
+  g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
+  out[t] = MCand{g, logp[q.m] + log(u / Z[q.m]), q.m, state};
+}
+__global__ void k_mbitonic_step(MCand* c, unsigned n, unsigned k, unsigned j) {
+  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  unsigned l = i ^ j;
+  if (l > i) {
+    MCand x = c[i], y = c[l];
+    bool up = (i & k) == 0;
+    if (up ? mcand_before(y, x) : mcand_before(x, y)) { c[i] = y; c[l] = x; }
+  }
+}
+__global__ void __launch_bounds__(1024) k_mbitonic_smem(MCand* c, unsigned n) {
+  extern __shared__ MCand smc[];
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) smc[i] = c[i];
+  __syncthreads();
+  for (unsigned k = 2; k <= n; k <<= 1)
+    for (unsigned j = k >> 1; j > 0; j >>= 1) {
+      for (unsigned i = threadIdx.x; i < n; i += blockDim.x) {
+        unsigned l = i ^ j;
+        if (l > i) {
+          MCand x = smc[i], y = smc[l];
+          bool up = (i & k) == 0;
+          if (up ? mcand_before(y, x) : mcand_before(x, y)) { smc[i] = y; smc[l] = x; }
+        }
+      }
+      __syncthreads();
+    }
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) c[i] = smc[i];
+}
+// first (= most probable, S8 order) member of every group of the sorted list
+__global__ void k_merge_first(const MCand* c, unsigned n, Cand* out, unsigned* count) {
+  unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const MCand x = c[t];
+  if (x.g == ~0ull) return;
+  if (t == 0 || c[t - 1].g != x.g) out[atomicAdd(count, 1u)] = Cand{x.score, x.parent, x.state};
+}
+__global__ void k_fill_sentinel(Cand* c, unsigned from, unsigned to) {
+  unsigned t = from + blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < to) c[t] = Cand{-INFINITY, 0x7fffffff, 0xffffffffu};
+}
+static int pext_host(int v, int mask) {
+  int out = 0, bit = 0;
+  for (int i = 0; i < 8; i++)
+    if ((mask >> i) & 1) { out |= ((v >> i) & 1) << bit; bit++; }
+  return out;
+}
+
 // new beam from the sorted candidates
 __global__ void k_new_beam(const Cand* cand, int nkeep, int M, const unsigned* st_old, unsigned* st_new, int ncell_ld,
                            int cellidx, const int* slot_old, int* slot_new, double* logp_new, const double* LG,
@@ -625,6 +733,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   const unsigned ccap = 1u << 22;                   // compact candidate list of the prefilter pass
   DBuf<double> ckeys(h, ccap), fmx(h, (size_t)M * 16);
   DBuf<Raw> craw(h, ccap);
+  const unsigned mcap = h->merge ? (1u << 20) : 1u;   // survivors handled by the merge route
+  DBuf<MCand> mcand(h, 2 * (size_t)mcap);
+  DBuf<Cand> mcands(h, 2 * (size_t)mcap + 4096);
+  DBuf<int> pid(h, M);
   DBuf<Cand> cand(h, npad);
   unsigned* st_cur = stA.p; unsigned* st_nxt = stB.p;
   double* lp_cur = lpA.p; double* lp_nxt = lpB.p;
@@ -787,7 +899,110 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       const int gsel = (int)std::min<i64>(148 * 8, (total + 255) / 256);
       unsigned ncand = 0;
       bool direct = total * c.nCh <= (i64)h->select_direct_max;       // few candidates: radix passes straight on V
-      if (!direct) {
+      bool cand_sorted = false;                                       // set by the merge route (cand.p final and sorted)
+      unsigned np2 = 2;
+      if (h->merge) {
+        // ---- parent part of the boundary: dense ids of the projected forward legs of rows y-1, y (host, tiny)
+        std::vector<unsigned> hst((size_t)nb * ncell);
+        TN_CUDA(cudaMemcpyAsync(hst.data(), st_cur, sizeof(unsigned) * hst.size(), cudaMemcpyDeviceToHost, h->stream));
+        TN_CUDA(cudaStreamSynchronize(h->stream));
+        std::map<std::vector<int>, int> ids;
+        std::vector<int> hpid(nb), key;
+        const unsigned smask = (1u << ns) - 1, hmask = (1u << (ns / 2)) - 1;
+        for (int m = 0; m < nb; m++) {
+          key.clear();
+          for (int yy = std::max(0, y - 1); yy <= y; yy++)
+            for (int xx = 0; xx < Lx; xx++) {
+              const int idx = yy * Lx + xx;
+              if (idx >= cellidx) break;
+              const CellDev& cc = h->cell(yy, xx);
+              const unsigned st = hst[(size_t)m * ncell + idx];
+              const int a_ = (int)(st & smask), b_ = S == 1 ? a_ : (int)((st >> ns) & smask), cl_ = (int)((st >> (2 * ns)) & hmask);
+              if (xx + 1 < Lx && yy * Lx + xx + 1 > cellidx) key.push_back(pext_host(a_, cc.m_right));
+              if (yy + 1 < Ly && (yy + 1) * Lx + xx > cellidx) key.push_back(pext_host(b_, cc.m_down));
+              if (S == 3 && xx + 1 < Lx && yy + 1 < Ly && (yy + 1) * Lx + xx + 1 > cellidx) key.push_back(pext_host(cl_, cc.m_dout));
+            }
+          hpid[m] = ids.emplace(key, (int)ids.size()).first->second;
+        }
+        TN_CUDA(cudaMemcpyAsync(pid.p, hpid.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, h->stream));
+        MergeLegs lg{c.Pr, c.Pd, c.Po, c.n_r, c.n_d, c.n_o, x + 1 < Lx, y + 1 < Ly, S == 3 && x + 1 < Lx && y + 1 < Ly};
+        int lgA = 0;
+        while ((1 << lgA) < c.nA) lgA++;
+        const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
+        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
+        TN_LAUNCH_CHECK(h);
+        double thr = 0.0;                                // few candidates: take every positive entry
+        if (!direct) {
+          for (int pass = 0; pass < 2; pass++) {
+            k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
+            TN_LAUNCH_CHECK(h);
+            k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, 0ull);
+            TN_LAUNCH_CHECK(h);
+          }
+          SelState cur = d2h(h, sel.p);
+          if (!cur.takeall) {
+            long long bits = (long long)cur.thresh;
+            memcpy(&thr, &bits, sizeof(double));
+            thr *= 1.0 - 1e-12;
+          }
+        }
+        bool ok = false;
+        unsigned n1 = 0, ng = 0;
+        for (int attempt = 0; attempt < 4; attempt++) {
+          TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+          k_sel_prefilter_merge<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, thr, fmx.p, craw.p, count.p, mcap);
+          TN_LAUNCH_CHECK(h);
+          n1 = d2h(h, count.p);
+          if (n1 > mcap) break;                          // too many survivors for the merge buffers: unmerged route
+          if (n1 == 0 && thr == 0.0) break;
+          unsigned mp2 = 2;
+          while (mp2 < n1 + 1) mp2 <<= 1;
+          k_merge_score<<<cdiv(mp2, 256), 256, 0, h->stream>>>(sa, craw.p, n1, mp2, lp_cur, Z.p, ns, S, pid.p, lg, mcand.p);
+          TN_LAUNCH_CHECK(h);
+          if (mp2 <= 2048) {
+            k_mbitonic_smem<<<1, 1024, mp2 * sizeof(MCand), h->stream>>>(mcand.p, mp2);
+            TN_LAUNCH_CHECK(h);
+          } else {
+            for (unsigned k = 2; k <= mp2; k <<= 1)
+              for (unsigned j = k >> 1; j > 0; j >>= 1) {
+                k_mbitonic_step<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, k, j);
+                TN_LAUNCH_CHECK(h);
+              }
+          }
+          TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+          k_merge_first<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, mcands.p, count.p);
+          TN_LAUNCH_CHECK(h);
+          ng = d2h(h, count.p);
+          if (ng >= (unsigned)M + 1 || thr == 0.0) { ok = true; break; }
+          thr = attempt < 2 ? thr / 64.0 : 0.0;          // fewer than M + 1 boundaries above the bound: lower it
+        }
+        if (ok) {
+          if (ng == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
+          h->st.merged_away += (int64_t)n1 - (int64_t)ng;
+          while (np2 < ng + 1) np2 <<= 1;
+          while (np2 <= (unsigned)M) np2 <<= 1;
+          k_fill_sentinel<<<cdiv(np2 - ng, 256), 256, 0, h->stream>>>(mcands.p, ng, np2);
+          TN_LAUNCH_CHECK(h);
+          if (np2 <= 4096) {
+            k_bitonic_smem<<<1, 1024, np2 * sizeof(Cand), h->stream>>>(mcands.p, np2);
+            TN_LAUNCH_CHECK(h);
+          } else {
+            for (unsigned k = 2; k <= np2; k <<= 1)
+              for (unsigned j = k >> 1; j > 0; j >>= 1) {
+                k_bitonic_step<<<cdiv(np2, 256), 256, 0, h->stream>>>(mcands.p, np2, k, j);
+                TN_LAUNCH_CHECK(h);
+              }
+          }
+          ncand = ng;
+          cand_sorted = true;
+        } else {
+          TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
+          TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
+        }
+      }
+      if (cand_sorted) {
+        // nothing: the merged route produced the sorted candidate list
+      } else if (!direct) {
         // (1) lower bound of the (M+1)-th largest key from a hashed 1/64 sample of V (two radix digits)
         for (int pass = 0; pass < 2; pass++) {
           k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
@@ -830,7 +1045,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           ncand = std::min(d2h(h, count.p), cap);
         }
       }
-      if (direct) {
+      if (direct && !cand_sorted) {
         TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
         TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
         for (int pass = 0; pass < 6; pass++) {
@@ -847,7 +1062,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         ncand = std::min(d2h(h, count.p), cap);
       }
       if (ncand == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
-      unsigned np2 = 2;
+      Cand* cand_final = cand_sorted ? mcands.p : cand.p;
+      if (!cand_sorted) {
       while (np2 < ncand + 1) np2 <<= 1;   // at least one sentinel so that cand[M] exists when ncand <= M
       while (np2 <= (unsigned)M) np2 <<= 1;
       if (np2 > npad) np2 = npad;
@@ -863,8 +1079,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
             TN_LAUNCH_CHECK(h);
           }
       }
+      }
       const int nkeep = (int)std::min<unsigned>(ncand, (unsigned)M);
-      k_new_beam<<<nkeep, 128, 0, h->stream>>>(cand.p, nkeep, M, st_cur, st_nxt, ncell, cellidx, sl_cur, sl_nxt, lp_nxt,
+      k_new_beam<<<nkeep, 128, 0, h->stream>>>(cand_final, nkeep, M, st_cur, st_nxt, ncell, cellidx, sl_cur, sl_nxt, lp_nxt,
                                                LG.p, npp, Dr, ldLv, Lv_nxt, c.Pd, c.Po, c.n_o, ns, S, pd.p);
       TN_LAUNCH_CHECK(h);
       std::swap(st_cur, st_nxt); std::swap(lp_cur, lp_nxt); std::swap(Lv_cur, Lv_nxt); std::swap(sl_cur, sl_nxt);

@@ -241,6 +241,7 @@ void tables_create(tn_handle* h) {
     c.tshift = S == 1 ? 0 : half;
     c.nT = S == 1 ? nA : nH;
     c.m_left = m.left; c.m_right = m.right; c.m_din = m.din; c.m_dout = m.dout;
+    c.m_up = m.up; c.m_down = m.down;
     c.n_l = 1 << popc(m.left); c.n_r = 1 << popc(m.right);
     c.n_u = 1 << popc(m.up); c.n_d = 1 << popc(m.down);
     c.n_i = 1 << popc(m.din); c.n_o = 1 << popc(m.dout);

@@ -39,6 +39,7 @@ struct CellDev {
   int n_l, n_r, n_u, n_d, n_i, n_o;   // projector ranges (Eq. (5))
   int bh_rows, bv_rows, bd_rows;      // rows of the incoming edge matrices (ranges of the neighbours)
   int m_left, m_right, m_din, m_dout; // coupled-bit masks (m_din relative to the hi half)
+  int m_up, m_down;                   // coupled-bit masks of the vertical sub-cluster
   const double *wA, *X, *Yc, *wC;     // [nA] [nT*nB] [nB*nCl] [nCl*nCh]
   const int *Pl, *Pr, *Pu, *Pd, *Pi, *Po;  // [nA] [nA] [nB] [nB] [nCh] [nCl]
   const double *Bh, *Bv, *Bd;         // [bh_rows*n_l] [bv_rows*n_u] [bd_rows*n_i]
@@ -82,6 +83,7 @@ struct tn_handle {
   bool have_logz = false;
   int D = 0, sweeps = 0;
   // options
+  int merge = 0;            // TN_OPT_MERGE: merge candidates by boundary before the bound (Fig. 3(d))
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
   int svd_skip_first = 0;   // predictor (contract.cu): skip the first Rayleigh-Ritz step of the next truncated SVD
   double svd_tol = 1e-11;

@@ -27,15 +27,15 @@ def mps_overlap(A, B):
     return inner(A, B) / np.sqrt(inner(A, A) * inner(B, B))
 
 
-def run_oracle(inst, beta, D, sweeps, M):
+def run_oracle(inst, beta, D, sweeps, M, merge=False):
     m = model.Model(inst).set_beta(beta)
     R, ln = mps.contract(m, D, sweeps)
-    out = search.branch_and_bound(m, R, ln, M)
+    out = search.branch_and_bound(m, R, ln, M, merge=merge)
     return m, R, ln, out
 
 
-def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=()):
-    m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M)
+def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=False):
+    m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M, merge=merge)
     with _tn(inst) as t:
         for key, val in options:
             t.set_option(key, val)
@@ -163,6 +163,27 @@ def test_numeric_failure_is_reported_not_hidden():
         with pytest.raises(tnb.TnError) as e:
             t.contract(-1, 0) if False else t.branch_and_bound(0)
         assert e.value.code in (-1, -3)
+
+
+MERGE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M)
+    (2, 3, 1, 4, 1.0, 1, 1.5, 0, 0, 16),
+    (3, 2, 2, 2, 0.9, 5, 0.7, 0, 0, 8),
+    (3, 3, 3, 2, 0.85, 7, 0.9, 0, 0, 32),       # mediating tensors, diagonal legs in the boundary
+    (3, 4, 2, 2, 0.9, 3, 0.9, 3, 1, 16),
+    (4, 4, 2, 4, 0.95, 2, 1.0, 6, 1, 64),       # ragged projectors: several cell states share one boundary
+    (3, 3, 3, 4, 0.9, 4, 1.0, 6, 2, 64),
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,D,sweeps,M", MERGE)
+@pytest.mark.parametrize("sampled", [False, True])
+def test_merge_by_boundary_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, sampled):
+    """TN_OPT_MERGE (Fig. 3(d)) against the oracle's merge switch, through both selection routes."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    opts = [(tnb.OPT_MERGE, 1)] + ([(tnb.OPT_SELECT_DIRECT_MAX, 0)] if sampled else [])
+    st = compare(inst, beta, D, sweeps, M, 1e-9 if D == 0 else 1e-6, check_rows=False, options=opts, merge=True)
+    assert st["merged_away"] > 0
 
 
 def test_zero_field_z2_instance():
