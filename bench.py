@@ -40,6 +40,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
     return ap.parse_args()
 
 
@@ -313,6 +314,8 @@ def run_ours(args):
 
     fp64_peak = tnb.tn_fp64_peak()
     t = tnb.TensorNetwork(inst)
+    if args.merge:
+        t.set_option(tnb.OPT_MERGE, 1)
     for _ in range(args.warmup):
         step(t)
     sampler = ClockSampler(local)
@@ -339,6 +342,8 @@ def run_ours(args):
     # ---- e2e: host buffers in, host buffers out, tn_create / tn_destroy inside the timed region
     def e2e_step():
         with tnb.TensorNetwork(inst) as tt:
+            if args.merge:
+                tt.set_option(tnb.OPT_MERGE, 1)
             return step(tt)
     e2e_ms = None
     if not args.no_e2e:
@@ -402,7 +407,7 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "l2": "flushed (256 MiB fill) between timed steps",
             "config": {"workload": workload_name(args.config, inst, run, beta), "D": D, "M": M, "sweeps": sweeps,
-                       "beta": beta, "parallelism": "replicas x%d" % world, "l2": "flush between steps"},
+                       "beta": beta, "merge": bool(args.merge), "parallelism": "replicas x%d" % world, "l2": "flush between steps"},
             "contract_rows_per_s": round(st["rows_contracted"] / max(st["ms_contract"], 1e-9) * 1e3, 3),
             "contract_ms": round(st["ms_contract"], 3), "search_ms": round(st["ms_search"], 3),
             "best_energy": float(E.min()), "n_states": int(len(E)), "log_p_discarded": float(pd),

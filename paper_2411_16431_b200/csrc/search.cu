@@ -566,34 +566,66 @@ __global__ void k_merge_score(SelArgs a, const Raw* raw, unsigned n, unsigned np
   g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
   out[t] = MCand{g, logp[q.m] + log(u / Z[q.m]), q.m, state};
 }
-__global__ void k_mbitonic_step(MCand* c, unsigned n, unsigned k, unsigned j) {
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  unsigned l = i ^ j;
-  if (l > i) {
-    MCand x = c[i], y = c[l];
-    bool up = (i & k) == 0;
-    if (up ? mcand_before(y, x) : mcand_before(x, y)) { c[i] = y; c[l] = x; }
-  }
-}
-__global__ void __launch_bounds__(1024) k_mbitonic_smem(MCand* c, unsigned n) {
-  extern __shared__ MCand smc[];
-  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) smc[i] = c[i];
+// Bitonic sort of n = 2^p elements with shared-memory tiles of TILE elements: one launch sorts every tile up to
+// k = TILE (direction from the GLOBAL index), then each k > TILE costs one global launch per j >= TILE and one
+// launch that finishes j < TILE inside the tiles: 6 launches for 32768 elements instead of 120.
+struct LessM { __device__ bool operator()(const MCand& x, const MCand& y) const { return mcand_before(x, y); } };
+struct LessC { __device__ bool operator()(const Cand& x, const Cand& y) const { return cand_before(x, y); } };
+template <class T, class Less, int TILE>
+__global__ void __launch_bounds__(1024) k_bitonic_tile(T* c, unsigned n, unsigned kfirst, unsigned klast) {
+  extern __shared__ unsigned char tile_raw[];
+  T* sm = reinterpret_cast<T*>(tile_raw);
+  const unsigned base = blockIdx.x * TILE, cnt = min((unsigned)TILE, n - base);
+  Less less;
+  for (unsigned i = threadIdx.x; i < cnt; i += blockDim.x) sm[i] = c[base + i];
   __syncthreads();
-  for (unsigned k = 2; k <= n; k <<= 1)
-    for (unsigned j = k >> 1; j > 0; j >>= 1) {
-      for (unsigned i = threadIdx.x; i < n; i += blockDim.x) {
+  for (unsigned k = kfirst; k <= klast; k <<= 1)
+    for (unsigned j = min(k >> 1, (unsigned)TILE >> 1); j > 0; j >>= 1) {
+      for (unsigned i = threadIdx.x; i < cnt; i += blockDim.x) {
         unsigned l = i ^ j;
         if (l > i) {
-          MCand x = smc[i], y = smc[l];
-          bool up = (i & k) == 0;
-          if (up ? mcand_before(y, x) : mcand_before(x, y)) { smc[i] = y; smc[l] = x; }
+          T x = sm[i], y = sm[l];
+          bool up = ((base + i) & k) == 0;
+          if (up ? less(y, x) : less(x, y)) { sm[i] = y; sm[l] = x; }
         }
       }
       __syncthreads();
     }
-  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) c[i] = smc[i];
+  for (unsigned i = threadIdx.x; i < cnt; i += blockDim.x) c[base + i] = sm[i];
 }
+template <class T, class Less>
+__global__ void k_bitonic_gstep(T* c, unsigned n, unsigned k, unsigned j) {
+  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  unsigned l = i ^ j;
+  if (l > i) {
+    Less less;
+    T x = c[i], y = c[l];
+    bool up = (i & k) == 0;
+    if (up ? less(y, x) : less(x, y)) { c[i] = y; c[l] = x; }
+  }
+}
+template <class T, class Less>
+static void bitonic_sort(tn_handle* h, T* c, unsigned n) {   // n a power of two
+  constexpr int TILE = 4096;
+  static bool attr = false;
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_bitonic_tile<T, Less, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE * (int)sizeof(T)));
+    attr = true;
+  }
+  const unsigned tiles = (n + TILE - 1) / TILE;
+  k_bitonic_tile<T, Less, TILE><<<tiles, 1024, std::min<unsigned>(n, TILE) * sizeof(T), h->stream>>>(c, n, 2, std::min<unsigned>(n, TILE));
+  TN_LAUNCH_CHECK(h);
+  for (unsigned k = 2 * TILE; k <= n; k <<= 1) {
+    for (unsigned j = k >> 1; j >= (unsigned)TILE; j >>= 1) {
+      k_bitonic_gstep<T, Less><<<cdiv(n, 256), 256, 0, h->stream>>>(c, n, k, j);
+      TN_LAUNCH_CHECK(h);
+    }
+    k_bitonic_tile<T, Less, TILE><<<tiles, 1024, TILE * sizeof(T), h->stream>>>(c, n, k, k);
+    TN_LAUNCH_CHECK(h);
+  }
+}
+
 // first (= most probable, S8 order) member of every group of the sorted list
 __global__ void k_merge_first(const MCand* c, unsigned n, Cand* out, unsigned* count) {
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -749,7 +781,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
   TN_CUDA(cudaMemsetAsync(st_cur, 0, sizeof(unsigned) * ncell, h->stream));
   static bool attr = false;
-  if (!attr) { TN_CUDA(cudaFuncSetAttribute(k_bitonic_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * (int)sizeof(Cand))); attr = true; }
+  if (!attr) {
+    TN_CUDA(cudaFuncSetAttribute(k_bitonic_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * (int)sizeof(Cand)));
+    attr = true;
+  }
 
   for (int y = 0; y < Ly; y++) {
     const std::vector<MpsTensor>& R = h->rows[y + 1];
@@ -959,16 +994,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           while (mp2 < n1 + 1) mp2 <<= 1;
           k_merge_score<<<cdiv(mp2, 256), 256, 0, h->stream>>>(sa, craw.p, n1, mp2, lp_cur, Z.p, ns, S, pid.p, lg, mcand.p);
           TN_LAUNCH_CHECK(h);
-          if (mp2 <= 2048) {
-            k_mbitonic_smem<<<1, 1024, mp2 * sizeof(MCand), h->stream>>>(mcand.p, mp2);
-            TN_LAUNCH_CHECK(h);
-          } else {
-            for (unsigned k = 2; k <= mp2; k <<= 1)
-              for (unsigned j = k >> 1; j > 0; j >>= 1) {
-                k_mbitonic_step<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, k, j);
-                TN_LAUNCH_CHECK(h);
-              }
-          }
+          bitonic_sort<MCand, LessM>(h, mcand.p, mp2);
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
           k_merge_first<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, mcands.p, count.p);
           TN_LAUNCH_CHECK(h);
@@ -983,16 +1009,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           while (np2 <= (unsigned)M) np2 <<= 1;
           k_fill_sentinel<<<cdiv(np2 - ng, 256), 256, 0, h->stream>>>(mcands.p, ng, np2);
           TN_LAUNCH_CHECK(h);
-          if (np2 <= 4096) {
-            k_bitonic_smem<<<1, 1024, np2 * sizeof(Cand), h->stream>>>(mcands.p, np2);
-            TN_LAUNCH_CHECK(h);
-          } else {
-            for (unsigned k = 2; k <= np2; k <<= 1)
-              for (unsigned j = k >> 1; j > 0; j >>= 1) {
-                k_bitonic_step<<<cdiv(np2, 256), 256, 0, h->stream>>>(mcands.p, np2, k, j);
-                TN_LAUNCH_CHECK(h);
-              }
-          }
+          bitonic_sort<Cand, LessC>(h, mcands.p, np2);
           ncand = ng;
           cand_sorted = true;
         } else {
