@@ -245,11 +245,11 @@ def measured_peaks():
 STAGES = [  # (stats ms key, label, kernel, flop key, bytes key, bound)
     ("ms_theta_apply", "theta_apply", "k_tsgemm<NT,8,N|T> (Theta-core x skinny: zipper SVD / variational / env applies)",
      "flop_theta_apply", "bytes_theta_apply", "tensor"),
-    ("ms_theta_build", "theta_build", "k_bgemm<.., ArTh, LdThE, EpTh> (Theta-core build) + projector maps", "flop_theta_build",
+    ("ms_theta_build", "theta_build", "k_bgemm_pipe<.., ArTh, BrTh, EpTh> (Theta-core build) + projector maps", "flop_theta_build",
      None, "tensor"),
-    ("ms_orth_svd", "orth_svd", "k_orth_pass (Cholesky-QR rounds) + k_jacobi_rows (Rayleigh-Ritz)", None, None, "alu"),
-    ("ms_search_rblocks", "search_rblocks", "k_gemm<LdHA,LdHB> + k_rs (right blocks)", None, None, "tensor"),
-    ("ms_search_cond", "search_cond", "k_bgemm<.., ArPV, LdPB, EpPV> + k_beam_Z (conditionals)", None, None, "tensor"),
+    ("ms_orth_svd", "orth_svd", "k_orth_coop (Cholesky-QR rounds, one cooperative launch) + k_jacobi_rows (Rayleigh-Ritz)", None, None, "alu"),
+    ("ms_search_rblocks", "search_rblocks", "k_gather_G, k_coef + k_tsgemm + k_rs (right blocks)", None, None, "tensor"),
+    ("ms_search_cond", "search_cond", "k_bgemm<.., ArPV, LdPB, EpPV> (conditionals, Z fused in the epilogue)", None, None, "tensor"),
     ("ms_search_select", "search_select", "k_sel_hist (sample) + k_sel_prefilter + k_csel_* + bitonic (top-M)", None, None,
      "hbm"),
     ("ms_tables", "tables", "k_tables", None, None, "hbm"),

@@ -843,13 +843,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         k_rs<<<cdiv(total, 256), 256, 0, h->stream>>>(c, H.p, rt[x].RM, nb, Dl, Dr, RS.p);
         TN_LAUNCH_CHECK(h);
       }
-      GemmDesc g;
-      g.B1 = nb; g.M = Dl; g.N = c.bh_rows; g.K = c.nA;
-      g.A = RS.p; g.a_b1 = (i64)Dl * c.nA; g.a_i = c.nA; g.a_k = 1;
-      g.B = c.BhS; g.b_k = 1; g.b_j = c.nA;
-      g.C = rt[x - 1].RM; g.c_b1 = (i64)Dl * c.bh_rows; g.c_i = c.bh_rows; g.c_j = 1;
-      g.nsplit = 1;
-      gemm_general(h, g);
+      // RM_{x-1}[(m, b'), r] = sum_a RS[(m, b'), a] BhS[r, a]: the beam stacks along the rows -> one GEMM
+      gemm_rm(h, false, true, nb * Dl, c.bh_rows, c.nA, RS.p, c.nA, c.BhS, c.nA, rt[x - 1].RM, c.bh_rows);
       k_norm_rm<<<nb, 256, 0, h->stream>>>(rt[x - 1].RM, Dl * c.bh_rows, rt[x].ls, rt[x - 1].ls);
       TN_LAUNCH_CHECK(h);
     }

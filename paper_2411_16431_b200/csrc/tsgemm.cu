@@ -196,7 +196,7 @@ void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb
   const int smax = (int)std::max<i64>(1, std::min<i64>(64, Kred / 128));
   for (int sp = 1; sp <= smax; sp++) {
     const i64 waves = (tiles * sp + slots - 1) / slots;
-    const double t = waves * ((double)((Kred + sp - 1) / sp) + 96.0) * t_k + (sp > 1 ? sp * t_ws + 3e-6 : 0.0);
+    const double t = waves * ((double)((Kred + sp - 1) / sp) + 96.0) * t_k + (sp > 1 ? sp * t_ws + 6e-6 : 0.0);
     if (t < best_t) { best_t = t; best = sp; }
   }
   if (warps == 8) launch_ts<NT, 8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);
