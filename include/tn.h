@@ -94,6 +94,8 @@ typedef struct {
   double flop_theta_apply;   /* algorithmic FLOP of the skinny GEMMs                        */
   double bytes_theta_apply;  /* algorithmic bytes of the skinny GEMMs (one read of Theta)    */
   double flop_search;        /* algorithmic FLOP of the search GEMMs                        */
+  double bytes_search_cond;  /* algorithmic bytes of the conditionals: one write of V (8 M n_b n_cl n_a per cell)  */
+  double bytes_search_select;/* algorithmic bytes of the top-M selection: one read of V per prefilter pass + the 1/64 sample passes */
   double min_sigma_rel;      /* max over the truncated bonds of (smallest retained sigma / sigma_1):
                                 the worst cut of Fig. 12(b); 0 if nothing was cut */
   int64_t svd_iterations;    /* total block-subspace iterations                             */

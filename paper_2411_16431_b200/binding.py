@@ -25,7 +25,7 @@ class TnStats(C.Structure):
     _fields_ = [(n, C.c_double) for n in (
         "ms_tables", "ms_contract", "ms_theta_build", "ms_theta_apply", "ms_orth_svd", "ms_search",
         "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
-        "bytes_theta_apply", "flop_search", "min_sigma_rel")] + [(n, C.c_int64) for n in (
+        "bytes_theta_apply", "flop_search", "bytes_search_cond", "bytes_search_select", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
             "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged")]
 

@@ -874,6 +874,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       {   // V[m][(b,cl)][a]
         int Mg = c.nB * c.nCl, Ng = c.nA;
         h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
+        h->st.bytes_search_cond += 8.0 * nb * (double)per_m;
         DBuf<double> cs(h, (size_t)nb * c.nA);
         k_colscale<<<cdiv((i64)nb * c.nA, 256), 256, 0, h->stream>>>(c.BhS, c.wA, hrow.p, nb, c.nA, cs.p);
         TN_LAUNCH_CHECK(h);
@@ -981,6 +982,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         for (int attempt = 0; attempt < 4; attempt++) {
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
           k_sel_prefilter_merge<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, thr, fmx.p, craw.p, count.p, mcap);
+          h->st.bytes_search_select += 8.0 * nb * (double)per_m * (attempt == 0 && !direct ? 1.0 + 2.0 / 64.0 : 1.0);
           TN_LAUNCH_CHECK(h);
           n1 = d2h(h, count.p);
           if (n1 > mcap) break;                          // too many survivors for the merge buffers: unmerged route
@@ -1031,6 +1033,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           while ((1 << lgA) < c.nA) lgA++;
           const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
           k_sel_prefilter<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap);
+          h->st.bytes_search_select += 8.0 * nb * (double)per_m * (1.0 + 2.0 / 64.0);
         }
         TN_LAUNCH_CHECK(h);
         const unsigned n1 = d2h(h, count.p);
