@@ -53,47 +53,45 @@ __device__ bool orth_factor(double* sG, double* sX, double* s_red, int k, double
   md = block_max256(md, s_red);
   if (dev <= tol) return true;
   const double floor_ = frel * md;
-  // ---- Cholesky G = L L^T (lower triangle of sG, in place).  A pivot at or below the floor (rounding noise of
-  // the Gram matrix, c * eps * md) is replaced by the floor and its sub-column is dropped: noise directions
-  // are scaled up by a bounded factor and are NOT used to "orthogonalise" later columns -- dividing noise by
-  // noise gives O(1) multipliers and an exponentially ill-conditioned L.  The next round sees them at a
-  // resolvable size.
+  // ---- Cholesky G = L L^T fused with the triangular inverse X = L^-1, two barriers per column.
+  // Column j of L is G'_ij / L_jj below the diagonal; the diagonal entry of sG keeps the updated pivot G'_jj (so
+  // no thread overwrites what another still reads and L_jj = sqrt(max(G'_jj, floor)) is recomputed where needed).
+  // X is kept with UNSCALED rows: row j of L^-1 is sX[j][:] / L_jj.
+  // A pivot at or below the floor (rounding noise of the Gram matrix, c * eps * md) is replaced by the floor and
+  // its sub-column is dropped: noise directions are scaled up by a bounded factor and are NOT used to
+  // "orthogonalise" later columns -- dividing noise by noise gives O(1) multipliers and an exponentially
+  // ill-conditioned L.  The next round sees them at a resolvable size.
+  for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
   for (int j = 0; j < k; j++) {
-    __syncthreads();
+    __syncthreads();                                   // updates of step j - 1 (and the X initialisation) are complete
     double d = sG[j * LG + j];
     const bool floored = !(d > floor_);
     if (floored) d = floor_;
-    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;
-    __syncthreads();
-    for (int i = j + tid; i < k; i += OR_THREADS)
-      sG[i * LG + j] = (i == j) ? d * inv : (floored ? 0.0 : sG[i * LG + j] * inv);
+    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;  // 1 / L_jj
+    for (int i = j + 1 + tid; i < k; i += OR_THREADS) sG[i * LG + j] = floored ? 0.0 : sG[i * LG + j] * inv;
     __syncthreads();
     if (floored) continue;
-    const int n = k - j - 1;
-    for (int idx = tid; idx < n * n; idx += OR_THREADS) {
+    const int n = k - j - 1, w = j + 1;
+    for (int idx = tid; idx < n * n; idx += OR_THREADS) {      // trailing update of G (lower triangle)
       int i = j + 1 + idx / n, c = j + 1 + idx % n;
       if (c <= i) sG[i * LG + c] -= sG[i * LG + j] * sG[c * LG + j];
     }
-  }
-  // ---- X = L^-1 (lower triangular) by a column sweep of rank-1 updates
-  for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
-  for (int p = 0; p < k; p++) {
-    __syncthreads();
-    const double lp = sG[p * LG + p];
-    const double ip = lp > 0.0 ? 1.0 / lp : 0.0;
-    for (int c = tid; c <= p; c += OR_THREADS) sX[p * LG + c] *= ip;
-    __syncthreads();
-    const int n = k - p - 1, w = p + 1;
-    for (int idx = tid; idx < n * w; idx += OR_THREADS) {
-      int i = p + 1 + idx / w, c = idx % w;
-      sX[i * LG + c] -= sG[i * LG + p] * sX[p * LG + c];
+    for (int idx = tid; idx < n * w; idx += OR_THREADS) {      // rank-1 update of the inverse with row j / L_jj
+      int i = j + 1 + idx / w, c = idx % w;
+      sX[i * LG + c] -= sG[i * LG + j] * (sX[j * LG + c] * inv);
     }
   }
   __syncthreads();
   // T = L^-T (upper triangular), zero-padded to KP x KP
   for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
     int c = idx / KP, j = idx % KP;
-    Tout[idx] = (c <= j && j < k) ? sX[j * LG + c] : 0.0;
+    double v = 0.0;
+    if (c <= j && j < k) {
+      double d = sG[j * LG + j];
+      if (!(d > floor_)) d = floor_;
+      v = d > 0.0 ? sX[j * LG + c] / sqrt(d) : 0.0;
+    }
+    Tout[idx] = v;
   }
   return false;
 }
