@@ -333,7 +333,8 @@ void jacobi_rows(tn_handle* h, const double* Min, int ld, int c, int r, double* 
     TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
   }
   if (need <= 200 * 1024) {
-    k_jacobi_rows<<<1, 1024, need, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, nullptr, 1, h->d_cnt);
+    const int jt = std::min(1024, std::max(128, 32 * ((c + 1) / 2)));   // one warp per pair: fewer warps, cheaper barriers
+    k_jacobi_rows<<<1, jt, need, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, nullptr, 1, h->d_cnt);
     TN_LAUNCH_CHECK(h);
   } else {
     double* work = h->dalloc<double>((size_t)c * r + (size_t)c * c);

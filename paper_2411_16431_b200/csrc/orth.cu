@@ -37,9 +37,10 @@ __device__ __forceinline__ double block_max256(double v, double* sh) {
 
 // Last stage of a round, run by ONE CTA on the reduced Gram matrix in shared memory (sG [k x k], ld KP + 1):
 // test ||G - I||, pivot-floored Cholesky, triangular inverse, T = L^-T to global memory (zero-padded KP x KP).
-// Returns true (to all threads) when Y is already orthonormal to rounding.
+// Returns (to all threads) 1 when Y is already orthonormal to rounding (no T written), 2 when ||G - I|| <= 1e-4
+// (applying this T gives an orthonormal block to rounding, u * cond(G): no further round is needed), else 0.
 template <int KP>
-__device__ bool orth_factor(double* sG, double* sX, double* s_red, int k, double tol, double frel, double* Tout) {
+__device__ int orth_factor(double* sG, double* sX, double* s_red, int k, double tol, double frel, double* Tout) {
   constexpr int LG = KP + 1;
   const int tid = threadIdx.x;
   double dev = 0.0, md = 0.0;
@@ -51,7 +52,7 @@ __device__ bool orth_factor(double* sG, double* sX, double* s_red, int k, double
   }
   dev = block_max256(dev, s_red);
   md = block_max256(md, s_red);
-  if (dev <= tol) return true;
+  if (dev <= tol) return 1;
   const double floor_ = frel * md;
   // ---- Cholesky G = L L^T fused with the triangular inverse X = L^-1, two barriers per column.
   // Column j of L is G'_ij / L_jj below the diagonal; the diagonal entry of sG keeps the updated pivot G'_jj (so
@@ -93,7 +94,7 @@ __device__ bool orth_factor(double* sG, double* sX, double* s_red, int k, double
     }
     Tout[idx] = v;
   }
-  return false;
+  return dev <= 1e-4 ? 2 : 0;
 }
 
 template <int KT>
@@ -214,8 +215,8 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y
     sG[(idx / KP) * LG + idx % KP] = s;
   }
   __syncthreads();
-  const bool ortho = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
-  if (tid == 0) { ctl->top = 0; ctl->rounds++; if (ortho) ctl->done = 1; }
+  const int verdict = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
+  if (tid == 0) { ctl->top = 0; ctl->rounds++; if (verdict == 1) ctl->done = 1; }
   if (tid < OR_MAXG) ctl->grp[tid] = 0;
 }
 
@@ -237,8 +238,9 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_coop(double* __restrict__ Y
   const int nb = gridDim.x, ngrp = (nb + OR_GS - 1) / OR_GS;
   double* gpart = part + (size_t)nb * KP * KP;
   const i64 ntile = (m + OR_ROWS - 1) / OR_ROWS;
+  bool last = false;   // set when the previous round reported ||G - I|| <= 1e-4: apply its T and stop
   for (int p = 0; p <= passes; p++) {
-    const bool has_T = p > 0, do_gram = p < passes;
+    const bool has_T = p > 0, do_gram = p < passes && !last;
     const double* Tin = Tbuf + (size_t)((p - 1) & 1) * KP * KP;
     double* Tout = Tbuf + (size_t)(p & 1) * KP * KP;
     __syncthreads();
@@ -314,32 +316,39 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_coop(double* __restrict__ Y
       }
     }
     grid.sync();
-    if ((int)blockIdx.x < ngrp) {          // level 1: CTA g reduces group g in CTA order
-      const int g0 = blockIdx.x * OR_GS, g1 = min(nb, g0 + OR_GS);
-      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
-        double s = 0.0;
+    const bool two_level = nb > 4 * OR_GS;   // small grids: CTA 0 adds the partials itself (one barrier less per round)
+    if (two_level) {
+      if ((int)blockIdx.x < ngrp) {        // level 1: CTA g reduces group g in CTA order
+        const int g0 = blockIdx.x * OR_GS, g1 = min(nb, g0 + OR_GS);
+        for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
+          double s = 0.0;
 #pragma unroll 4
-        for (int b = g0; b < g1; b++) s += __ldcg(part + (size_t)b * KP * KP + idx);
-        gpart[(size_t)blockIdx.x * KP * KP + idx] = s;
+          for (int b = g0; b < g1; b++) s += __ldcg(part + (size_t)b * KP * KP + idx);
+          gpart[(size_t)blockIdx.x * KP * KP + idx] = s;
+        }
       }
+      grid.sync();
     }
-    grid.sync();
-    if (blockIdx.x == 0) {                 // level 2 + factorisation
+    if (blockIdx.x == 0) {                 // level 2 (or the only level) + factorisation
       double* sG = sm;
       double* sX = sm + KP * LG;
+      const double* src = two_level ? gpart : part;
+      const int nsrc = two_level ? ngrp : nb;
       __syncthreads();
       for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
         double s = 0.0;
 #pragma unroll 4
-        for (int b = 0; b < ngrp; b++) s += __ldcg(gpart + (size_t)b * KP * KP + idx);
+        for (int b = 0; b < nsrc; b++) s += __ldcg(src + (size_t)b * KP * KP + idx);
         sG[(idx / KP) * LG + idx % KP] = s;
       }
       __syncthreads();
-      const bool ortho = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
-      if (tid == 0) { ctl->rounds++; if (ortho) ctl->done = 1; }
+      const int verdict = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
+      if (tid == 0) { ctl->rounds++; if (verdict) ctl->done = verdict; }
     }
     grid.sync();
-    if (*(volatile int*)&ctl->done) break;
+    const int verdict = *(volatile int*)&ctl->done;
+    if (verdict == 1) break;
+    last = verdict == 2;
   }
 }
 
