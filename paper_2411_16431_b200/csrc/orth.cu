@@ -21,6 +21,13 @@ constexpr int OR_ROWS = 64, OR_THREADS = 256;
 constexpr int OR_GS = 12, OR_MAXG = 16;   // two-level ordered reduction: groups of OR_GS CTAs
 struct OrthCtl { unsigned top; int done; int rounds; int pad; unsigned grp[OR_MAXG]; };
 
+__device__ __forceinline__ double rsqrt_newton(double x) {   // MUFU seed + two Newton steps: full precision, no IEEE sqrt / div
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double hx = 0.5 * x;
+  y = y * (1.5 - hx * y * y);
+  return y * (1.5 - hx * y * y);
+}
 __device__ __forceinline__ double block_max256(double v, double* sh) {
   const int tid = threadIdx.x;
   __syncthreads();
@@ -63,23 +70,55 @@ __device__ int orth_factor(double* sG, double* sX, double* s_red, int k, double 
   // "orthogonalise" later columns -- dividing noise by noise gives O(1) multipliers and an exponentially
   // ill-conditioned L.  The next round sees them at a resolvable size.
   for (int idx = tid; idx < k * k; idx += OR_THREADS) sX[(idx / k) * LG + idx % k] = (idx / k == idx % k) ? 1.0 : 0.0;
+  // thread (ty, tx) = (tid / 32, tid % 32) walks rows ty, ty + 8, ... and columns tx, tx + 32, ...: no divisions
+  const int tx = tid & 31, ty = tid >> 5;
   for (int j = 0; j < k; j++) {
     __syncthreads();                                   // updates of step j - 1 (and the X initialisation) are complete
     double d = sG[j * LG + j];
     const bool floored = !(d > floor_);
     if (floored) d = floor_;
-    const double inv = d > 0.0 ? 1.0 / sqrt(d) : 0.0;  // 1 / L_jj
+    // 1 / L_jj; pivots below 1e-290 (only possible when the whole block is that small) take the exact route
+    const double inv = d > 1e-290 ? rsqrt_newton(d) : (d > 0.0 ? 1.0 / sqrt(d) : 0.0);
     for (int i = j + 1 + tid; i < k; i += OR_THREADS) sG[i * LG + j] = floored ? 0.0 : sG[i * LG + j] * inv;
     __syncthreads();
     if (floored) continue;
-    const int n = k - j - 1, w = j + 1;
-    for (int idx = tid; idx < n * n; idx += OR_THREADS) {      // trailing update of G (lower triangle)
-      int i = j + 1 + idx / n, c = j + 1 + idx % n;
-      if (c <= i) sG[i * LG + c] -= sG[i * LG + j] * sG[c * LG + j];
-    }
-    for (int idx = tid; idx < n * w; idx += OR_THREADS) {      // rank-1 update of the inverse with row j / L_jj
-      int i = j + 1 + idx / w, c = idx % w;
-      sX[i * LG + c] -= sG[i * LG + j] * (sX[j * LG + c] * inv);
+    if constexpr (KP <= 48) {
+      // all operands of this column's updates are read into registers first, then written: no load waits on a store
+      constexpr int NR = KP / 8, NC = (KP + 31) / 32;
+      double li[NR], lc[NC], xj[NC], gv[NR][NC], xv[NR][NC];
+  #pragma unroll
+      for (int a = 0; a < NR; a++) {
+        const int i = j + 1 + ty + 8 * a;
+        li[a] = i < k ? sG[i * LG + j] : 0.0;
+      }
+  #pragma unroll
+      for (int b = 0; b < NC; b++) {
+        const int c = j + 1 + tx + 32 * b, c2 = tx + 32 * b;
+        lc[b] = c < k ? sG[c * LG + j] : 0.0;
+        xj[b] = c2 <= j ? sX[j * LG + c2] * inv : 0.0;
+      }
+  #pragma unroll
+      for (int a = 0; a < NR; a++)
+  #pragma unroll
+        for (int b = 0; b < NC; b++) {
+          const int i = j + 1 + ty + 8 * a, c = j + 1 + tx + 32 * b, c2 = tx + 32 * b;
+          gv[a][b] = (i < k && c <= i) ? sG[i * LG + c] : 0.0;
+          xv[a][b] = (i < k && c2 <= j) ? sX[i * LG + c2] : 0.0;
+        }
+  #pragma unroll
+      for (int a = 0; a < NR; a++)
+  #pragma unroll
+        for (int b = 0; b < NC; b++) {
+          const int i = j + 1 + ty + 8 * a, c = j + 1 + tx + 32 * b, c2 = tx + 32 * b;
+          if (i < k && c <= i) sG[i * LG + c] = gv[a][b] - li[a] * lc[b];       // trailing update of G
+          if (i < k && c2 <= j) sX[i * LG + c2] = xv[a][b] - li[a] * xj[b];     // rank-1 update of L^-1
+        }
+    } else {   // larger blocks: the fully unrolled, predicated form above is issue-bound; walk the valid ranges only
+      for (int i = j + 1 + ty; i < k; i += OR_THREADS / 32) {
+        const double lij = sG[i * LG + j];
+        for (int c = j + 1 + tx; c <= i; c += 32) sG[i * LG + c] -= lij * sG[c * LG + j];        // trailing update of G
+        for (int c = tx; c <= j; c += 32) sX[i * LG + c] -= lij * (sX[j * LG + c] * inv);         // rank-1 update of L^-1
+      }
     }
   }
   __syncthreads();
@@ -90,7 +129,7 @@ __device__ int orth_factor(double* sG, double* sX, double* s_red, int k, double 
     if (c <= j && j < k) {
       double d = sG[j * LG + j];
       if (!(d > floor_)) d = floor_;
-      v = d > 0.0 ? sX[j * LG + c] / sqrt(d) : 0.0;
+      v = d > 1e-290 ? sX[j * LG + c] * rsqrt_newton(d) : (d > 0.0 ? sX[j * LG + c] / sqrt(d) : 0.0);
     }
     Tout[idx] = v;
   }
@@ -222,7 +261,7 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_pass(double* __restrict__ Y
 
 // All rounds of one orthonormalisation in ONE cooperative launch (grid <= resident CTAs): the rounds are separated
 // by grid-wide barriers instead of kernel boundaries, which removes ~5 launches and their gaps from every call.
-// Same arithmetic and the same reduction order as k_orth_pass (bit-identical results).
+// Same arithmetic as k_orth_pass; the Gram partials are added in a different (also fixed) association.
 template <int KT>
 __global__ void __launch_bounds__(OR_THREADS) k_orth_coop(double* __restrict__ Y, i64 m, int k, double* __restrict__ Tbuf,
                                                           double* __restrict__ part, OrthCtl* ctl, int passes, double tol,
@@ -316,31 +355,35 @@ __global__ void __launch_bounds__(OR_THREADS) k_orth_coop(double* __restrict__ Y
       }
     }
     grid.sync();
-    const bool two_level = nb > 4 * OR_GS;   // small grids: CTA 0 adds the partials itself (one barrier less per round)
-    if (two_level) {
-      if ((int)blockIdx.x < ngrp) {        // level 1: CTA g reduces group g in CTA order
-        const int g0 = blockIdx.x * OR_GS, g1 = min(nb, g0 + OR_GS);
-        for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
-          double s = 0.0;
-#pragma unroll 4
-          for (int b = g0; b < g1; b++) s += __ldcg(part + (size_t)b * KP * KP + idx);
-          gpart[(size_t)blockIdx.x * KP * KP + idx] = s;
-        }
+    {   // every CTA reduces its slice of the KP x KP entries over all partials: thread (e, q) adds partials
+        // 8q .. 8q+7 (eight loads in flight), thread e then adds the group sums in order -- fixed association
+      const int E = KP * KP, e0 = (int)((i64)E * blockIdx.x / nb), e1 = (int)((i64)E * (blockIdx.x + 1) / nb);
+      const int EL = e1 - e0, nq = (nb + 7) / 8;
+      double* s_ps = sm;                               // EL * nq <= KP * KP <= the dynamic shared memory of this kernel
+      __syncthreads();
+      for (int w = tid; w < EL * nq; w += OR_THREADS) {
+        const int e = w % EL, q = w / EL;
+        double v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) v[u] = 8 * q + u < nb ? __ldcg(part + (size_t)(8 * q + u) * E + e0 + e) : 0.0;
+        double ssum = 0.0;
+#pragma unroll
+        for (int u = 0; u < 8; u++) ssum += v[u];
+        s_ps[q * EL + e] = ssum;
       }
-      grid.sync();
+      __syncthreads();
+      for (int e = tid; e < EL; e += OR_THREADS) {
+        double ssum = 0.0;
+        for (int q = 0; q < nq; q++) ssum += s_ps[q * EL + e];
+        gpart[e0 + e] = ssum;
+      }
     }
-    if (blockIdx.x == 0) {                 // level 2 (or the only level) + factorisation
+    grid.sync();
+    if (blockIdx.x == 0) {                 // factorisation of the reduced Gram matrix
       double* sG = sm;
       double* sX = sm + KP * LG;
-      const double* src = two_level ? gpart : part;
-      const int nsrc = two_level ? ngrp : nb;
       __syncthreads();
-      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) {
-        double s = 0.0;
-#pragma unroll 4
-        for (int b = 0; b < nsrc; b++) s += __ldcg(src + (size_t)b * KP * KP + idx);
-        sG[(idx / KP) * LG + idx % KP] = s;
-      }
+      for (int idx = tid; idx < KP * KP; idx += OR_THREADS) sG[(idx / KP) * LG + idx % KP] = __ldcg(gpart + idx);
       __syncthreads();
       const int verdict = orth_factor<KP>(sG, sX, s_red, k, tol, frel, Tout);
       if (tid == 0) { ctl->rounds++; if (verdict) ctl->done = verdict; }
