@@ -217,6 +217,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
                                                       unsigned long long* cnt) {
   extern __shared__ double sm[];
   __shared__ int s_rot;
+  __shared__ unsigned long long s_maxrel;
   __shared__ double s_norm[1024];   // c <= 1024
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   double* Mw = use_smem ? sm : gwork;
@@ -243,19 +244,24 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
   __syncthreads();
   if (c > 1) {
     for (int sweep = 0; sweep < 60; sweep++) {
-      if (tid == 0) s_rot = 0;
+      if (tid == 0) { s_rot = 0; s_maxrel = 0ull; }
       __syncthreads();
       for (int step = 0; step < ce - 1; step++) {
         for (int pi = warp; pi < ce / 2; pi += nwarp) {
           int p, q;
           if (pi == 0) { p = ce - 1; q = step; }
-          else { p = (step + pi) % (ce - 1); q = (step - pi + (ce - 1)) % (ce - 1); }
+          else {
+            p = step + pi; if (p >= ce - 1) p -= ce - 1;
+            q = step - pi; if (q < 0) q += ce - 1;
+          }
           if (p >= c || q >= c) continue;
           if (p > q) { int t = p; p = q; q = t; }
           double* xp = Mw + (size_t)p * r;
           double* xq = Mw + (size_t)q * r;
           double a = 0, b = 0, g = 0;
-          for (int i = lane; i < r; i += 32) {
+          const double u0 = lane < r ? xp[lane] : 0.0, v0 = lane < r ? xq[lane] : 0.0;   // first 32 entries stay in registers
+          a = u0 * u0; b = v0 * v0; g = u0 * v0;
+          for (int i = lane + 32; i < r; i += 32) {
             double u = xp[i], v = xq[i];
             a += u * u; b += v * v; g += u * v;
           }
@@ -273,7 +279,11 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
             const double d = b - a, q2 = d * d + 4.0 * g * g;
             const double t = 2.0 * (d >= 0.0 ? g : -g) * rcp_fast(fabs(d) + q2 * rsqrt_fast(q2));
             const double cs = rsqrt_fast(1.0 + t * t), sn = cs * t;
-            for (int i = lane; i < r; i += 32) {
+            if (lane < r) {
+              xp[lane] = cs * u0 - sn * v0;
+              xq[lane] = sn * u0 + cs * v0;
+            }
+            for (int i = lane + 32; i < r; i += 32) {
               double u = xp[i], v = xq[i];
               xp[i] = cs * u - sn * v;
               xq[i] = sn * u + cs * v;
@@ -285,15 +295,22 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
               wp[i] = cs * u - sn * v;
               wq[i] = sn * u + cs * v;
             }
-            if (lane == 0) s_rot = 1;
+            if (lane == 0) {
+              s_rot = 1;
+              // largest squared relative off-diagonal g^2 / (a b) rotated in this sweep (positive doubles order like integers)
+              atomicMax(&s_maxrel, (unsigned long long)__double_as_longlong(g * g * rcp_fast(a * b)));
+            }
           }
         }
         __syncthreads();
       }
-      int rot = s_rot;
+      const int rot = s_rot;
+      const double maxrel2 = __longlong_as_double((long long)s_maxrel);
       __syncthreads();
       if (tid == 0 && cnt) cnt[1]++;
-      if (!rot) break;
+      // quadratic convergence: once every rotation of a sweep had |g| / sqrt(a b) < 1e-10 the next sweep would find
+      // nothing above 1e-15, so it is not run
+      if (!rot || maxrel2 < 1e-20) break;
     }
   }
   // norms, ranks (descending, ties by index), sorted outputs
