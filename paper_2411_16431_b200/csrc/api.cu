@@ -366,7 +366,7 @@ void tn_destroy(tn_handle* h) {
     mps_free(h);
     tables_destroy(h);
     for (void* p : {(void*)h->d_eu, (void*)h->d_ev, (void*)h->d_J, (void*)h->d_h, (void*)h->d_cell_of,
-                    (void*)h->d_bit_of, (void*)h->d_cnt, (void*)h->d_tile_cnt})
+                    (void*)h->d_bit_of, (void*)h->d_cnt})
       if (p) h->dfree(p);
     trim_free_list(h);
     for (auto& l : h->live) raw_free(h, l);

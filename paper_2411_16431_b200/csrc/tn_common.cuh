@@ -98,7 +98,6 @@ struct tn_handle {
   std::vector<Block> live, cached;
   tn_stats st;
   cudaEvent_t ev[2] = {nullptr, nullptr};
-  unsigned* d_tile_cnt = nullptr;        // tsgemm.cu: arrival counters of the fused split reduction (all zero between launches)
   unsigned long long* d_cnt = nullptr;   // device counters: [0] Jacobi calls, [1] Jacobi sweeps
 
   void* dmalloc(size_t bytes);

@@ -15,7 +15,6 @@
 namespace {
 
 constexpr int TS_BK = 16, TS_STAGES = 3;
-constexpr i64 TS_MAX_TILES = 1 << 16;   // output tiles with a self-resetting arrival counter (fused split reduction)
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -31,8 +30,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int NT, int WARPS, bool TRANS>
 __global__ void __launch_bounds__(WARPS * 32, (NT <= 10 || WARPS < 8) ? 2 : 1)
 k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i64 ldb, double* __restrict__ C, i64 ldc,
-         i64 Mout, int Nfull, i64 Kred, i64 kper, double* __restrict__ ws, int nz, i64 sBz, i64 sCz,
-         unsigned* __restrict__ tile_cnt) {
+         i64 Mout, int Nfull, i64 Kred, i64 kper, double* __restrict__ ws, int nz, i64 sBz, i64 sCz) {
   constexpr int BM = 16 * WARPS, NTH = 32 * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK);   // doubles
   constexpr int LDB = smem_ld(NP);
@@ -141,29 +139,6 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
       }
     }
   }
-  if (nsplit > 1 && tile_cnt) {
-    // fused split reduction: the last CTA of this output tile to arrive adds the nsplit partial tiles in split
-    // order (deterministic) and writes C; the counter resets itself for the next launch
-    __shared__ int s_last;
-    __threadfence();
-    __syncthreads();
-    const unsigned tile = blockIdx.x + gridDim.x * blockIdx.z;
-    if (tid == 0) s_last = atomicAdd(&tile_cnt[tile], 1u) == (unsigned)nsplit - 1;
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    if (tid == 0) tile_cnt[tile] = 0;
-    const double* w0 = ws + (size_t)bz * nsplit * Mout * Nfull + n_off;
-    double* cb = C + (i64)bz * sCz + n_off;
-    const int rows = (int)min((i64)BM, Mout - m0);
-    for (int idx = tid; idx < rows * N; idx += NTH) {
-      const i64 row = m0 + idx / N;
-      const int col = idx % N;
-      double sum = 0.0;
-      for (int sp = 0; sp < nsplit; sp++) sum += __ldcg(w0 + (size_t)sp * Mout * Nfull + row * Nfull + col);
-      cb[row * ldc + col] = sum;
-    }
-  }
 }
 
 // C[i][j] = sum_s ws[s][i][j]  (fixed order)
@@ -195,20 +170,10 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
   const int nbz = tsb.n, nz = (N + NP - 1) / NP;
   double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nbz * nsplit * Mout * N) : nullptr;
   dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit, (unsigned)(nz * nbz));
-  unsigned* cnt = nullptr;
-  if (nsplit > 1 && (i64)grid.x * grid.z <= TS_MAX_TILES) {
-    if (!h->d_tile_cnt) {
-      h->d_tile_cnt = h->dalloc<unsigned>(TS_MAX_TILES);
-      TN_CUDA(cudaMemsetAsync(h->d_tile_cnt, 0, sizeof(unsigned) * TS_MAX_TILES, h->stream));
-    }
-    cnt = h->d_tile_cnt;
-  }
   k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws, nz,
-                                                                     tsb.sB, tsb.sC, cnt);
+                                                                     tsb.sB, tsb.sC);
   TN_LAUNCH_CHECK(h);
-  if (nsplit > 1 && cnt) {
-    h->dfree(ws);
-  } else if (nsplit > 1) {
+  if (nsplit > 1) {
     k_ts_reduce<<<dim3(cdiv(Mout * N, 256), nbz), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc, tsb.sC);
     TN_LAUNCH_CHECK(h);
     h->dfree(ws);
