@@ -410,7 +410,20 @@ __global__ void k_map_L_med(CellDev c, const double* Y, double* Yk, int outer, i
   Yk[t] = acc;
 }
 // Y[o][(l,i)][s] = sum_{a: Pl a = l} sum_cl sum_{ch: Pi ch = i} wC[cl][ch] Yk[o][(a,cl)][s]
-__global__ void k_map_LT_med(CellDev c, const double* Yk, double* Y, int outer, int s, int nbits, int half) {
+// W2[i][cl] = sum_{ch: Pi ch = i} wC[cl][ch] is built once per CTA in shared memory (n_i * nCl <= 256 entries), so
+// the inner loop is one FMA per (a, cl) with loads that are coalesced over s.
+__global__ void __launch_bounds__(256) k_map_LT_med(CellDev c, const double* Yk, double* Y, int outer, int s, int nbits,
+                                                    int half) {
+  __shared__ double W2[256];
+  const int fc_mask = (~c.m_din) & (c.nCh - 1), nfc = c.nCh / c.n_i;
+  for (int e = threadIdx.x; e < c.n_i * c.nCl; e += blockDim.x) {
+    const int i = e / c.nCl, cl = e % c.nCl;
+    const int c0 = pdep8(i, c.m_din);
+    double w = 0.0;
+    for (int fc = 0; fc < nfc; fc++) w += c.wC[cl * c.nCh + (c0 | pdep8(fc, fc_mask))];
+    W2[e] = w;
+  }
+  __syncthreads();
   i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   int wl = c.n_l * c.n_i;
   i64 total = (i64)outer * wl * s;
@@ -419,17 +432,15 @@ __global__ void k_map_LT_med(CellDev c, const double* Yk, double* Y, int outer, 
   int li = (int)((t / s) % wl);
   int o = (int)(t / ((i64)s * wl));
   int l = li / c.n_i, i = li % c.n_i;
-  int fa_mask = (~c.m_left) & (c.nA - 1), fc_mask = (~c.m_din) & (c.nCh - 1);
-  int nfa = c.nA / c.n_l, nfc = c.nCh / c.n_i;
-  int a0 = pdep8(l, c.m_left), c0 = pdep8(i, c.m_din);
+  int fa_mask = (~c.m_left) & (c.nA - 1);
+  int nfa = c.nA / c.n_l;
+  int a0 = pdep8(l, c.m_left);
+  const double* w2 = W2 + i * c.nCl;
   double acc = 0.0;
   for (int fa = 0; fa < nfa; fa++) {
-    int a = a0 | pdep8(fa, fa_mask);
-    for (int cl = 0; cl < c.nCl; cl++) {
-      double w = 0.0;
-      for (int fc = 0; fc < nfc; fc++) w += c.wC[cl * c.nCh + (c0 | pdep8(fc, fc_mask))];
-      acc += w * Yk[((i64)o * c.nK + (i64)a * c.nCl + cl) * s + is];
-    }
+    const int a = a0 | pdep8(fa, fa_mask);
+    const double* src = Yk + ((i64)o * c.nK + (i64)a * c.nCl) * s + is;
+    for (int cl = 0; cl < c.nCl; cl++) acc += w2[cl] * src[(i64)cl * s];
   }
   Y[t] = acc;
 }
