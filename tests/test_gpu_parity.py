@@ -186,6 +186,30 @@ def test_merge_by_boundary_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, sa
     assert st["merged_away"] > 0
 
 
+EDGE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, h): the degenerate shapes the method has
+    (1, 3, 2, 2, 1.0, 1, 1.0, 0, 0, 8, "uniform"),       # one row: no boundary MPS at all
+    (1, 1, 3, 2, 1.0, 1, 1.0, 0, 0, 8, "uniform"),       # one cell
+    (3, 1, 2, 2, 1.0, 2, 1.0, 0, 0, 8, "uniform"),       # one column: every bond of every MPS is 1
+    (1, 4, 3, 2, 0.9, 3, 0.8, 0, 0, 16, "uniform"),      # one row with mediating positions
+    (4, 1, 3, 2, 0.9, 3, 0.8, 0, 0, 16, "uniform"),
+    (2, 2, 1, 2, 1.0, 4, 1.0, 0, 0, 300, "uniform"),     # M > 2^8 states: everything kept, log p_d = -inf
+    (1, 2, 2, 4, 1.0, 9, 1.0, 0, 0, 70000, "uniform"),   # M > 2^16 states through the selection kernels
+    (2, 2, 2, 2, 0.0, 5, 1.0, 0, 0, 16, "uniform"),      # no couplings: product distribution
+    (2, 2, 2, 2, 0.0, 5, 1.0, 0, 0, 16, "zero"),         # H = 0: uniform distribution, every rank is a tie
+    (3, 3, 3, 2, 0.0, 5, 1.0, 2, 1, 16, "uniform"),      # truncated D on rank-1 boundaries
+    (2, 3, 2, 2, 0.9, 6, 6.0, 0, 0, 16, "uniform"),      # cold: weights span e^-100
+    (2, 3, 2, 2, 0.9, 6, 1e-3, 0, 0, 16, "uniform"),     # hot: nearly uniform
+    (2, 2, 2, 2, 1.0, 7, 1.0, 0, 0, 1, "uniform"),       # M = 1: greedy descent
+    (3, 3, 2, 2, 0.9, 8, 1.0, 1, 1, 8, "uniform"),       # D = 1
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,D,sweeps,M,h", EDGE)
+def test_degenerate_shapes_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, h):
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed, h=h)
+    compare(inst, beta, D, sweeps, M, 1e-9 if D == 0 else 1e-6)
+
+
 def test_zero_field_z2_instance():
     inst = instances.lattice(3, 3, 2, 4, p_keep=1.0, seed=21, h="zero")
     compare(inst, 2.0, 8, 1, 32, 1e-6)

@@ -263,6 +263,52 @@ def test_no_prune_beam_equals_bruteforce_order():
     assert out["log_pd"] == -np.inf
 
 
+DEGENERATE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, h): shapes where pieces of the network disappear
+    (1, 3, 2, 2, 1.0, 1, 1.0, "uniform"),      # one row: no boundary MPS
+    (1, 1, 3, 2, 1.0, 1, 1.0, "uniform"),      # one cell
+    (3, 1, 2, 2, 1.0, 2, 1.0, "uniform"),      # one column: all bonds 1
+    (1, 3, 3, 2, 0.9, 3, 0.8, "uniform"),      # one row, mediating positions
+    (3, 1, 3, 2, 0.9, 3, 0.8, "uniform"),
+    (2, 2, 2, 2, 0.0, 5, 1.0, "uniform"),      # no couplings
+    (2, 2, 2, 2, 0.9, 6, 6.0, "uniform"),      # cold
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,h", DEGENERATE)
+def test_degenerate_shapes_against_bruteforce(Ly, Lx, S, ns, p, seed, beta, h):
+    """log Z, the probabilities of the kept states and the discarded mass against plain enumeration."""
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed, h=h)
+    E = brute.all_energies(inst)
+    lz = brute.log_z(E, beta)
+    m = model.Model(inst).set_beta(beta)
+    Rm, ln = mps.contract(m, 0, 0)
+    M = 8
+    out = search.branch_and_bound(m, Rm, ln, M)
+    assert abs(out["log_z"] - lz) <= 1e-12 * abs(lz)
+    # every returned state carries its exact Boltzmann probability
+    assert np.allclose(out["logp"], -beta * energy.energies(inst, out["states"]) - lz, rtol=0, atol=1e-10)
+    assert np.all(np.diff(out["logp"]) <= 1e-12)                       # ranks are sorted
+    if inst.n_spins > 12:
+        return
+    # with no pruning the list is the brute-force order and nothing is discarded
+    full = search.branch_and_bound(m, Rm, ln, 1 << inst.n_spins)
+    assert full["states"].shape[0] == 1 << inst.n_spins and full["log_pd"] == -np.inf
+    idx, El = brute.lowest(E, M)
+    assert np.allclose(full["energies"][:M], El, rtol=0, atol=1e-12)
+
+
+def test_uniform_distribution_closed_form():
+    """H = 0: Z = 2^N, every state has log p = -N log 2, the beam discards 1 - M 2^-N exactly."""
+    inst = instances.lattice(2, 2, 2, 2, p_keep=0.0, seed=5, h="zero")
+    m = model.Model(inst).set_beta(1.0)
+    Rm, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, Rm, ln, 16)
+    N = inst.n_spins
+    assert abs(out["log_z"] - N * np.log(2.0)) < 1e-12
+    assert np.allclose(out["logp"], -N * np.log(2.0), rtol=0, atol=1e-12)
+    assert len({tuple(r) for r in out["states"].tolist()}) == 16
+
+
 # ---------------------------------------------------------------- P8: loop-planted ground state
 @pytest.mark.parametrize("seed", [0, 1])
 def test_loop_planted_ground_state(seed):
