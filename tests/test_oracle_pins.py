@@ -367,6 +367,38 @@ def test_compress_gauge_independent_and_monotone():
     assert fid[0] < 1 - 1e-9                                         # the cut really truncates
 
 
+def test_compress_fidelity_obeys_eckart_young():
+    """Any MPS with bond <= D across a cut has overlap with the unit-norm exact row vector of at most
+    sqrt(sum of the D largest sigma^2 of the exact vector's unfolding at that cut) (Eckart-Young, the bound behind
+    'truncating the bond dimension'); the variational passes must come within a
+    modest factor of the best single-cut infidelity.  Also: the returned bonds really are <= D, the result has
+    unit norm, and exp(log-norm) is the norm of the projection of the exact vector on it up to the cut's error."""
+    m, Rex = _row_problem()
+    y = 1
+    pos = mps.row_positions(m, y)
+    exact = mps.mpo_mps_dense(pos, Rex[y + 1])
+    nex = np.linalg.norm(exact)
+    v = exact / nex
+    dims = v.shape
+    for D in (2, 3, 4):
+        cap = 1.0
+        for cut in range(1, len(dims)):                         # unfolding: positions < cut | positions >= cut
+            sv = np.linalg.svd(v.reshape(int(np.prod(dims[:cut])), -1), compute_uv=False)
+            cap = min(cap, float(np.sqrt((sv[:D] ** 2).sum())))
+        for sweeps in (0, 2):
+            st = {}
+            N, ln = mps.compress(pos, Rex[y + 1], D, sweeps, stats=st)
+            assert max(st["bonds"][0][:-1]) <= D and st["bonds"][0][-1] == 1
+            w = mps.mps_to_dense(N)
+            assert abs(np.linalg.norm(w) - 1) < 1e-12
+            fid = abs((w * v).sum())
+            assert fid <= cap + 1e-12
+            if sweeps == 2:                                      # near-optimal: within 4x of the single-cut bound
+                assert 1 - fid <= 4 * len(dims) * (1 - cap) + 1e-12
+                # one-site variational optimum: the centre tensor is the projection, so norm = <w|exact>
+                assert abs(np.exp(ln) - abs((w * exact).sum())) <= 1e-9 * nex
+
+
 def test_compress_large_D_equals_exact():
     m, Rex = _row_problem()
     y = 1
