@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
+    ap.add_argument("--transform", type=int, default=0,
+                    help="lattice transformation 0..7 (PAPER.md:270; instances.transformed; Zephyr-shaped configs only)")
     return ap.parse_args()
 
 
@@ -291,6 +293,9 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     inst, run = replica_instance(args.config, rank)           # one independent replica per rank
+    if args.transform:
+        import instances
+        inst = instances.transformed(inst, args.transform)
     beta = run["beta"][args.beta_index]
     D, sweeps, M = run["D"], run["sweeps"], run["M"]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -408,7 +413,7 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "l2": "flushed (256 MiB fill) between timed steps",
             "config": {"workload": workload_name(args.config, inst, run, beta), "D": D, "M": M, "sweeps": sweeps,
-                       "beta": beta, "merge": bool(args.merge), "parallelism": "replicas x%d" % world, "l2": "flush between steps"},
+                       "beta": beta, "merge": bool(args.merge), "transform": int(args.transform), "parallelism": "replicas x%d" % world, "l2": "flush between steps"},
             "contract_rows_per_s": round(st["rows_contracted"] / max(st["ms_contract"], 1e-9) * 1e3, 3),
             "contract_ms": round(st["ms_contract"], 3), "search_ms": round(st["ms_search"], 3),
             "best_energy": float(E.min()), "n_states": int(len(E)), "log_p_discarded": float(pd),

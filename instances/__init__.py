@@ -125,6 +125,37 @@ def lattice(Ly, Lx, S, n_s, p_keep=1.0, seed=0, h="uniform", h_scale=1.0, name="
                     seed=seed, p_keep=p_keep)
 
 
+def transformed(inst, t: int):
+    """One of the 8 lattice transformations of PAPER.md:270 ("8 distinct transformations of the 2D lattice ...
+    rotations and reflections") as a pure re-indexing of the cluster map: spin ids, the edge list, J and h are
+    untouched, so states and energies of a transformed run compare directly with the original.
+    t bit 0: mirror x, bit 1: mirror y, bit 2: transpose (applied last).  The synthetic geometry admits them as
+    follows: S = 1 (config 1) and S = 2 (Zephyr-shaped): all 8; under transposition the horizontal sub-cluster A
+    and the vertical sub-cluster B swap roles and, for the A_hi x B_lo rule to hold again, lo and hi swap inside
+    both.  S = 3 (Pegasus-shaped): only t = 0, the single (x+1, y+1) diagonal of the shape has no mirror image."""
+    t = int(t)
+    if not 0 <= t < 8:
+        raise ValueError("t must be 0..7")
+    if inst.S == 3 and t != 0:
+        raise ValueError("the Pegasus-shaped lattice (one diagonal direction) admits only the identity")
+    cy, cx = inst.cell_y.copy(), inst.cell_x.copy()
+    sub, pos = inst.sub.copy(), inst.pos.copy()
+    Ly, Lx = inst.Ly, inst.Lx
+    if t & 1:
+        cx = (Lx - 1 - cx).astype(np.int32)
+    if t & 2:
+        cy = (Ly - 1 - cy).astype(np.int32)
+    if t & 4:
+        cy, cx = cx, cy
+        Ly, Lx = Lx, Ly
+        if inst.S == 2:
+            sub = (1 - sub).astype(np.int32)
+            pos = ((pos + inst.n_s // 2) % inst.n_s).astype(np.int32)
+    out = Instance(inst)
+    out.update(name=f"{inst.name}_t{t}", Ly=Ly, Lx=Lx, cell_y=cy, cell_x=cx, sub=sub, pos=pos, transform=t)
+    return out
+
+
 def loop_planted(Ly, Lx, S, n_s, seed=0, n_loops=None, min_len=4, max_len=8, name=""):
     """Loop-planted instance with known ground-state energy (BASELINE.json config 5).
 

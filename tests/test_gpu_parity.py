@@ -210,6 +210,34 @@ def test_degenerate_shapes_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, h)
     compare(inst, beta, D, sweeps, M, 1e-9 if D == 0 else 1e-6)
 
 
+@pytest.mark.parametrize("t", range(8))
+def test_lattice_transformations_parity(t):
+    """The 8 lattice transformations of PAPER.md:270 are re-indexings of the cluster map handed to tn_create
+    (instances.transformed): on every map the CUDA path must match the oracle run on the same map, at exact D
+    (1e-9, both cell kinds that admit them) and at truncated D with ragged projectors (1e-6)."""
+    compare(instances.transformed(instances.lattice(2, 3, 2, 2, p_keep=0.85, seed=4), t), 1.1, 0, 0, 8, 1e-9)
+    compare(instances.transformed(instances.lattice(3, 2, 1, 4, p_keep=0.9, seed=6), t), 1.1, 0, 0, 8, 1e-9)
+    compare(instances.transformed(instances.lattice(3, 4, 2, 4, p_keep=0.9, seed=11), t), 1.0, 6, 1, 32, 1e-6)
+
+
+def test_lattice_transformations_spread_of_log_z():
+    """Z-spread diagnostic: log Z is the same number on all 8 maps at exact D, and the truncated
+    contractions scatter around it by no more than their truncation error."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(3, 4, 2, 4, p_keep=0.9, seed=11)
+    exact, trunc = [], []
+    for t in range(8):
+        with tnb.TensorNetwork(instances.transformed(inst, t)) as tn:
+            tn.set_beta(1.0)
+            tn.contract(0, 0)
+            exact.append(tn.log_z())
+            tn.contract(6, 1)
+            trunc.append(tn.log_z())
+    exact, trunc = np.array(exact), np.array(trunc)
+    assert np.ptp(exact) <= 1e-9 * abs(exact[0])
+    assert np.ptp(trunc) > 0 and np.abs(trunc - exact[0]).max() <= 1e-2 * abs(exact[0])
+
+
 def test_zero_field_z2_instance():
     inst = instances.lattice(3, 3, 2, 4, p_keep=1.0, seed=21, h="zero")
     compare(inst, 2.0, 8, 1, 32, 1e-6)

@@ -329,6 +329,39 @@ def test_loop_planted_zephyr_shape_energy_of_planted_state():
     assert energy.energy(inst, inst.s_star) == inst.E0
 
 
+# ---------------------------------------------------------------- lattice transformations
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed", [(2, 3, 2, 2, 0.85, 4), (3, 2, 1, 4, 0.9, 6)])
+def test_lattice_transformations_leave_exact_results_unchanged(Ly, Lx, S, ns, p, seed):
+    """The 8 transformations only re-index the cluster map: brute force (which never looks at the map) fixes
+    log Z and the low-energy states; the exact contraction on every transformed map must reproduce them, and the
+    exact-D beam must return the same states (energies bit-exact, spins in the original ids)."""
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    beta = 1.1
+    Eall = brute.all_energies(inst)                          # N = 24: 2^24 states
+    lz = brute.log_z(Eall, beta)
+    idx, El = brute.lowest(Eall, 8)
+    assert np.diff(El).min() > 1e-9                          # unique order
+    ref_states = brute.index_to_spins(idx, inst.n_spins)
+    maps = set()
+    for t in range(8):
+        it = instances.transformed(inst, t)
+        assert np.array_equal(it.edge_u, inst.edge_u) and np.array_equal(it.J, inst.J)
+        maps.add((it.Ly, it.Lx, it.cell_y.tobytes(), it.cell_x.tobytes(), it.sub.tobytes(), it.pos.tobytes()))
+        m = model.Model(it).set_beta(beta)
+        R, ln = mps.contract(m, 0, 0)
+        out = search.branch_and_bound(m, R, ln, 8)
+        assert abs(out["log_z"] - lz) <= 1e-12 * abs(lz), t
+        # beta = 1.1, M = 8: the beam may prune a low-energy state; the ground state it must keep
+        assert np.array_equal(out["states"][0], ref_states[0]), t
+        assert np.array_equal(out["energies"], energy.energies(inst, out["states"])), t
+        # the beam content depends on the search order (that is why the paper runs all 8), but at exact D
+        # every state it returns carries its exact Boltzmann log-probability, which brute force fixes
+        assert np.allclose(out["logp"], -beta * out["energies"] - lz, rtol=0, atol=1e-10), t
+    assert len(maps) == 8                                    # the eight maps are distinct
+    with pytest.raises(ValueError):
+        instances.transformed(instances.lattice(2, 2, 3, 2), 1)
+
+
 # ---------------------------------------------------------------- P10-P12: compress
 def _row_problem(seed=3, D=4):
     inst = instances.lattice(3, 4, 2, 2, p_keep=0.9, seed=seed)
