@@ -266,7 +266,7 @@ struct SvdInfo { int flag, keep; double res, sig0, sigk, sigl; };   // device ->
 __global__ void k_resid_flag(const double* part, int nblk, int k, const int* keep, const double* sig, double tol,
                              int* flag, SvdInfo* info, double* res_out, int col0) {
   __shared__ int bad;
-  __shared__ double worst[128];
+  __shared__ double worst[1024];   // one slot per thread: the block has up to 1024 threads (exact mode: k up to TN_OPT_EXACT_CAP)
   if (threadIdx.x == 0) bad = 0;
   __syncthreads();
   // columns of this block are columns col0 .. col0 + k - 1 of the full Ritz list; sig points at the FULL list
@@ -441,6 +441,7 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
     svd_trunc_locked(cx, op, chi, ks, Vz, C, sig0_out);
     return;
   }
+  if (ks > 1024) tn_throw(TN_ERR_ARG, "truncated SVD block of %d columns: at most 1024 are supported", ks);
   DBuf<double> Om(h, (size_t)n * ks), Z(h, (size_t)n * ks), Ya(h, (size_t)m * ks), Yb(h, (size_t)m * ks);
   DBuf<double> TV(h, (size_t)m * ks), US(h, (size_t)m * ks);
   DBuf<double> B(h, (size_t)ks * ks), Bo(h, (size_t)ks * ks), Wt(h, (size_t)ks * ks), sig(h, ks);

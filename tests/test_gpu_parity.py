@@ -220,6 +220,13 @@ def test_lattice_transformations_parity(t):
     compare(instances.transformed(instances.lattice(3, 4, 2, 4, p_keep=0.9, seed=11), t), 1.0, 6, 1, 32, 1e-6)
 
 
+def test_exact_contraction_with_svd_blocks_above_128_columns():
+    """Regression: the exact (D <= 0) contraction of this map runs SVD blocks of 256 columns (retained rank 58); the
+    residual-flag kernel used a 128-entry shared array for one slot per column (illegal address for k > 128)."""
+    inst = instances.transformed(instances.lattice(3, 4, 2, 4, p_keep=0.9, seed=11), 1)
+    compare(inst, 1.0, 0, 0, 32, 1e-9)
+
+
 def test_lattice_transformations_spread_of_log_z():
     """Z-spread diagnostic: log Z is the same number on all 8 maps at exact D, and the truncated
     contractions scatter around it by no more than their truncation error."""
