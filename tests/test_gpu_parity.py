@@ -58,13 +58,21 @@ def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=Fa
     # energies: bit-exact with the oracle's fixed-order recomputation of the SAME states
     assert np.array_equal(E, energy.energies(inst, states))
     # bitstrings identical rank by rank wherever the oracle's adjacent logp gaps exceed the tolerance
+    # At h = 0 every state is exactly degenerate with its global flip: which member of a pair survives a cut that
+    # falls between the two is arbitrary (and decides the sign of its descendants), so states are compared up to
+    # the flip (normalised to s_0 = +1) there; the last rank may also tie with a discarded candidate, which
+    # log p_d (the largest discarded probability) bounds.
+    z2 = not np.any(inst.h)
+    canon = (lambda s: s * s[0]) if z2 else (lambda s: s)
     lp = ref["logp"]
     gap_tol = 10 * tol * np.abs(lp).max()
     for r in range(n):
         lo = r == 0 or lp[r - 1] - lp[r] > gap_tol
-        hi = r == n - 1 or lp[r] - lp[r + 1] > gap_tol
-        if lo and hi:
-            assert np.array_equal(states[r], ref["states"][r]), r
+        hi = (lp[r] - ref["log_pd"] > gap_tol) if r == n - 1 else lp[r] - lp[r + 1] > gap_tol
+        if lo and hi and not np.array_equal(canon(states[r]), canon(ref["states"][r])):
+            # h = 0 on a disconnected graph: every component flips freely, the state of rank r is one of several
+            # exactly degenerate ones; anything else is a mismatch
+            assert z2 and E[r] == energy.energies(inst, ref["states"][r:r + 1])[0], r
     if np.isfinite(ref["log_pd"]):
         assert abs(pd - ref["log_pd"]) <= 10 * tol * abs(ref["log_pd"]), (pd, ref["log_pd"])
     else:
@@ -243,6 +251,54 @@ def test_lattice_transformations_spread_of_log_z():
     exact, trunc = np.array(exact), np.array(trunc)
     assert np.ptp(exact) <= 1e-9 * abs(exact[0])
     assert np.ptp(trunc) > 0 and np.abs(trunc - exact[0]).max() <= 1e-2 * abs(exact[0])
+
+
+def _random_case(i):
+    """Seeded random small case: every cell kind, thinned edges, zero / random fields, exact and truncated D with
+    0-2 passes, beam sizes from 1 to 64, lattice transformations, merge by boundary, both selection routes."""
+    r = np.random.default_rng(9000 + i)
+    S = int(r.integers(1, 4))
+    ns = int(r.choice([2, 4])) if S < 3 else 2
+    if S == 2 and ns == 4 and r.random() < 0.5:
+        ns = 2
+    Ly, Lx = int(r.integers(1, 4)), int(r.integers(1, 5))
+    if S * ns >= 8:
+        Lx = min(Lx, 3)
+    p = float(r.choice([0.7, 0.85, 0.95, 1.0]))
+    beta = float(r.uniform(0.3, 3.0))
+    exact = r.random() < 0.4
+    D = 0 if exact else int(r.integers(2, 9))
+    sweeps = 0 if exact else int(r.integers(0, 3))
+    M = int(r.choice([1, 3, 8, 17, 32, 64]))
+    t = int(r.integers(0, 8)) if S < 3 else 0
+    merge = bool(r.random() < 0.25)
+    h = "zero" if r.random() < 0.2 else "uniform"
+    sampled = bool(r.random() < 0.3)
+    inst = instances.transformed(instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=9000 + 7 * i, h=h), t)
+    return inst, beta, D, sweeps, M, merge, sampled
+
+
+@pytest.mark.parametrize("block", range(8))
+def test_random_small_cases_parity(block):
+    """160 seeded random small cases (20 per block) through the full parity comparison.  A case whose truncated
+    contraction breaks down in the oracle itself (a non-positive normaliser at tiny D) has no reference and is skipped;
+    at most a few may do so."""
+    import paper_2411_16431_b200 as tnb
+    skipped = 0
+    for i in range(20 * block, 20 * block + 20):
+        inst, beta, D, sweeps, M, merge, sampled = _random_case(i)
+        opts = ([(tnb.OPT_MERGE, 1)] if merge else []) + ([(tnb.OPT_SELECT_DIRECT_MAX, 0)] if sampled else [])
+        try:
+            with np.errstate(divide="raise", invalid="raise"):
+                run_oracle(inst, beta, D, sweeps, M, merge=merge)
+        except (FloatingPointError, ValueError):
+            skipped += 1
+            continue
+        try:
+            compare(inst, beta, D, sweeps, M, 1e-9 if D == 0 else 1e-6, options=opts, merge=merge)
+        except AssertionError as e:
+            raise AssertionError(f"random case {i}: {e}") from e
+    assert skipped <= 2
 
 
 def test_zero_field_z2_instance():
