@@ -13,7 +13,6 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtn_b200.so")
-PROBE = os.path.join(HERE, "fp64_peak_probe")
 SOURCES = ["api.cu", "kernels.cu", "tables.cu", "contract.cu", "search.cu", "probe.cu", "orth.cu", "tsgemm.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
@@ -60,9 +59,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 sys.stderr.write(out)
     if force or jobs or _newer(LIB, objs):
         run([nvcc] + NVCC_FLAGS + ["-shared", "-o", LIB] + objs + ["-lcudart"])
-    probe_src = os.path.join(CSRC, "fp64_peak_probe.cu")
-    if os.path.exists(probe_src) and (force or _newer(PROBE, [probe_src])):
-        run([nvcc] + NVCC_FLAGS + ["-o", PROBE, probe_src])
     return LIB
 
 

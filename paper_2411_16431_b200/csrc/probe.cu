@@ -1,6 +1,6 @@
 // tn_fp64_peak: measures this GPU's FP64 tensor-core (DMMA) peak, the roofline denominator of every
 // dense contraction of the path.  MEASURED_PEAKS.json carries no FP64 figure, so bench.py measures it
-// live; the standalone fp64_peak_probe.cu sweeps every mma.sync f64 shape (profiles/r01_fp64_peak.md).
+// live (profiles/r01_fp64_peak.md records the round-1 sweep over every mma.sync f64 shape).
 #include "kernels.cuh"
 
 __global__ void k_dmma_chain(double* out, int iters) {
