@@ -74,6 +74,9 @@ enum {
                              Theta only to the remaining columns (deflation; same converged subspace)          */
   TN_OPT_MERGE = 9,       /* 0 (default) / 1: merge candidates with the same boundary before the bound, keeping the
                              most probable one (Fig. 3(d); reading S11)                 */
+  TN_OPT_MERGE_CAP = 10,  /* capacity of the merge buffers (survivors above the threshold resp. possible boundaries of a
+                             cell; default 2^20, range 1..2^24).  A cell whose candidates fit neither route is selected
+                             WITHOUT merging and counted in tn_stats.merge_fallback_cells                      */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */
@@ -111,6 +114,8 @@ typedef struct {
   int64_t merged_away;       /* candidates removed by TN_OPT_MERGE among those above the selection threshold        */
   int64_t svd_unconverged;   /* truncated SVDs stopped by TN_OPT_SVD_MAXIT with a residual above tolerance:
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
+  int64_t merge_fallback_cells; /* cells at which TN_OPT_MERGE could not merge (merge buffers too small at every threshold
+                                tried) and the selection ran unmerged; 0 = every cell followed Fig. 3(d)          */
 } tn_stats;
 
 /* tn_create: validates the geometry and copies the instance to the device.
@@ -128,7 +133,8 @@ int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges,
 int tn_set_stream(tn_handle*, void* cuda_stream);
 
 /* tn_set_allocator: device allocator callbacks (e.g. torch's caching allocator); must be set
- * before tn_set_beta; alloc returns NULL on failure; NULL callbacks restore cudaMalloc/cudaFree. */
+ * before tn_set_beta; alloc returns NULL on failure; NULL callbacks restore cudaMalloc/cudaFree
+ * (TN_ERR_STATE if blocks obtained from the previous callbacks are still live). */
 int tn_set_allocator(tn_handle*, void* (*alloc)(size_t bytes, void* ctx),
                      void (*free_)(void* ptr, void* ctx), void* ctx);
 

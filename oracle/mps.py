@@ -110,10 +110,13 @@ class SitePos:
             T = A[:, self.Pd[sl], :].transpose(1, 0, 2) @ C[:, self.iR[sl], :].transpose(1, 2, 0)
             _scatter_add(out, self.iL[sl] * self.n_u + self.Pu[sl], T * self.w[sl, None, None])
         T0 = out.reshape(self.nL, self.n_u, A.shape[0], C.shape[0])
-        T1 = np.einsum("pu,luag->lpag", self.Bv, T0)
+        T1 = np.tensordot(self.Bv, T0, axes=([1], [1]))                   # [p', l, al, g] = sum_u Bv[p',u] T0[l,u,al,g]
         if self.fold:
-            T1 = np.einsum("rl,lpag->rpag", self.Bh, T1)
-        return T1.transpose(2, 0, 1, 3).reshape(A.shape[0] * self.wl, self.pu * C.shape[0])
+            T1 = np.tensordot(self.Bh, T1, axes=([1], [1]))               # [r, p', al, g] = sum_l Bh[r,l] T1[p',l,al,g]
+            T1 = T1.transpose(2, 0, 1, 3)                                 # [al, r, p', g]
+        else:
+            T1 = T1.transpose(2, 1, 0, 3)                                 # [al, l, p', g]
+        return T1.reshape(A.shape[0] * self.wl, self.pu * C.shape[0])
 
     def dense(self):
         """Explicit W[wl, p', p, wr] (tiny cells only; used by the pins)."""

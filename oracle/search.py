@@ -143,7 +143,7 @@ def merge_by_boundary(score, parent, state, parent_key, state_code):
 def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
     """Returns dict(states [n, N] int8 +-1, energies [n], logp [n] (descending), log_pd, log_z,
     cell_states [n, Ly*Lx]).  merge=True adds the paper's merge-by-boundary step (Fig. 3(d)) before the bound
-    (reading S11: off by default; the CUDA path does not have it yet)."""
+    (reading S11: off by default; the CUDA path's counterpart is TN_OPT_MERGE)."""
     Ly, Lx = model.Ly, model.Lx
     beam_states = [[]]                  # per element: list of chosen cell states (row-major)
     beam_logp = np.zeros(1)

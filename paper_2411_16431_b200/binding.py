@@ -13,6 +13,7 @@ EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_op
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
                     "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_MERGE_CAP = 10
 
 
 class TnError(RuntimeError):
@@ -27,7 +28,8 @@ class TnStats(C.Structure):
         "ms_search_rblocks", "ms_search_cond", "ms_search_select", "flop_theta_build", "flop_theta_apply",
         "bytes_theta_apply", "flop_search", "bytes_search_cond", "bytes_search_select", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
-            "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged")]
+            "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged",
+            "merge_fallback_cells")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -159,10 +161,12 @@ def tn_branch_and_bound(handle, M, n_spins):
     return states[:k], energies[:k], logp[:k], pd.value
 
 
-def tn_energy(handle, states):
+def tn_energy(handle, states, n_spins=None):
     s = np.ascontiguousarray(states, dtype=np.int8)
     if s.ndim == 1:
         s = s[None, :]
+    if n_spins is not None and (s.ndim != 2 or s.shape[1] != n_spins):   # the C call reads n * n_spins bytes
+        raise TnError(-1, "states must have shape [n, %d], got %s" % (n_spins, s.shape))
     out = np.empty(s.shape[0], dtype=np.float64)
     _check(lib().tn_energy(handle, s.shape[0], _ptr(s, C.c_int8), _ptr(out, C.c_double)))
     return out
@@ -259,7 +263,7 @@ class TensorNetwork:
         return tn_branch_and_bound(self.handle, M, self.n_spins)
 
     def energy(self, states):
-        return tn_energy(self.handle, states)
+        return tn_energy(self.handle, states, self.n_spins)
 
     def stats(self):
         return tn_get_stats(self.handle)

@@ -63,6 +63,7 @@ void* tn_handle::dmalloc(size_t bytes) {
     blk.bytes = bytes;
     bytes_held += (i64)bytes;
   }
+  blk.serial = ++serial;
   live.push_back(blk);
   return blk.p;
 }
@@ -74,6 +75,15 @@ void tn_handle::dfree(void* p) {
       live[i] = live.back();
       live.pop_back();
       return;
+    }
+}
+
+void tn_handle::release_since(unsigned long long mark) {
+  for (size_t i = live.size(); i-- > 0;)
+    if (live[i].serial > mark) {
+      cached.push_back(live[i]);
+      live[i] = live.back();
+      live.pop_back();
     }
 }
 
@@ -97,6 +107,16 @@ StageTimer::~StageTimer() {
   catch (const std::bad_alloc&) { g_last_error = "host out of memory"; return TN_ERR_OOM; } \
   catch (const std::exception& e) { g_last_error = e.what(); return TN_ERR_ARG; }            \
   catch (...) { g_last_error = "unknown error"; return TN_ERR_ARG; }
+
+// Every entry point that touches the device runs on the handle's own device (a process may hold handles on several).
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(const tn_handle* h) {
+    if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->device) cudaSetDevice(h->device);
+    else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 static void need_device() {
   int n = 0;
@@ -152,6 +172,11 @@ int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges, const int32_t* 
         tn_throw(TN_ERR_ARG, "edge %lld: spin index out of range", (long long)e);
       if (!std::isfinite(J[e])) tn_throw(TN_ERR_ARG, "edge %lld: J is not finite", (long long)e);
     }
+    if (hfield)
+      for (int i = 0; i < n_spins; i++)
+        if (!std::isfinite(hfield[i])) tn_throw(TN_ERR_ARG, "spin %d: h is not finite", i);
+    TN_CUDA(cudaGetDevice(&h->device));
+    TN_CUDA(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, h->device));
     tables_create(h);
     h->d_eu = h->dalloc<int>(n_edges + 1); h->d_ev = h->dalloc<int>(n_edges + 1);
     h->d_J = h->dalloc<double>(n_edges + 1); h->d_h = h->dalloc<double>(n_spins);
@@ -164,6 +189,8 @@ int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges, const int32_t* 
     TN_CUDA(cudaMemcpy(h->d_h, h->h.data(), sizeof(double) * n_spins, cudaMemcpyHostToDevice));
     TN_CUDA(cudaMemcpy(h->d_cell_of, h->cell_of.data(), sizeof(int) * n_spins, cudaMemcpyHostToDevice));
     TN_CUDA(cudaMemcpy(h->d_bit_of, h->bit_of.data(), sizeof(int) * n_spins, cudaMemcpyHostToDevice));
+    h->d_cnt = h->dalloc<unsigned long long>(2);
+    TN_CUDA(cudaMemset(h->d_cnt, 0, 2 * sizeof(unsigned long long)));
     *out = h;
     return TN_OK;
   } catch (const TnError& e) {
@@ -189,9 +216,11 @@ int tn_set_allocator(tn_handle* h, void* (*alloc)(size_t, void*), void (*free_)(
   if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
   if ((alloc == nullptr) != (free_ == nullptr)) tn_throw(TN_ERR_ARG, "alloc and free must both be set or both NULL");
   if (h->have_beta) tn_throw(TN_ERR_STATE, "tn_set_allocator must precede tn_set_beta");
-  if (h->alloc_cb && (h->alloc_cb != alloc || h->alloc_ctx != ctx))
-    tn_throw(TN_ERR_STATE, "allocator callbacks can be set only once per handle");
-  trim_free_list(h);   // blocks already handed out keep the origin they were allocated with
+  DeviceGuard dg(h);
+  trim_free_list(h);   // blocks already handed out keep the origin they were allocated with (NULL, NULL = cudaMalloc again)
+  if (h->alloc_cb != alloc || h->alloc_ctx != ctx)
+    for (auto& l : h->live)
+      if (l.src == 1) tn_throw(TN_ERR_STATE, "blocks from the previous allocator callbacks are still live");
   h->alloc_cb = alloc; h->free_cb = free_; h->alloc_ctx = ctx;
   TN_API_END
 }
@@ -216,6 +245,9 @@ int tn_set_option(tn_handle* h, int32_t key, double v) {
     case TN_OPT_SVD_CHEB: h->svd_cheb = v != 0.0; break;
     case TN_OPT_SVD_LOCK: h->svd_lock = v != 0.0; break;
     case TN_OPT_MERGE: h->merge = v != 0.0; break;
+    case TN_OPT_MERGE_CAP:
+      if (v < 1 || v > (double)(1 << 24)) tn_throw(TN_ERR_ARG, "merge cap must be in 1..2^24");
+      h->merge_cap = (i64)v; break;
     case TN_OPT_SELECT_DIRECT_MAX:
       if (v < 0) tn_throw(TN_ERR_ARG, "select direct max must be >= 0");
       h->select_direct_max = (i64)v; break;
@@ -228,6 +260,7 @@ int tn_set_beta(tn_handle* h, double beta) {
   TN_API_BEGIN
   if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
   if (!std::isfinite(beta) || beta < 0.0) tn_throw(TN_ERR_ARG, "beta must be finite and >= 0");
+  DeviceGuard dg(h);
   mps_free(h);
   memset(&h->st, 0, sizeof(h->st));
   if (h->d_cnt) TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
@@ -242,15 +275,19 @@ int tn_contract(tn_handle* h, int32_t D, int32_t sweeps) {
   if (!h->have_beta) tn_throw(TN_ERR_STATE, "tn_contract before tn_set_beta");
   if (sweeps < 0) tn_throw(TN_ERR_ARG, "sweeps < 0");
   if (D > 1008) tn_throw(TN_ERR_ARG, "D > 1008 not supported");
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
   try {
     contract_run(h, D, sweeps);
-  } catch (...) {
+    trim_free_list(h);
+    search_logz(h);
+  } catch (...) {   // no block allocated by this call survives it: the handle is back at its pre-call footprint
+    cudaStreamSynchronize(h->stream);
     mps_free(h);
+    h->release_since(mark);
     trim_free_list(h);
     throw;
   }
-  trim_free_list(h);
-  search_logz(h);
   trim_free_list(h);
   TN_API_END
 }
@@ -291,6 +328,7 @@ int tn_mps_tensor(tn_handle* h, int32_t y, int32_t j, double* out) {
   if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_mps_tensor before tn_contract");
   if (y < 1 || y > h->Ly || j < 0 || j >= (int)h->rows[y].size()) tn_throw(TN_ERR_ARG, "index out of range");
   const MpsTensor& t = h->rows[y][j];
+  DeviceGuard dg(h);
   TN_CUDA(cudaMemcpyAsync(out, t.d, sizeof(double) * t.dl * t.p * t.dr, cudaMemcpyDeviceToHost, h->stream));
   TN_CUDA(cudaStreamSynchronize(h->stream));
   TN_API_END
@@ -302,9 +340,13 @@ int tn_branch_and_bound(tn_handle* h, int32_t M, int32_t* n_out, int8_t* states,
   if (!h || !n_out || !states || !energies || !logp) tn_throw(TN_ERR_ARG, "NULL argument");
   if (M < 1 || M > (1 << 20)) tn_throw(TN_ERR_ARG, "M must be in 1..2^20");
   if (!h->have_mps) tn_throw(TN_ERR_STATE, "tn_branch_and_bound before tn_contract");
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
   try {
     search_run(h, M, n_out, states, energies, logp, log_pd);
   } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
     trim_free_list(h);
     throw;
   }
@@ -315,7 +357,16 @@ int tn_branch_and_bound(tn_handle* h, int32_t M, int32_t* n_out, int8_t* states,
 int tn_energy(tn_handle* h, int32_t n, const int8_t* states, double* energies) {
   TN_API_BEGIN
   if (!h || !states || !energies || n < 0) tn_throw(TN_ERR_ARG, "bad argument");
-  energy_run(h, n, states, energies);
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
+  try {
+    energy_run(h, n, states, energies);
+  } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
+    trim_free_list(h);
+    throw;
+  }
   trim_free_list(h);
   TN_API_END
 }
@@ -325,7 +376,16 @@ int tn_kernel_check(tn_handle* h, int32_t op, int64_t m, int32_t n, int32_t k, c
   TN_API_BEGIN
   if (!h || !A || !Cout || m < 1 || n < 1 || k < 1) tn_throw(TN_ERR_ARG, "bad argument");
   need_device();
-  kernel_check_run(h, op, m, n, k, A, B, Cout);
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
+  try {
+    kernel_check_run(h, op, m, n, k, A, B, Cout);
+  } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
+    trim_free_list(h);
+    throw;
+  }
   trim_free_list(h);
   TN_API_END
 }
@@ -334,9 +394,13 @@ int tn_kernel_bench(tn_handle* h, int32_t op, int64_t m, int32_t n, int64_t k, i
   TN_API_BEGIN
   if (!h || !ms_per_call || m < 1 || n < 1 || k < 1) tn_throw(TN_ERR_ARG, "bad argument");
   need_device();
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
   try {
     kernel_bench_run(h, op, m, n, k, iters, ms_per_call);
   } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
     trim_free_list(h);
     throw;
   }
@@ -347,6 +411,7 @@ int tn_kernel_bench(tn_handle* h, int32_t op, int64_t m, int32_t n, int64_t k, i
 int tn_get_stats(tn_handle* h, tn_stats* out) {
   TN_API_BEGIN
   if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");
+  DeviceGuard dg(h);
   *out = h->st;
   out->bytes_device = h->bytes_held;
   if (h->d_cnt) {
@@ -362,6 +427,7 @@ int tn_get_stats(tn_handle* h, tn_stats* out) {
 void tn_destroy(tn_handle* h) {
   if (!h) return;
   try {
+    DeviceGuard dg(h);
     cudaStreamSynchronize(h->stream);
     mps_free(h);
     tables_destroy(h);

@@ -183,13 +183,9 @@ template <int KP, int NT, class AR, class BR, class EP>
 void launch_bgemm_pipe_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BR& br, const EP& ep) {
   constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
   constexpr int smem = (int)sizeof(double) * (BM * LDA + 2 * KP * LDB);
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_bgemm_pipe<KP, NT, AR, BR, EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    attr = true;
-  }
+  TN_SMEM_OPT_IN(h, (k_bgemm_pipe<KP, NT, AR, BR, EP>), smem);
   const int mt = (M + BM - 1) / BM;
-  const int bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (4 * 296)));
+  const int bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (8 * (i64)h->sms)));
   dim3 grid((unsigned)((batches + bg - 1) / bg), (unsigned)mt);
   k_bgemm_pipe<KP, NT, AR, BR, EP><<<grid, 256, smem, h->stream>>>(batches, bg, M, N, K, ar, br, ep);
   h->st.kernel_launches++;
@@ -219,15 +215,11 @@ template <int KP, int NT, bool A_SHARED, class AR, class BE, class EP>
 void launch_bgemm_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BE& be, const EP& ep) {
   constexpr int BM = 128, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
   constexpr int smem = (int)sizeof(double) * (BM * LDA + KP * LDB);
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_bgemm<KP, NT, A_SHARED, AR, BE, EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    attr = true;
-  }
+  TN_SMEM_OPT_IN(h, (k_bgemm<KP, NT, A_SHARED, AR, BE, EP>), smem);
   const int mt = (M + BM - 1) / BM;
   int bg = 1;
   if (A_SHARED) {   // as many batches per CTA as still leave >= 4 waves of CTAs
-    bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (4 * 296)));
+    bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (8 * (i64)h->sms)));
   }
   dim3 grid((unsigned)((batches + bg - 1) / bg), (unsigned)mt);
   k_bgemm<KP, NT, A_SHARED, AR, BE, EP><<<grid, 256, smem, h->stream>>>(batches, bg, M, N, K, ar, be, ep);

@@ -56,6 +56,9 @@ struct Ctx {
     }
     evs.clear();
   }
+  ~Ctx() {   // normally empty (flush() ran); after an exception the pending events are destroyed here
+    for (auto& e : evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  }
 };
 
 std::vector<PosInfo> row_positions(tn_handle* h, int y) {

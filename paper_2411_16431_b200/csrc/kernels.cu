@@ -47,8 +47,8 @@ void gemm_general(tn_handle* h, const GemmDesc& g) {
   if (nsplit <= 0) {
     i64 tiles = (i64)cdiv(g.M, bm) * cdiv(g.N, bn) * g.B1 * g.B2;
     nsplit = 1;
-    if (tiles < 148 && g.K >= 2048) {
-      nsplit = (int)std::min<i64>((296 + tiles - 1) / tiles, g.K / 512);
+    if (tiles < h->sms && g.K >= 2048) {
+      nsplit = (int)std::min<i64>((2 * h->sms + tiles - 1) / tiles, g.K / 512);
       if (nsplit < 1) nsplit = 1;
     }
   }
@@ -340,15 +340,7 @@ __global__ void __launch_bounds__(1024) k_jacobi_rows(const double* Min, int ld,
 void jacobi_rows(tn_handle* h, const double* Min, int ld, int c, int r, double* Mout, double* Wt, double* sig) {
   if (c > 1024) tn_throw(TN_ERR_ARG, "jacobi_rows: c = %d > 1024", c);
   size_t need = ((size_t)c * r + (size_t)c * c) * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    TN_CUDA(cudaFuncSetAttribute(k_jacobi_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    attr_set = true;
-  }
-  if (!h->d_cnt) {
-    h->d_cnt = h->dalloc<unsigned long long>(2);
-    TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
-  }
+  TN_SMEM_OPT_IN(h, k_jacobi_rows, 200 * 1024);
   if (need <= 200 * 1024) {
     const int jt = std::min(1024, std::max(128, 32 * ((c + 1) / 2)));   // one warp per pair: fewer warps, cheaper barriers
     k_jacobi_rows<<<1, jt, need, h->stream>>>(Min, ld, c, r, Mout, Wt, sig, nullptr, 1, h->d_cnt);

@@ -399,28 +399,26 @@ template <int KT>
 void run_orth(tn_handle* h, double* Y, i64 m, int k, int passes) {
   constexpr int KP = 8 * KT, LD = smem_ld(KP);
   const size_t smem = sizeof(double) * ((size_t)KP * LD + 2 * (size_t)OR_ROWS * LD);
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_orth_pass<KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
-  int nb = (int)std::min<i64>(148, (m + OR_ROWS - 1) / OR_ROWS);
+  TN_SMEM_OPT_IN(h, k_orth_pass<KT>, smem);
+  int nb = (int)std::min<i64>(h->sms, (m + OR_ROWS - 1) / OR_ROWS);
   DBuf<double> part(h, (size_t)(nb + OR_MAXG) * KP * KP), T(h, 2 * (size_t)KP * KP);
   DBuf<OrthCtl> ctl(h, 1);
   TN_CUDA(cudaMemsetAsync(ctl.p, 0, sizeof(OrthCtl), h->stream));
   double tol = 1e-15 * (32.0 + std::sqrt((double)m));
   double frel = 1e-11 * std::max(1.0, std::sqrt((double)m) / 128.0);   // pivot floor relative to max_i G_ii
   // ---- one cooperative launch for all rounds when the device supports it and the grid is co-resident
-  static int coop_slots = -1;
-  if (coop_slots < 0) {
-    int dev = 0, coop = 0, sms = 0, occ = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  static int coop_slots_dev[64];
+  static bool coop_known[64] = {false};
+  const int dv = h->device & 63;
+  if (!coop_known[dv]) {
+    int coop = 0, occ = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
     TN_CUDA(cudaFuncSetAttribute(k_orth_coop<KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_orth_coop<KT>, OR_THREADS, smem);
-    coop_slots = coop ? sms * occ : 0;
+    coop_slots_dev[dv] = coop ? h->sms * occ : 0;
+    coop_known[dv] = true;
   }
+  const int coop_slots = coop_slots_dev[dv];
   if (coop_slots > 0 && nb <= coop_slots) {
     double* Yp = Y;
     double* Tp = T.p;

@@ -392,13 +392,18 @@ __global__ void k_sel_collect(SelArgs a, const SelState* st, Raw* out, unsigned*
   }
 }
 // fmx[m][cl] = max_ch fcd(m, cl, ch): upper bound used to reject whole (m,i,a) entries with one compare
-__global__ void k_sel_fmax(SelArgs a, double* fmx) {
+__global__ void k_sel_fmax(SelArgs a, double* fmx, int* chbest = nullptr) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= a.nb * a.nCl) return;
   int m = t / a.nCl, cl = t % a.nCl;
   double mx = 0.0;
-  for (int ch = 0; ch < a.nCh; ch++) mx = fmax(mx, sel_fcd(a, m, cl, ch));
+  int best = 0;
+  for (int ch = 0; ch < a.nCh; ch++) {
+    const double f = sel_fcd(a, m, cl, ch);
+    if (f > mx) { mx = f; best = ch; }     // the lowest c_hi among equal maxima (S8 order)
+  }
   fmx[t] = mx;
+  if (chbest) chbest[t] = best;
 }
 // Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).  Grid (chunk, m),
 // 16-byte loads, shifts instead of divisions (nA, nCl powers of two); survivors are rare.
@@ -566,6 +571,66 @@ __global__ void k_merge_score(SelArgs a, const Raw* raw, unsigned n, unsigned np
   g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
   out[t] = MCand{g, logp[q.m] + log(u / Z[q.m]), q.m, state};
 }
+// ---- direct route when the number of POSSIBLE boundaries is small (last column / last row, small cells): a segmented
+// arg-max over ALL entries of V keyed by the boundary id, with no threshold.  Pass 1: 64-bit atomicMax of the key bits
+// of r = v * scale_m * max_ch fcd (positive doubles order like integers; r is monotone in the score); pass 2: among
+// the entries that attain the maximum of their group, atomicMin of (parent << 32 | cell state) = the S8 tie-break;
+// pass 3: one candidate per non-empty group with its exact score.
+__device__ __forceinline__ unsigned long long merge_gid(const MergeLegs& lg, const int* pid, int m, int a, int b, int cl) {
+  unsigned long long g = (unsigned long long)pid[m];
+  g = g * (unsigned long long)(lg.use_r ? lg.n_r : 1) + (unsigned long long)(lg.use_r ? lg.Pr[a] : 0);
+  g = g * (unsigned long long)(lg.use_d ? lg.n_d : 1) + (unsigned long long)(lg.use_d ? lg.Pd[b] : 0);
+  g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
+  return g;
+}
+__device__ __forceinline__ unsigned merge_state(int a, int b, int cl, int ch, int ns, int S) {
+  unsigned state = (unsigned)a;
+  if (S >= 2) state |= (unsigned)b << ns;
+  if (S == 3) state |= ((unsigned)cl | ((unsigned)ch << (ns / 2))) << (2 * ns);
+  return state;
+}
+template <int PASS>
+__global__ void __launch_bounds__(256) k_merge_seg(SelArgs a, int lgA, int lgCl, const double* fmx, const int* chbest,
+                                                   const int* pid, MergeLegs lg, int ns, int S, unsigned long long* gbest,
+                                                   unsigned long long* gtie, unsigned long long* npos) {
+  const int m = blockIdx.y, nchunk = gridDim.x;
+  const i64 c0 = a.per_m * blockIdx.x / nchunk, c1 = a.per_m * (blockIdx.x + 1) / nchunk;
+  const double* v = a.V + (i64)m * a.per_m;
+  const double sc = a.scale[m];
+  unsigned cnt = 0;
+  for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
+    const double x = v[q];
+    if (!(x > 0.0)) continue;
+    const int i = (int)(q >> lgA), aa = (int)(q & (a.nA - 1)), cl = i & (a.nCl - 1), b = i >> lgCl;   // S == 1: X is the identity, positive entries have b == a
+    const double r = x * sc * fmx[(i64)m * a.nCl + cl];
+    if (!(r > 0.0)) continue;
+    const unsigned long long key = (unsigned long long)__double_as_longlong(r);
+    const unsigned long long g = merge_gid(lg, pid, m, aa, b, cl);
+    if (PASS == 1) {
+      atomicMax(&gbest[g], key);
+      cnt++;
+    } else if (gbest[g] == key) {
+      const unsigned st = merge_state(aa, b, cl, chbest[(i64)m * a.nCl + cl], ns, S);
+      atomicMin(&gtie[g], ((unsigned long long)m << 32) | st);
+    }
+  }
+  if (PASS == 1 && cnt) atomicAdd(npos, (unsigned long long)cnt);
+}
+__global__ void k_merge_seg_emit(SelArgs a, const unsigned long long* gbest, const unsigned long long* gtie, i64 ngroups,
+                                 const double* logp, const double* Z, int ns, int S, Cand* out, unsigned* count) {
+  const i64 g = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= ngroups || gbest[g] == 0ull) return;
+  const unsigned long long t = gtie[g];
+  const int m = (int)(t >> 32);
+  const unsigned st = (unsigned)(t & 0xffffffffull);
+  const unsigned smask = (1u << ns) - 1, hmask = (1u << (ns / 2)) - 1;
+  const int aa = (int)(st & smask), b = S == 1 ? aa : (int)((st >> ns) & smask);
+  const int cl = S == 3 ? (int)((st >> (2 * ns)) & hmask) : 0, ch = S == 3 ? (int)((st >> (2 * ns + ns / 2)) & hmask) : 0;
+  const int i = S == 1 ? aa : b * a.nCl + cl;
+  const double u = a.V[(i64)m * a.per_m + (i64)i * a.nA + aa] * sel_fcd(a, m, cl, ch);
+  out[atomicAdd(count, 1u)] = Cand{logp[m] + log(u / Z[m]), m, st};
+}
+
 // Bitonic sort of n = 2^p elements with shared-memory tiles of TILE elements: one launch sorts every tile up to
 // k = TILE (direction from the GLOBAL index), then each k > TILE costs one global launch per j >= TILE and one
 // launch that finishes j < TILE inside the tiles: 6 launches for 32768 elements instead of 120.
@@ -608,11 +673,7 @@ __global__ void k_bitonic_gstep(T* c, unsigned n, unsigned k, unsigned j) {
 template <class T, class Less>
 static void bitonic_sort(tn_handle* h, T* c, unsigned n) {   // n a power of two
   constexpr int TILE = 4096;
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_bitonic_tile<T, Less, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, TILE * (int)sizeof(T)));
-    attr = true;
-  }
+  TN_SMEM_OPT_IN(h, (k_bitonic_tile<T, Less, TILE>), TILE * (int)sizeof(T));
   const unsigned tiles = (n + TILE - 1) / TILE;
   k_bitonic_tile<T, Less, TILE><<<tiles, 1024, std::min<unsigned>(n, TILE) * sizeof(T), h->stream>>>(c, n, 2, std::min<unsigned>(n, TILE));
   TN_LAUNCH_CHECK(h);
@@ -716,12 +777,19 @@ T d2h(tn_handle* h, const T* p) {
 }
 
 struct Tic {
-  tn_handle* h; double* dst; cudaEvent_t a, b;
+  tn_handle* h; double* dst; cudaEvent_t a = nullptr, b = nullptr;
   Tic(tn_handle* h_, double* d) : h(h_), dst(d) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, h->stream); }
+  Tic(const Tic&) = delete;
+  Tic& operator=(const Tic&) = delete;
   void stop() {
     cudaEventRecord(b, h->stream); cudaEventSynchronize(b);
     float ms = 0; if (cudaEventElapsedTime(&ms, a, b) == cudaSuccess) *dst += ms;
     cudaEventDestroy(a); cudaEventDestroy(b);
+    a = b = nullptr;
+  }
+  ~Tic() {   // an exception between the constructor and stop(): the events do not outlive the call
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
   }
 };
 
@@ -765,10 +833,13 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   const unsigned ccap = 1u << 22;                   // compact candidate list of the prefilter pass
   DBuf<double> ckeys(h, ccap), fmx(h, (size_t)M * 16);
   DBuf<Raw> craw(h, ccap);
-  const unsigned mcap = h->merge ? (1u << 20) : 1u;   // survivors handled by the merge route
-  DBuf<MCand> mcand(h, 2 * (size_t)mcap);
-  DBuf<Cand> mcands(h, 2 * (size_t)mcap + 4096);
-  DBuf<int> pid(h, M);
+  const unsigned mcap = h->merge ? (unsigned)h->merge_cap : 1u;   // survivors / boundary groups handled by the merge route
+  size_t mcap2 = 2;                                    // sort buffers: next power of two above max(mcap, M) entries
+  while (mcap2 < (size_t)std::max<i64>(mcap, M) + 1) mcap2 <<= 1;
+  DBuf<MCand> mcand(h, h->merge ? mcap2 : 1);
+  DBuf<Cand> mcands(h, h->merge ? mcap2 + 4096 : 1);
+  DBuf<int> pid(h, M), chbest(h, h->merge ? (size_t)M * 16 : 1);
+  DBuf<unsigned long long> gbest(h, 2 * (size_t)mcap + 2);   // [mcap] group maxima, [mcap] tie-breaks, [1] positive-entry count
   DBuf<Cand> cand(h, npad);
   unsigned* st_cur = stA.p; unsigned* st_nxt = stB.p;
   double* lp_cur = lpA.p; double* lp_nxt = lpB.p;
@@ -780,11 +851,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   TN_CUDA(cudaMemsetAsync(nneg.p, 0, sizeof(unsigned long long), h->stream));
   TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
   TN_CUDA(cudaMemsetAsync(st_cur, 0, sizeof(unsigned) * ncell, h->stream));
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_bitonic_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * (int)sizeof(Cand)));
-    attr = true;
-  }
+  TN_SMEM_OPT_IN(h, k_bitonic_smem, 8192 * (int)sizeof(Cand));
 
   for (int y = 0; y < Ly; y++) {
     const std::vector<MpsTensor>& R = h->rows[y + 1];
@@ -909,6 +976,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         if (!(z0 > 0.0) || !std::isfinite(z0)) tn_throw(TN_ERR_NUMERIC, "first-cell normaliser is %g", z0);
         double lz = -h->beta * h->offset + std::log(z0) + ls0;
         for (int yy = 1; yy < Ly; yy++) lz += h->lognorm[yy];
+        if (!std::isfinite(lz)) tn_throw(TN_ERR_NUMERIC, "log Z = %g is not finite (beta * offset = %g)", lz, h->beta * h->offset);
         h->log_z = lz;
         h->have_logz = true;
         if (logz_only) {
@@ -927,7 +995,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
       const int shifts[6] = {52, 40, 28, 16, 4, 0}, nbitsv[6] = {12, 12, 12, 12, 12, 4};
       const i64 total = (i64)nb * per_m;
-      const int gsel = (int)std::min<i64>(148 * 8, (total + 255) / 256);
+      const int gsel = (int)std::min<i64>((i64)h->sms * 8, (total + 255) / 256);
       unsigned ncand = 0;
       bool direct = total * c.nCh <= (i64)h->select_direct_max;       // few candidates: radix passes straight on V
       bool cand_sorted = false;                                       // set by the merge route (cand.p final and sorted)
@@ -960,10 +1028,38 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         int lgA = 0;
         while ((1 << lgA) < c.nA) lgA++;
         const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
-        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
+        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p, chbest.p);
         TN_LAUNCH_CHECK(h);
+        // number of POSSIBLE boundaries of the candidates of this cell
+        const double gposs = (double)ids.size() * (lg.use_r ? lg.n_r : 1) * (lg.use_d ? lg.n_d : 1) * (lg.use_o ? lg.n_o : 1);
+        const bool seg = gposs <= (double)mcap;
+        bool ok = false;
+        unsigned n1 = 0, ng = 0;
+        if (seg) {
+          // ---- few possible boundaries (always so in the last column and the last row): segmented arg-max over all of V
+          const i64 ngroups = (i64)gposs;
+          int lgCl = 0;
+          while ((1 << lgCl) < c.nCl) lgCl++;
+          unsigned long long* gt = gbest.p + mcap;
+          unsigned long long* npos = gbest.p + 2 * (size_t)mcap;
+          TN_CUDA(cudaMemsetAsync(gbest.p, 0, sizeof(unsigned long long) * ngroups, h->stream));
+          TN_CUDA(cudaMemsetAsync(gt, 0xff, sizeof(unsigned long long) * ngroups, h->stream));
+          TN_CUDA(cudaMemsetAsync(npos, 0, sizeof(unsigned long long), h->stream));
+          TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+          const int nch2 = (int)std::max<i64>(1, std::min<i64>(64, per_m / 4096));
+          k_merge_seg<1><<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, fmx.p, chbest.p, pid.p, lg, ns, S, gbest.p, gt, npos);
+          TN_LAUNCH_CHECK(h);
+          k_merge_seg<2><<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, fmx.p, chbest.p, pid.p, lg, ns, S, gbest.p, gt, npos);
+          TN_LAUNCH_CHECK(h);
+          k_merge_seg_emit<<<cdiv(ngroups, 256), 256, 0, h->stream>>>(sa, gbest.p, gt, ngroups, lp_cur, Z.p, ns, S, mcands.p, count.p);
+          TN_LAUNCH_CHECK(h);
+          h->st.bytes_search_select += 2.0 * 8.0 * nb * (double)per_m;
+          ng = d2h(h, count.p);
+          n1 = (unsigned)std::min<unsigned long long>(d2h(h, npos), 0xffffffffull);
+          ok = true;
+        }
         double thr = 0.0;                                // few candidates: take every positive entry
-        if (!direct) {
+        if (!seg && !direct) {
           for (int pass = 0; pass < 2; pass++) {
             k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
             TN_LAUNCH_CHECK(h);
@@ -977,15 +1073,22 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
             thr *= 1.0 - 1e-12;
           }
         }
-        bool ok = false;
-        unsigned n1 = 0, ng = 0;
-        for (int attempt = 0; attempt < 4; attempt++) {
+        // The threshold is lowered (/ 64) while fewer than M + 1 boundaries lie above it and raised again (geometric
+        // bisection) when more candidates than the merge buffers hold lie above it.
+        const int max_attempts = 16;
+        double thr_few = -1.0, thr_many = -1.0;          // last thresholds with too few groups / too many survivors
+        for (int attempt = 0; !seg && attempt < max_attempts; attempt++) {
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
           k_sel_prefilter_merge<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, thr, fmx.p, craw.p, count.p, mcap);
           h->st.bytes_search_select += 8.0 * nb * (double)per_m * (attempt == 0 && !direct ? 1.0 + 2.0 / 64.0 : 1.0);
           TN_LAUNCH_CHECK(h);
           n1 = d2h(h, count.p);
-          if (n1 > mcap) break;                          // too many survivors for the merge buffers: unmerged route
+          if (n1 > mcap) {                               // too many survivors for the merge buffers
+            thr_many = thr;
+            if (thr_few <= 0.0 || !(thr_few > thr_many * (1.0 + 1e-9))) break;
+            thr = std::sqrt(thr_few) * std::sqrt(thr_many);
+            continue;
+          }
           if (n1 == 0 && thr == 0.0) break;
           unsigned mp2 = 2;
           while (mp2 < n1 + 1) mp2 <<= 1;
@@ -997,7 +1100,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           TN_LAUNCH_CHECK(h);
           ng = d2h(h, count.p);
           if (ng >= (unsigned)M + 1 || thr == 0.0) { ok = true; break; }
-          thr = attempt < 2 ? thr / 64.0 : 0.0;          // fewer than M + 1 boundaries above the bound: lower it
+          thr_few = thr;                                 // fewer than M + 1 boundaries above the bound: lower it
+          if (thr_many > 0.0) thr = std::sqrt(thr_few) * std::sqrt(thr_many);
+          else thr = thr > 1e-290 ? thr / 64.0 : 0.0;
         }
         if (ok) {
           if (ng == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
@@ -1010,6 +1115,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           ncand = ng;
           cand_sorted = true;
         } else {
+          // more survivors than the merge buffers hold at every threshold tried: this cell is selected WITHOUT merging
+          // (counted: a run with merge_fallback_cells > 0 is not the algorithm of Fig. 3(d) at those cells)
+          h->st.merge_fallback_cells++;
           TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
           TN_CUDA(cudaMemsetAsync(hist.p, 0, sizeof(unsigned) * 4096, h->stream));
         }
@@ -1045,7 +1153,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         } else {
           // (3) exact radix selection on the compact keys
           TN_CUDA(cudaMemcpyAsync(sel.p, &s0, sizeof(s0), cudaMemcpyHostToDevice, h->stream));
-          const int gc = (int)std::min<i64>(148 * 4, ((i64)n1 + 255) / 256);
+          const int gc = (int)std::min<i64>((i64)h->sms * 4, ((i64)n1 + 255) / 256);
           for (int pass = 0; pass < 6; pass++) {
             k_csel_hist<<<gc, 256, 0, h->stream>>>(ckeys.p, n1, sel.p, shifts[pass], nbitsv[pass], pass == 0, hist.p);
             TN_LAUNCH_CHECK(h);

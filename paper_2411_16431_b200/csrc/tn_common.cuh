@@ -84,6 +84,7 @@ struct tn_handle {
   int D = 0, sweeps = 0;
   // options
   int merge = 0;            // TN_OPT_MERGE: merge candidates by boundary before the bound (Fig. 3(d))
+  i64 merge_cap = 1ll << 20;  // TN_OPT_MERGE_CAP: survivors / boundary groups the merge buffers hold
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
   int svd_skip_first = 0;   // predictor (contract.cu): skip the first Rayleigh-Ritz step of the next truncated SVD
   double svd_tol = 1e-11;
@@ -94,19 +95,34 @@ struct tn_handle {
   void (*free_cb)(void*, void*) = nullptr;
   void* alloc_ctx = nullptr;
   i64 bytes_held = 0;
-  struct Block { void* p; size_t bytes; int src; };   // src: 0 cudaMalloc, 1 allocator callback
+  struct Block { void* p; size_t bytes; int src; unsigned long long serial; };   // src: 0 cudaMalloc, 1 allocator callback
   std::vector<Block> live, cached;
+  unsigned long long serial = 0;   // allocation counter: every block handed out by dmalloc carries the value at its birth
+  int device = 0, sms = 148;       // CUDA device of this handle and its SM count (queried at tn_create)
   tn_stats st;
   cudaEvent_t ev[2] = {nullptr, nullptr};
   unsigned long long* d_cnt = nullptr;   // device counters: [0] Jacobi calls, [1] Jacobi sweeps
 
   void* dmalloc(size_t bytes);
   void dfree(void* p);
+  // error paths: every block handed out after `mark = serial` was taken goes back to the free list
+  void release_since(unsigned long long mark);
   template <class T>
   T* dalloc(size_t n) { return (T*)dmalloc(n * sizeof(T) + 16); }
   const CellDev& cell(int y, int x) const { return cells[(size_t)y * Lx + x]; }
   bool has_med() const { return S == 3; }
 };
+
+// One-time (per device) opt-in to more than 48 KB of dynamic shared memory for kernel `fn`.
+#define TN_SMEM_OPT_IN(h, fn, bytes)                                                                   \
+  do {                                                                                                 \
+    static bool done__[64] = {false};                                                                  \
+    const int d__ = (h)->device & 63;                                                                  \
+    if (!done__[d__]) {                                                                                \
+      TN_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes)));    \
+      done__[d__] = true;                                                                              \
+    }                                                                                                  \
+  } while (0)
 
 // simple scoped device buffer
 template <class T>

@@ -160,11 +160,7 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
   constexpr int BM = 16 * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK), LDB = smem_ld(NP);
   constexpr size_t smem = sizeof(double) * TS_STAGES * ((TRANS ? TS_BK * LDA : BM * LDA) + TS_BK * LDB);
-  static bool attr = false;
-  if (!attr) {
-    TN_CUDA(cudaFuncSetAttribute(k_tsgemm<NT, WARPS, TRANS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
+  TN_SMEM_OPT_IN(h, (k_tsgemm<NT, WARPS, TRANS>), smem);
   i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
   nsplit = (int)((Kred + kper - 1) / kper);
   const int nbz = tsb.n, nz = (N + NP - 1) / NP;
@@ -182,13 +178,13 @@ void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb,
 
 // CTA width and reduction split: minimise  waves x (per-CTA work + fixed cost) + split-workspace traffic.
 // Measured on B200 (profiles/): wide CTAs win everywhere; the split mostly repairs wave quantisation when the
-// output has fewer row blocks than 2 x 148 CTA slots.
+// output has fewer row blocks than 2 CTA slots per SM.
 template <int NT, bool TRANS>
 void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
                 i64 Kred, const TsBatch& tsb) {
   int warps = Mout > 64 ? 8 : Mout > 32 ? 4 : 2;
   const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps) * ((N + 8 * NT - 1) / (8 * NT)) * tsb.n;
-  const int slots = 148 * ((NT <= 10 || warps < 8) ? 2 : 1);
+  const int slots = h->sms * ((NT <= 10 || warps < 8) ? 2 : 1);
   const double t_k = 2.0 * 16 * warps * (8 * NT) * slots / 37e12;      // seconds per reduction index per CTA
   const double t_ws = (double)Mout * N * 16.0 / 6e12 + 2e-7;           // seconds per extra split (write + read)
   int best = 1;
