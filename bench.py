@@ -1,17 +1,24 @@
 """bench.py -- times the whole hot path (a1 tables -> a2-a4 boundary-MPS contraction -> a5 branch and bound)
 of one synthetic instance per step, through the C ABI of libtn_b200.so.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference] [--no-headline]
 
-Workload: BASELINE.json configs[I] (default I = 1, the Zephyr-shaped 6x6x16 instance; configs[0] is the
-brute-force parity case).  A step = tn_set_beta + tn_contract(D, sweeps) + tn_branch_and_bound(M) on an
-instance that is already resident in HBM (tn_create done before the timed region).  The `e2e` arm repeats
-the measurement with tn_create (host -> device copy of the instance) and tn_destroy inside the timed
-region; results always come back to caller-allocated host buffers.  Multi-GPU: replicas only (DESIGN.md
-section 9) -- every rank solves its own seeded instance, no data-path collective; NCCL is used for the
-barrier and the max-over-ranks of the device time.
+Workload: BASELINE.json configs[I].  Default I = 2, the Pegasus-shaped 8x8x24 instance (N = 1536, D = 32, M = 1024):
+the largest config whose `--steps 20 --warmup 5` run fits the driver's per-arm time limit (about 3 s per step; every
+kernel is in its streaming regime, the Theta-core is 8.6 GB >> L2).  The north_star target workload, configs[3]
+(Pegasus-shaped 15x15x24, N = 5400, D = 64, M = 1024, three variational passes, beta = 2), takes about two minutes per
+step, so the same JSON line carries a `headline` record of ONE timed step of it (own stage table, roofline and clocks;
+`--no-headline` skips it, N = 1 only).
+A step = tn_set_beta + tn_contract(D, sweeps) + tn_branch_and_bound(M) on an instance that is already resident in HBM
+(tn_create done before the timed region).  The `e2e` arm repeats the measurement with tn_create (host -> device copy
+of the instance) and tn_destroy inside the timed region; results always come back to caller-allocated host buffers.
+Multi-GPU: replicas only -- every rank solves its own seeded instance (or, with
+`--replicas transforms`, its own lattice transformation of ONE instance), no data-path collective; NCCL
+is used for the barrier and the max-over-ranks of the device time.
 
---impl reference times the CPU oracle (oracle/, numpy fp64) on a bounded sample of the same workload.
+--impl reference times the CPU oracle (oracle/, numpy fp64) as it stands: the whole instance where it finishes in
+bounded time (configs[0], [1]), else the largest whole sub-problem that does, with any scaled figure labelled
+"extrapolated".
 """
 from __future__ import annotations
 
@@ -35,15 +42,30 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0-based)")
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (0-based)")
     ap.add_argument("--beta-index", type=int, default=0, help="which beta of the config's sweep")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-headline", action="store_true",
+                    help="skip the one-step record of configs[3] (the north_star target workload)")
+    ap.add_argument("--replicas", default="seeds", choices=["seeds", "transforms"],
+                    help="what the N ranks differ by: generator seeds (default) or the 8 lattice transformations "
+                         "of one instance (PAPER.md:270; best-of-N energy and log Z spread are reported)")
+    ap.add_argument("--streams", type=int, default=1,
+                    help="N = 1 with --replicas transforms: run the 8 maps as concurrent replicas on this many "
+                         "CUDA streams (one host thread per stream)")
     ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
     ap.add_argument("--transform", type=int, default=0,
                     help="lattice transformation 0..7 (PAPER.md:270; instances.transformed; Zephyr-shaped configs only)")
     return ap.parse_args()
+
+
+def config_record(ci, inst, run, beta, merge, transform, world):
+    """The `config` object of the JSON line (same keys in both arms, so that the driver sees the same config)."""
+    return {"workload": workload_name(ci, inst, run, beta), "D": run["D"], "M": run["M"], "sweeps": run["sweeps"],
+            "beta": beta, "merge": bool(merge), "transform": int(transform), "parallelism": "replicas x%d" % world,
+            "l2": "flush between steps"}
 
 
 def workload_name(ci, inst, run, beta):
@@ -52,38 +74,82 @@ def workload_name(ci, inst, run, beta):
 
 
 # ----------------------------------------------------------------------------------------------------
-# CPU oracle on a bounded sample: the top `rows` rows of the instance, whole path
+# CPU oracle, as it stands, on the whole instance or on the largest whole sub-problem that finishes in bounded time
 # ----------------------------------------------------------------------------------------------------
-def slice_rows(inst, rows):
-    """Sub-instance made of the first `rows` cell rows (spins are row-major, so it is a prefix)."""
+def sub_lattice(inst, rows, cols):
+    """Sub-instance made of the top-left `rows` x `cols` block of cells (spin ids re-numbered, edges inside kept)."""
+    import numpy as np
     import instances
-    keep = inst.cell_y < rows
-    n = int(keep.sum())
+    keep = (inst.cell_y < rows) & (inst.cell_x < cols)
+    idx = np.flatnonzero(keep)
+    remap = -np.ones(inst.n_spins, dtype=np.int64)
+    remap[idx] = np.arange(idx.size)
     ke = keep[inst.edge_u] & keep[inst.edge_v]
     d = dict(inst)
-    d.update(n_spins=n, edge_u=inst.edge_u[ke], edge_v=inst.edge_v[ke], J=inst.J[ke], h=inst.h[:n], Ly=rows,
-             cell_y=inst.cell_y[:n], cell_x=inst.cell_x[:n], sub=inst.sub[:n], pos=inst.pos[:n])
+    d.update(n_spins=int(idx.size), edge_u=remap[inst.edge_u[ke]].astype(np.int32),
+             edge_v=remap[inst.edge_v[ke]].astype(np.int32), J=inst.J[ke], h=inst.h[idx], Ly=rows, Lx=cols,
+             cell_y=inst.cell_y[idx], cell_x=inst.cell_x[idx], sub=inst.sub[idx], pos=inst.pos[idx])
     return instances.Instance(d)
 
 
-def oracle_sample(inst, run, beta, rows=2):
-    """Runs oracle/ as it stands on the top `rows` rows (tables, rows-1 boundary-MPS rows, B&B over all
-    cells of the slice).  Returns (measured seconds, extrapolated seconds per full instance, description)."""
-    from oracle import model, mps, search
-    s = slice_rows(inst, min(rows, inst.Ly))
-    t0 = time.perf_counter()
-    m = model.Model(s).set_beta(beta)
-    t1 = time.perf_counter()
-    R, ln = mps.contract(m, run["D"], run["sweeps"])
-    t2 = time.perf_counter()
-    search.branch_and_bound(m, R, ln, run["M"])
-    t3 = time.perf_counter()
-    cells_s, cells = s.Ly * s.Lx, inst.Ly * inst.Lx
-    est = (t1 - t0) * cells / cells_s + (t2 - t1) * (inst.Ly - 1) / max(1, s.Ly - 1) + (t3 - t2) * cells / cells_s
-    desc = ("oracle/ (numpy fp64) on the top %d of %d cell rows (%d of %d spins): tables %.1fs, %d boundary-MPS "
-            "row(s) %.1fs, B&B over %d cells %.1fs; value = extrapolation to the full instance by cell / row "
-            "counts" % (s.Ly, inst.Ly, s.n_spins, inst.n_spins, t1 - t0, s.Ly - 1, t2 - t1, cells_s, t3 - t2))
-    return t3 - t0, est, desc
+# (rows, cols, beam) of the oracle sample per config: None = the whole instance.  Pegasus-shaped cells have 2^24
+# states: every oracle operation on one cell costs seconds, so the sample there is a 2 x 2 block with one beam element.
+ORACLE_SAMPLE = {0: None, 1: None, 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64)}
+ORACLE_SAMPLE_SMALL = {0: None, 1: (2, 6, 256), 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64)}   # reference arm, many steps
+
+
+class OracleSample:
+    """Times oracle/ (numpy fp64, never tuned for this) on `spec` of the workload.  The instance preprocessing
+    (cluster energies, projectors: oracle.model.Model.__init__, the counterpart of tn_create) is done once and timed
+    separately; a step = set_beta + contract(D, sweeps) + branch_and_bound, like the GPU arm's step."""
+
+    def __init__(self, inst, run, beta, spec):
+        from oracle import model
+        self.full, self.run, self.beta = inst, run, beta
+        self.whole = spec is None or (spec[0] >= inst.Ly and spec[1] >= inst.Lx and spec[2] >= run["M"])
+        self.rows, self.cols, self.M = (inst.Ly, inst.Lx, run["M"]) if self.whole else spec
+        self.inst = inst if self.whole else sub_lattice(inst, self.rows, self.cols)
+        t0 = time.perf_counter()
+        self.model = model.Model(self.inst)
+        self.t_setup = time.perf_counter() - t0
+
+    def step(self):
+        from oracle import mps, search
+        t0 = time.perf_counter()
+        m = self.model.set_beta(self.beta)
+        t1 = time.perf_counter()
+        R, ln = mps.contract(m, self.run["D"], self.run["sweeps"])
+        t2 = time.perf_counter()
+        search.branch_and_bound(m, R, ln, self.M)
+        t3 = time.perf_counter()
+        self.parts = (t1 - t0, t2 - t1, t3 - t2)
+        return t3 - t0
+
+    def positions(self, cols):
+        return 2 * cols - 1 if self.inst.S == 3 else cols
+
+    def estimate(self):
+        """Seconds per FULL instance from the last step: the measurement itself when the sample is the whole instance,
+        else scaled by cell / (row x position) / (cell x beam) counts -- a LOWER bound, the old bonds inside a two-row
+        sample are 1 where a full-height lattice has up to D."""
+        tb, tc, ts = self.parts
+        if self.whole:
+            return tb + tc + ts
+        f, s = self.full, self.inst
+        cells = (f.Ly * f.Lx) / (s.Ly * s.Lx)
+        rows = (f.Ly - 1) * self.positions(f.Lx) / max(1, (s.Ly - 1) * self.positions(s.Lx))
+        return tb * cells + tc * rows + ts * cells * self.run["M"] / self.M
+
+    def describe(self):
+        tb, tc, ts = self.parts
+        what = ("the WHOLE instance" if self.whole else
+                "the top-left %d x %d cells (%d of %d spins) with beam %d of %d"
+                % (self.rows, self.cols, self.inst.n_spins, self.full.n_spins, self.M, self.run["M"]))
+        tail = "" if self.whole else ("; value = measured parts scaled by cell, row x position and cell x beam counts "
+                                      "(extrapolated, a lower bound: old bonds in a 2-row sample are 1, not D)")
+        return ("oracle/ (numpy fp64, as it stands) on %s: instance preprocessing %.1fs (once, outside the step), "
+                "step = tables %.1fs + %d boundary-MPS row(s) %.1fs + B&B over %d cells %.1fs%s"
+                % (what, self.t_setup, tb, self.inst.Ly - 1, tc, self.inst.Ly * self.inst.Lx, ts, tail))
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -163,20 +229,24 @@ def run_reference(args):
     inst, run = instances.config(args.config)
     beta = run["beta"][args.beta_index]
     import numpy  # noqa: F401  (loads the BLAS whose thread count is reported)
+    table = ORACLE_SAMPLE if args.steps + args.warmup <= 3 else ORACLE_SAMPLE_SMALL
+    smp = OracleSample(inst, run, beta, table[args.config])
     for _ in range(args.warmup):
-        oracle_sample(inst, run, beta)
-    ests, meas, desc = [], [], ""
+        smp.step()
+    ests, meas = [], []
     for _ in range(args.steps):
-        tm, est, desc = oracle_sample(inst, run, beta)
-        ests.append(est)
-        meas.append(tm)
+        meas.append(smp.step())
+        ests.append(smp.estimate())
     v = sum(ests) / len(ests)
     cores = host_threads()
+    # value and ms_per_step are the SAME quantity (seconds per full instance); the measured sample time sits beside them
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * sum(meas) / len(meas), "higher_is_better": False,
+            "warmup": args.warmup, "ms_per_step": 1e3 * v, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config, inst, run, beta)},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "extrapolated": not smp.whole, "sample_seconds_per_step": sum(meas) / len(meas),
+            "config": config_record(args.config, inst, run, beta, False, 0, 1),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.describe(),
+                             "extrapolated": not smp.whole, "sample_seconds": round(sum(meas) / len(meas), 2)},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
@@ -249,24 +319,91 @@ STAGES = [  # (stats ms key, label, kernel, flop key, bytes key, bound)
      "flop_theta_apply", "bytes_theta_apply", "tensor"),
     ("ms_theta_build", "theta_build", "k_bgemm_pipe<.., ArTh, BrTh, EpTh> (Theta-core build) + projector maps", "flop_theta_build",
      None, "tensor"),
-    ("ms_orth_svd", "orth_svd", "k_orth_coop (Cholesky-QR rounds, one cooperative launch) + k_jacobi_rows (Rayleigh-Ritz)", None, None, "alu"),
-    ("ms_search_rblocks", "search_rblocks", "k_gather_G, k_coef + k_tsgemm + k_rs (right blocks)", None, None, "tensor"),
-    ("ms_search_cond", "search_cond", "k_bgemm<.., ArPV, LdPB, EpPV> (conditionals, Z fused in the epilogue)", None,
-     "bytes_search_cond", "hbm"),
+    ("ms_orth_svd", "orth_svd", "k_orth_coop (Cholesky-QR rounds, one cooperative launch) + k_jacobi_rows (Rayleigh-Ritz)",
+     "flop_orth_svd", None, "alu"),
+    ("ms_search_rblocks", "search_rblocks", "k_gather_G, k_coef + k_tsgemm + k_rs (right blocks)", "flop_search_rblocks", None,
+     "tensor"),
+    ("ms_search_cond", "search_cond", "k_bgemm<.., ArPV, LdPB, EpPV> (conditionals, Z and the top-M prefilter fused in the epilogue)",
+     "flop_search_cond", "bytes_search_cond", "tensor"),
     ("ms_search_select", "search_select", "k_sel_hist (sample) + k_sel_prefilter + k_csel_* + bitonic (top-M)", None,
      "bytes_search_select", "hbm"),
     ("ms_tables", "tables", "k_tables", None, None, "hbm"),
 ]
+DFMA_PEAK_TFLOPS = 35.8   # plain FP64 FMA peak measured on this pool's B200 (profiles/r01_fp64_peak.md)
 
 
-def stored_traffic(workload_key):
-    """dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+def stored_traffic(config_index, stage):
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture OF THAT CONFIG
+    (profiles/r02_traffic.json, which names the capture command), or (None, reason)."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
     try:
         with open(p) as f:
-            return json.load(f).get(workload_key)
+            rec = json.load(f).get("configs[%d]:%s" % (config_index, stage))
     except (OSError, ValueError):
-        return None
+        rec = None
+    if rec is None:
+        return None, "no committed ncu --set full capture of this kernel at configs[%d]" % config_index
+    return rec["dram_bytes_per_launch"], rec.get("source", "profiles/r02_traffic.json")
+
+
+def stage_report(st, ci, fp64_peak, peaks, peak_src):
+    """Per-stage table (CUDA-event times and analytic FLOP / byte counters of tn_get_stats) and the roofline record of
+    the TIME-DOMINANT stage of this run."""
+    total = max(st["ms_contract"] + st["ms_search"] + st["ms_tables"], 1e-9)
+    stages = {}
+    for key, label, kern, fk, bk, bound in STAGES:
+        ms = st[key]
+        d = {"ms": round(ms, 3), "share": round(ms / total, 4), "kernel": kern, "bound": bound}
+        if fk and ms > 0 and st.get(fk, 0) > 0:
+            d["tflops"] = round(st[fk] / ms * 1e-9, 3)
+            d["frac_fp64_tensor" if bound != "alu" else "frac_fp64_alu"] = round(
+                st[fk] / ms * 1e-9 / (fp64_peak if bound != "alu" else DFMA_PEAK_TFLOPS), 4)
+        if bk and ms > 0:
+            d["gbs"] = round(st[bk] / ms * 1e-6, 1)
+            d["frac_hbm"] = round(st[bk] / ms * 1e-6 / peaks["hbm_gbs"], 4)
+        stages[label] = d
+    named = sum(st[k[0]] for k in STAGES)
+    stages["other"] = {"ms": round(total - named, 3), "share": round((total - named) / total, 4),
+                       "kernel": "maps on skinny operands outside the stage timers, copies, host round trips"}
+    dom = max(STAGES, key=lambda k: st[k[0]])
+    key, label, kern, fk, bk, bound = dom
+    ms_dom = st[key]
+    tr, tr_src = stored_traffic(ci, label)
+    launches = int(st["theta_apply_calls"]) if label == "theta_apply" else None
+    roof = {"bound": bound, "kernel": kern, "stage": label, "share_of_step": stages[label]["share"],
+            "traffic": tr, "traffic_source": tr_src, "launches_per_step": launches}
+    if bound in ("tensor", "alu") and fk:
+        ach = st[fk] / ms_dom * 1e-9 if ms_dom > 0 else 0.0
+        pk = fp64_peak if bound == "tensor" else DFMA_PEAK_TFLOPS
+        roof.update({"achieved": round(ach, 3), "peak": round(pk, 2), "unit": "TFLOP/s", "frac": round(ach / pk, 4),
+                     "algorithmic_flop_per_step": st[fk],
+                     "peak_source": ("tn_fp64_peak(): mma.sync m8n8k4 f64 (SASS DMMA) chain measured in this run "
+                                     "(MEASURED_PEAKS.json has no FP64 entry)" if bound == "tensor" else
+                                     "plain DFMA chain measured on this pool (profiles/r01_fp64_peak.md); the stage is "
+                                     "latency-bound, see DESIGN.md section 6")})
+        if bk:
+            roof["algorithmic_bytes_per_step"] = st[bk]
+            roof["achieved_gbs"] = round(st[bk] / ms_dom * 1e-6, 1) if ms_dom > 0 else None
+            roof["hbm_peak_gbs"] = peaks["hbm_gbs"]
+            roof["hbm_peak_source"] = peak_src
+        if launches:
+            roof["algorithmic_flop_per_launch"] = st[fk] / launches
+            roof["algorithmic_bytes_per_launch"] = st[bk] / launches if bk else None
+            roof["avg_launch_ms"] = round(ms_dom / launches, 4)
+    else:
+        ach = st[bk] / ms_dom * 1e-6 if (bk and ms_dom > 0) else 0.0
+        roof.update({"achieved": round(ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                     "frac": round(ach / peaks["hbm_gbs"], 4), "peak_source": peak_src,
+                     "algorithmic_bytes_per_step": st[bk] if bk else None})
+    return stages, roof
+
+
+def zspread(logzs):
+    """Z-spread diagnostic of PAPER.md:284, App. C: spread of log Z over the lattice transformations."""
+    import numpy as np
+    z = np.asarray(logzs, dtype=np.float64)
+    return {"log_z": [float(v) for v in z], "ptp": float(np.ptp(z)), "std": float(z.std()),
+            "rel_ptp": float(np.ptp(z) / abs(z.mean())) if z.size and z.mean() != 0 else None}
 
 
 def run_ours(args):
@@ -292,18 +429,34 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    inst, run = replica_instance(args.config, rank)           # one independent replica per rank
-    if args.transform:
-        import instances
-        inst = instances.transformed(inst, args.transform)
+    transform = int(args.transform)
+    if args.replicas == "transforms":
+        inst, run = instances.config(args.config)                 # ONE instance, rank r contracts map r
+        if inst.S == 3:
+            raise SystemExit("--replicas transforms: the Pegasus-shaped lattice admits only the identity map "
+                             "(DESIGN.md section 0, f3); use --config 1 or 4")
+        if world > 1:
+            transform = rank % 8
+    else:
+        inst, run = replica_instance(args.config, rank)           # one independent seeded replica per rank
+    base_inst = inst
+    if transform:
+        inst = instances.transformed(inst, transform)
     beta = run["beta"][args.beta_index]
-    D, sweeps, M = run["D"], run["sweeps"], run["M"]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    fp64_peak = tnb.tn_fp64_peak()
+    peaks, peak_src = measured_peaks()
 
-    def step(t):
-        t.set_beta(beta)
-        t.contract(D, sweeps)
-        return t.branch_and_bound(M)
+    def make_tn(ins):
+        t = tnb.TensorNetwork(ins)
+        if args.merge:
+            t.set_option(tnb.OPT_MERGE, 1)
+        return t
+
+    def step(t, b, r):
+        t.set_beta(b)
+        t.contract(r["D"], r["sweeps"])
+        return t.branch_and_bound(r["M"])
 
     def timed(fn, n):
         """n calls of fn, each bracketed by CUDA events on the launching stream; L2 flushed in between."""
@@ -318,24 +471,11 @@ def run_ours(args):
             tot += e0.elapsed_time(e1)
         return tot, outs
 
-    fp64_peak = tnb.tn_fp64_peak()
-    t = tnb.TensorNetwork(inst)
-    if args.merge:
-        t.set_option(tnb.OPT_MERGE, 1)
-    for _ in range(args.warmup):
-        step(t)
-    sampler = ClockSampler(local)
-    barrier()
-    if rank == 0:
-        sampler.start()
-    ms_total, outs = timed(lambda: step(t), args.steps)
-    barrier()
-    st = t.stats()                                               # stage timers of the last timed step
-    # the dominant kernel timed alone at this workload's largest apply shape (burst figure, warm L2 for small shapes)
-    alone = None
-    if rank == 0:
-        c0 = 1 << inst.n_s
-        nK = c0 * ((1 << (inst.n_s // 2)) if inst.S == 3 else 1)
+    def kernel_alone(t, ins, r):
+        """the dominant kernel timed alone at this workload's largest apply shape (burst figure)"""
+        c0 = 1 << ins.n_s
+        nK = c0 * ((1 << (ins.n_s // 2)) if ins.S == 3 else 1)
+        D = r["D"]
         mk, nk, sk = D * nK, c0 * D, min(D + 16, 96)
         alone = {"shape": "Tc[%d x %d] x [%d x %d]" % (mk, nk, nk, sk)}
         for op, nm in ((tnb.CHECK_GEMM_N, "N"), (tnb.CHECK_GEMM_T, "T")):
@@ -343,14 +483,27 @@ def run_ours(args):
             alone[nm] = {"ms": round(ms1, 4), "tflops": round(2.0 * mk * nk * sk / ms1 * 1e-9, 2),
                          "frac_fp64_tensor": round(2.0 * mk * nk * sk / ms1 * 1e-9 / fp64_peak, 4),
                          "gbs": round(8.0 * mk * nk / ms1 * 1e-6, 1)}
+        return alone
+
+    # ---- main arm: W warm-up steps, then K timed steps on the resident instance
+    t = make_tn(inst)
+    for _ in range(args.warmup):
+        step(t, beta, run)
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    ms_total, outs = timed(lambda: step(t, beta, run), args.steps)
+    barrier()
+    st = t.stats()                                               # stage timers of the last timed step
+    log_z = t.log_z()
+    alone = kernel_alone(t, inst, run) if rank == 0 else None
     t.close()
 
     # ---- e2e: host buffers in, host buffers out, tn_create / tn_destroy inside the timed region
     def e2e_step():
-        with tnb.TensorNetwork(inst) as tt:
-            if args.merge:
-                tt.set_option(tnb.OPT_MERGE, 1)
-            return step(tt)
+        with make_tn(inst) as tt:
+            return step(tt, beta, run)
     e2e_ms = None
     if not args.no_e2e:
         for _ in range(min(args.warmup, 2)):
@@ -366,71 +519,123 @@ def run_ours(args):
     ms_total = maxr(ms_total)
     if e2e_ms is not None:
         e2e_ms = maxr(e2e_ms)
+    states, E, logp, pd = outs
+    replicas = None
+    if args.replicas == "transforms":
+        # best-of-maps energy and the spread of log Z over the maps
+        if world > 1:
+            got = [None] * world
+            dist.all_gather_object(got, (transform, float(E.min()), float(log_z)))
+            replicas = {"mode": "one map per rank", "maps": [g[0] for g in got], "best_energy_per_map": [g[1] for g in got],
+                        "best_energy": min(g[1] for g in got), "z_spread": zspread([g[2] for g in got])}
+        elif rank == 0:
+            replicas = transforms_on_streams(tnb, instances, base_inst, run, beta, args, torch)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    states, E, logp, pd = outs
     K = args.steps
     ms_step = ms_total / K
     value = whole_job_value(ms_total, K, world)                  # seconds per instance over the whole job
     h2d = int(inst.edge_u.nbytes + inst.edge_v.nbytes + inst.J.nbytes + inst.h.nbytes + inst.cell_y.nbytes
               + inst.cell_x.nbytes + inst.sub.nbytes + inst.pos.nbytes)
-    d2h = int(M * inst.n_spins + 2 * 8 * M + 8 + 4)
-    peaks, peak_src = measured_peaks()
-
-    # ---- per-stage table and the roofline of the dominant kernel
-    stages = {}
-    for key, label, kern, fk, bk, bound in STAGES:
-        ms = st[key]
-        d = {"ms": round(ms, 3), "share": round(ms / max(st["ms_contract"] + st["ms_search"] + st["ms_tables"], 1e-9), 4),
-             "kernel": kern, "bound": bound}
-        if fk and ms > 0:
-            d["tflops"] = round(st[fk] / ms * 1e-9, 3)
-            d["frac_fp64_tensor"] = round(st[fk] / ms * 1e-9 / fp64_peak, 4)
-        if bk and ms > 0:
-            d["gbs"] = round(st[bk] / ms * 1e-6, 1)
-            d["frac_hbm"] = round(st[bk] / ms * 1e-6 / peaks["hbm_gbs"], 4)
-        stages[label] = d
-    sflop = st["flop_search"]
-    if st["ms_search"] > 0:
-        stages["search_total"] = {"ms": round(st["ms_search"], 3), "tflops": round(sflop / st["ms_search"] * 1e-9, 3)}
-    dom = STAGES[0]                                              # the FLOP carrier: Theta-core x skinny GEMMs (k_tsgemm)
-    ms_dom = st[dom[0]]
-    achieved = st[dom[3]] / ms_dom * 1e-9 if ms_dom > 0 else 0.0
-    tr = stored_traffic("configs[%d]" % args.config)
-    roofline = {"bound": "tensor", "achieved": round(achieved, 3), "peak": round(fp64_peak, 2), "unit": "TFLOP/s",
-                "frac": round(achieved / fp64_peak, 4), "traffic": tr["dram_bytes_per_launch"] if tr else None,
-                "kernel": dom[2], "stage": dom[1], "share_of_step": stages[dom[1]]["share"],
-                "launches_per_step": int(st["theta_apply_calls"]),
-                "peak_source": "tn_fp64_peak(): mma.sync m8n8k4 f64 (SASS DMMA) chain measured in this run "
-                               "(MEASURED_PEAKS.json has no FP64 entry; profiles/r01_fp64_peak.md); HBM peak %s = %.1f GB/s"
-                               % (peak_src, peaks["hbm_gbs"]),
-                "algorithmic_flop_per_step": st[dom[3]], "algorithmic_bytes_per_step": st["bytes_theta_apply"],
-                "achieved_gbs": round(st["bytes_theta_apply"] / ms_dom * 1e-6, 1) if ms_dom > 0 else None,
-                "kernel_alone": alone}
+    d2h = int(run["M"] * inst.n_spins + 2 * 8 * run["M"] + 8 + 4)
+    stages, roofline = stage_report(st, args.config, fp64_peak, peaks, peak_src)
+    roofline["kernel_alone"] = alone
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "l2": "flushed (256 MiB fill) between timed steps",
-            "config": {"workload": workload_name(args.config, inst, run, beta), "D": D, "M": M, "sweeps": sweeps,
-                       "beta": beta, "merge": bool(args.merge), "transform": int(args.transform), "parallelism": "replicas x%d" % world, "l2": "flush between steps"},
+            "config": config_record(args.config, inst, run, beta, args.merge, transform, world),
             "contract_rows_per_s": round(st["rows_contracted"] / max(st["ms_contract"], 1e-9) * 1e3, 3),
             "contract_ms": round(st["ms_contract"], 3), "search_ms": round(st["ms_search"], 3),
-            "best_energy": float(E.min()), "n_states": int(len(E)), "log_p_discarded": float(pd),
-            "gpu_launches": int(st["kernel_launches"]) * K, "stages": stages, "roofline": roofline, "clocks": clocks,
+            "best_energy": float(E.min()), "log_z": float(log_z), "n_states": int(len(E)), "log_p_discarded": float(pd),
+            "min_sigma_rel": st["min_sigma_rel"], "negative_u": int(st["negative_u"]),
+            "svd_unconverged": int(st["svd_unconverged"]), "merge_fallback_cells": int(st["merge_fallback_cells"]),
+            "gpu_launches": int(st["kernel_launches"]) * K, "launches_per_step": int(st["kernel_launches"]),
+            "stages": stages, "roofline": roofline, "clocks": clocks,
             "fp64_tensor_peak_tflops": round(fp64_peak, 2)}
+    if replicas is not None:
+        line["replicas"] = replicas
     if "E0" in inst:
         line["planted"] = diversity_report(inst, states, E)
     if e2e_ms is not None:
         line["e2e"] = {"value": whole_job_value(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h}
+    # ---- the north_star target workload: ONE timed step of configs[3] (N = 5400, D = 64, M = 1024, 3 passes, beta = 2)
+    if world == 1 and not args.no_headline and args.config != 3:
+        line["headline"] = headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local)
     if world == 1 and not args.no_cpu_baseline:
-        tm, est, desc = oracle_sample(inst, run, beta)
-        line["cpu_baseline"] = {"value": est, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": desc,
-                                "sample_seconds": round(tm, 2)}
+        smp = OracleSample(base_inst if not transform else inst, run, beta, ORACLE_SAMPLE[args.config])
+        tm = smp.step()
+        line["cpu_baseline"] = {"value": smp.estimate(), "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+                                "sample": smp.describe(), "extrapolated": not smp.whole, "sample_seconds": round(tm, 2)}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local):
+    """One timed step (after a tables-only warm-up of the handle) of BASELINE.json configs[3] at beta = 2: the
+    ~5400-spin D = 64, M = 1024 instance of north_star, with its own stage table, roofline and clocks.  A single step:
+    `steps` = 1, `warmup` = 0 -- a record inside the driver-observed run, not the line's `value`."""
+    ci, bi = 3, 1
+    inst, run = instances.config(ci)
+    beta = run["beta"][bi]
+    sampler = ClockSampler(local)
+    t = tnb.TensorNetwork(inst)
+    if args.merge:
+        t.set_option(tnb.OPT_MERGE, 1)
+    sampler.start()
+    ms, outs = timed(lambda: step(t, beta, run), 1)
+    st = t.stats()
+    lz = t.log_z()
+    t.close()
+    clocks = sampler.stop()
+    states, E, logp, pd = outs
+    stages, roofline = stage_report(st, ci, fp64_peak, peaks, peak_src)
+    return {"config": config_record(ci, inst, run, beta, args.merge, 0, 1), "steps": 1, "warmup": 0,
+            "value": ms * 1e-3, "unit": UNIT, "ms_per_step": ms, "contract_ms": round(st["ms_contract"], 3),
+            "search_ms": round(st["ms_search"], 3), "best_energy": float(E.min()), "log_z": float(lz),
+            "log_p_discarded": float(pd), "min_sigma_rel": st["min_sigma_rel"], "negative_u": int(st["negative_u"]),
+            "svd_unconverged": int(st["svd_unconverged"]), "launches_per_step": int(st["kernel_launches"]),
+            "peak_device_bytes": int(st["bytes_device"]), "stages": stages, "roofline": roofline, "clocks": clocks}
+
+
+def transforms_on_streams(tnb, instances, inst, run, beta, args, torch):
+    """N = 1: the 8 lattice transformations of ONE instance as concurrent replicas ("all 8 ...
+    transformations"), one handle per map, `--streams` CUDA streams with one host thread each (a handle is
+    single-threaded, distinct handles are independent).  Reports best-of-8, the log Z spread and the wall time of the
+    whole batch next to the sum of the per-map device times."""
+    import numpy as np
+    ns = max(1, min(8, int(args.streams)))
+    streams = [torch.cuda.Stream() for _ in range(ns)]
+    res = [None] * 8
+
+    def work(k):
+        with torch.cuda.stream(streams[k]):
+            for tmap in range(k, 8, ns):
+                with tnb.TensorNetwork(instances.transformed(inst, tmap)) as t:   # binds the thread's current stream
+                    if args.merge:
+                        t.set_option(tnb.OPT_MERGE, 1)
+                    t.set_beta(beta)
+                    t.contract(run["D"], run["sweeps"])
+                    lz = t.log_z()
+                    states, E, logp, pd = t.branch_and_bound(run["M"])
+                    st = t.stats()
+                res[tmap] = (float(E.min()), float(lz), st["ms_contract"] + st["ms_search"] + st["ms_tables"])
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    th = [threading.Thread(target=work, args=(k,)) for k in range(ns)]
+    for x in th:
+        x.start()
+    for x in th:
+        x.join()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    return {"mode": "8 maps on %d stream(s), one GPU" % ns, "maps": list(range(8)),
+            "best_energy_per_map": [r[0] for r in res], "best_energy": min(r[0] for r in res),
+            "z_spread": zspread([r[1] for r in res]), "batch_wall_s": round(wall, 4),
+            "sum_of_device_ms": round(sum(r[2] for r in res), 3)}
 
 
 if __name__ == "__main__":

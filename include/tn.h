@@ -116,6 +116,10 @@ typedef struct {
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
   int64_t merge_fallback_cells; /* cells at which TN_OPT_MERGE could not merge (merge buffers too small at every threshold
                                 tried) and the selection ran unmerged; 0 = every cell followed Fig. 3(d)          */
+  double flop_orth_svd;      /* algorithmic FLOP of the orthonormalisations: 2 Cholesky-QR rounds of 4 m k^2 each per call
+                                (Gram + apply; the rounds actually run are decided on the device, 1..5)             */
+  double flop_search_rblocks;/* algorithmic FLOP of the right-block GEMMs (part of flop_search)                      */
+  double flop_search_cond;   /* algorithmic FLOP of the conditional GEMMs LG and V (part of flop_search)             */
 } tn_stats;
 
 /* tn_create: validates the geometry and copies the instance to the device.

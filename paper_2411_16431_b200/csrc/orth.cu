@@ -443,6 +443,7 @@ void orth_columns_jacobi(tn_handle* h, double* Y, i64 m, int k, int passes);   /
 
 void orth_columns(tn_handle* h, double* Y, i64 m, int k, int passes) {
   if (m <= 0 || k <= 0) return;
+  h->st.flop_orth_svd += 2.0 * 4.0 * (double)m * k * k;
   if (k <= 16) run_orth<2>(h, Y, m, k, passes);
   else if (k <= 32) run_orth<4>(h, Y, m, k, passes);
   else if (k <= 48) run_orth<6>(h, Y, m, k, passes);

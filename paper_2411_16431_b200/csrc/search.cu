@@ -805,6 +805,7 @@ void build_G(tn_handle* h, const MpsTensor& S, const MpsTensor* Q, RowTab& rt) {
     g.nsplit = 1;
     gemm_general(h, g);
     h->st.flop_search += 2.0 * rt.npp * rt.Dl * (double)rt.Dr * S.dr;
+    h->st.flop_search_rblocks += 2.0 * rt.npp * rt.Dl * (double)rt.Dr * S.dr;
   } else {
     rt.Dl = S.dl; rt.Dr = S.dr; rt.npp = S.p;
     rt.G = h->dalloc<double>((size_t)rt.npp * rt.Dl * rt.Dr);
@@ -885,6 +886,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       {   // H[(m,t)][(b',b'')] = sum_{(b,cl)} coef[(b,cl)][(m,t)] G[(Pd b, Po cl)][(b',b'')]
         const int Mg = (int)DD, Ng = nb * c.nT, Kg = c.nB * c.nCl;
         h->st.flop_search += 2.0 * Mg * (double)Ng * Kg;
+        h->st.flop_search_rblocks += 2.0 * Mg * (double)Ng * Kg + 2.0 * nb * (double)Dl * c.nA * Dr +
+                                     2.0 * nb * (double)Dl * c.bh_rows * c.nA;
         bool done = false;
         if ((DD & 1) == 0 && (Ng & 1) == 0) {
           // both operands materialised row-major in the reduction index, then the streaming GEMM (tsgemm.cu)
@@ -937,10 +940,12 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         k_gemm<64, 64, 16, 2, 2, true, true, LdLv, LdGj, StPlain><<<grid, 128, 0, h->stream>>>(nb, Ng, Dl, 1, a, b, e);
         TN_LAUNCH_CHECK(h);
         h->st.flop_search += 2.0 * nb * (double)Ng * Dl;
+        h->st.flop_search_cond += 2.0 * nb * (double)Ng * Dl;
       }
       {   // V[m][(b,cl)][a]
         int Mg = c.nB * c.nCl, Ng = c.nA;
         h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
+        h->st.flop_search_cond += 2.0 * nb * (double)Mg * Ng * Dr;
         h->st.bytes_search_cond += 8.0 * nb * (double)per_m;
         DBuf<double> cs(h, (size_t)nb * c.nA);
         k_colscale<<<cdiv((i64)nb * c.nA, 256), 256, 0, h->stream>>>(c.BhS, c.wA, hrow.p, nb, c.nA, cs.p);

@@ -75,6 +75,12 @@ def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=Fa
         assert abs(lz - ref["log_z"]) <= tol * abs(ref["log_z"]), (lz, ref["log_z"])
         states, E, logp, pd = t.branch_and_bound(M)
         st = t.stats()
+    check_lists(inst, ref, states, E, logp, pd, tol)
+    return st
+
+
+def check_lists(inst, ref, states, E, logp, pd, tol):
+    """Final lists of the CUDA path against the oracle's (`ref`: logp, states, log_pd): element by element."""
     n = ref["logp"].size
     assert states.shape[0] == n
     assert np.allclose(logp, ref["logp"], rtol=tol, atol=0), np.abs(logp - ref["logp"]).max()
@@ -102,7 +108,6 @@ def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=Fa
         assert abs(pd - ref["log_pd"]) <= 10 * tol * abs(ref["log_pd"]), (pd, ref["log_pd"])
     else:
         assert pd == ref["log_pd"]
-    return st
 
 
 EXACT = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, M)
