@@ -207,9 +207,78 @@ def truncate_rank(s, D, gap_guard=True):
     return max(k, 1)
 
 
-def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
+_M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
+
+
+def hash_uniform(seed, p, g, c):
+    """Counter-based uniform(-1, 1) numbers Omega[(p', gamma), col] for the randomized SVD: SplitMix64's finaliser
+    (public-domain, S. Vigna) of the counter seed * 0x100000001B3 + ((p' * 4096 + gamma) * 1024 + col).  The numbers the
+    method draws are an INPUT of the algorithm (PAPER.md:169-177 'randomized SVD'); the CUDA path implements the same
+    generator, indexed by (p', gamma, col) and not by any memory layout."""
+    pp, gg, cc = np.meshgrid(np.arange(p, dtype=np.uint64), np.arange(g, dtype=np.uint64),
+                             np.arange(c, dtype=np.uint64), indexing="ij")
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed) * np.uint64(0x100000001B3) + ((pp * np.uint64(4096) + gg) * np.uint64(1024) + cc)
+        z = z + np.uint64(0x9E3779B97F4A7C15)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        z = z ^ (z >> np.uint64(31))
+    u = (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+    return (2.0 * u - 1.0).reshape(p * g, c)
+
+
+def randomized_svd(Th, pu, g, ks, iters, seed):
+    """Truncated randomized SVD of Theta (refs [43, 44] = randomized range finder with `iters`
+    subspace iterations, matrix-free: only Theta x block and Theta^T x block are used):
+        Om <- orth(Omega);  repeat iters times:  Y <- orth(Theta Om);  Z <- Theta^T Y;  Om <- orth(Z);
+        B = Om^T Z = W diag(s) X^T  (small SVD);   right vectors V = Om W, Ritz values s.
+    Returns (V [n, ks], s [ks]).  The connector is Theta V (exact for the chosen V), computed by the caller."""
+    Om, _ = np.linalg.qr(hash_uniform(seed, pu, g, ks))
+    Z = None
+    for _ in range(max(1, iters)):
+        Y, _ = np.linalg.qr(Th @ Om)
+        Z = Th.T @ Y
+        Om, _ = np.linalg.qr(Z)
+    W, sv, _ = np.linalg.svd(Om.T @ Z)
+    return Om @ W, sv
+
+
+def truncate_mps(N, D, gap_guard=True, min_sigma=None):
+    """Second step of the two-step truncation 2 chi -> chi ('targeting 2 chi singular values with
+    randomized SVD, which, after variational refinement, are further truncated to the target chi singular values'):
+    canonical MPS compression -- left-canonicalise, then SVD every bond right -> left keeping <= D values.
+    Returns (tensors with unit norm, log of the norm removed by the truncation)."""
+    N, r_last = left_canonicalize(N)
+    n = len(N)
+    N[n - 1] = N[n - 1] * r_last
+    for j in range(n - 1, 0, -1):
+        dl, p, dr = N[j].shape
+        U, sv, Vt = np.linalg.svd(N[j].reshape(dl, p * dr), full_matrices=False)
+        k = truncate_rank(sv, D, gap_guard)
+        if min_sigma is not None and k < np.count_nonzero(sv > RANK_TOL * sv[0]):
+            min_sigma.append(sv[k - 1] / sv[0])
+        N[j] = Vt[:k].reshape(k, p, dr)
+        N[j - 1] = np.einsum("apb,bc->apc", N[j - 1], U[:, :k] * sv[:k])
+    nrm = np.linalg.norm(N[0])
+    N[0] = N[0] / nrm
+    return N, float(np.log(nrm))
+
+
+def compress(positions, A, D, sweeps, gap_guard=True, stats=None, schedule=0, sweep_range=2, svd_mode=0,
+             rsvd_iters=2, oversample=16, two_step=False, seed=None):
     """R_y = compress(T_y R_{y+1}; D, sweeps).  A: tensors of R_{y+1} (any gauge).
     Returns (tensors of R_y with unit norm, log of the norm removed).
+
+    Options (readings S21-S23; the defaults are the parity definition S1-S4):
+      schedule   0: whole zipper, then `sweeps` passes (the paper's variant (ii), PAPER.md:179);
+                 1: the paper's preferred schedule: every zipper step is followed by a variational sweep
+                    of the instantaneous stage of the zipper over the `sweep_range` positions to the right of the
+                    centre and back ('limit the range ... to a few tensors in the vicinity of the instantaneous
+                    centre'), then `sweeps` global passes as before.
+      svd_mode   0: converged truncated SVD (S1; LAPACK here); 1: randomized SVD with `rsvd_iters` subspace iterations
+                 and `oversample` extra columns, random block from hash_uniform(seed[0]++).
+      two_step   zipper and passes at bond 2 D, then truncate_mps to D.
+      seed       one-element list: running count of truncated SVDs of this contraction (the random block's seed).
 
     Range (reading S19): the norm of a row is exp(-O(beta N_row)) and under/overflows fp64 on
     the large lattices, so every environment is kept at O(1) and the positive scale removed from it is
@@ -218,26 +287,70 @@ def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
     Renv[j] / Lenv[j].  Positive rescalings change nothing but the bookkeeping."""
     n = len(positions)
     A, r_last = left_canonicalize(A)
+    Dz = 2 * D if (two_step and D > 0) else D       # bond kept by the zipper and the passes
+    if seed is None:
+        seed = [1]
     Renv = [None] * n
     lsR = [0.0] * n
     Renv[n - 1] = np.full((1, 1, 1), r_last)       # trivial unity connector x the folded norm
     N = [None] * n
+    Lenv = [None] * n
     min_sigma = []
     ls0 = 0.0
     for j in range(n - 1, -1, -1):                  # C-2 zipper, right -> left
         pos = positions[j]
         Th = pos.theta(A[j], Renv[j])
-        U, s, Vt = np.linalg.svd(Th, full_matrices=False)
-        k = truncate_rank(s, D, gap_guard)
+        g = Renv[j].shape[0]
+        if svd_mode == 1 and D > 0 and min(Th.shape) > Dz:
+            ks = min(min(Dz, min(Th.shape)) + oversample, min(Th.shape))
+            V, s = randomized_svd(Th, pos.pu, g, ks, rsvd_iters, seed[0])
+            k = truncate_rank(s, Dz, gap_guard)
+            Vk = V[:, :k]
+            N[j] = Vk.T.reshape(k, pos.pu, g)
+            scale = s[0] if s[0] > 0 else 1.0
+            Cn = ((Th @ Vk) / scale).reshape(A[j].shape[0], pos.wl, k)
+        else:
+            U, s, Vt = np.linalg.svd(Th, full_matrices=False)
+            k = truncate_rank(s, Dz, gap_guard)
+            N[j] = Vt[:k].reshape(k, pos.pu, g)
+            scale = s[0] if s[0] > 0 else 1.0
+            Cn = (U[:, :k] * (s[:k] / scale)).reshape(A[j].shape[0], pos.wl, k)
+        seed[0] += 1
         min_sigma.append(s[k - 1] / s[0] if s[0] > 0 else 0.0)
-        N[j] = Vt[:k].reshape(k, pos.pu, Renv[j].shape[0])
-        scale = s[0] if s[0] > 0 else 1.0
-        Cn = (U[:, :k] * (s[:k] / scale)).reshape(A[j].shape[0], pos.wl, k)
         if j > 0:
             Renv[j - 1] = Cn.transpose(2, 1, 0)
             lsR[j - 1] = lsR[j] + np.log(scale)
         else:
             ls0 = lsR[0] + np.log(scale)
+        if schedule == 1 and D > 0 and sweep_range > 0 and j < n - 1:
+            # ---- PAPER.md:177: variational sweep of the instantaneous stage of the zipper, positions j .. kmax.
+            # The block [connector . N_j ... N_kmax ...] approximates (A_j W_j) ... (A_{n-1} W_{n-1}) with its left
+            # legs (old bond, MPO bond) open; an orthonormal basis Q of the connector's range on those legs plays the
+            # left environment of position j (DESIGN.md reading S21).
+            kmax = min(n - 1, j + sweep_range)
+            al, wl = A[j].shape[0], pos.wl
+            Q, _ = np.linalg.qr(Cn.reshape(al * wl, k))
+            Lenv[j] = Q.reshape(al, wl, Q.shape[1]).transpose(2, 1, 0)
+            for q in range(j, kmax):                                   # left -> right
+                N[q] = positions[q].update(Lenv[q], A[q], Renv[q])
+                g1, p1, g2 = N[q].shape
+                Qq, _ = np.linalg.qr(N[q].reshape(g1 * p1, g2))
+                N[q] = Qq.reshape(g1, p1, Qq.shape[1])
+                E = positions[q].env_left(Lenv[q], A[q], N[q])
+                Lenv[q + 1] = E / np.linalg.norm(E)
+            for q in range(kmax, j - 1, -1):                           # right -> left, back to the zipper's centre
+                N[q] = positions[q].update(Lenv[q], A[q], Renv[q])
+                g1, p1, g2 = N[q].shape
+                Qq, _ = np.linalg.qr(N[q].reshape(g1, p1 * g2).T)
+                N[q] = Qq.T.reshape(Qq.shape[1], p1, g2)
+                E = positions[q].env_right(Renv[q], A[q], N[q])
+                nE = np.linalg.norm(E)
+                if q > 0:
+                    Renv[q - 1] = E / nE
+                    lsR[q - 1] = lsR[q] + np.log(nE)
+                else:
+                    Cn = (E / nE).transpose(2, 1, 0)
+                    ls0 = lsR[0] + np.log(nE)
     assert Cn.shape == (1, 1, 1)
     centre = 0
     N[0] = N[0] * Cn[0, 0, 0]
@@ -278,6 +391,10 @@ def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
                 centre = 0
     nrm = np.linalg.norm(N[centre])
     N[centre] = N[centre] / nrm
+    ln_trunc = 0.0
+    if two_step and D > 0:
+        N, ln_trunc = truncate_mps(N, D, gap_guard, min_sigma)
+    log_centre += ln_trunc
     if stats is not None:
         stats.setdefault("min_sigma", []).append(min(min_sigma))
         stats.setdefault("pass_norms", []).append(norms)
@@ -285,13 +402,15 @@ def compress(positions, A, D, sweeps, gap_guard=True, stats=None):
     return N, float(np.log(nrm) + log_centre)
 
 
-def contract(model, D, sweeps, gap_guard=True, stats=None):
+def contract(model, D, sweeps, gap_guard=True, stats=None, **options):
     """Boundary MPS R_y for y = Ly .. 1 (R_0 is never needed: log Z comes from the first cell's
-    normaliser in the search, C-6).  Returns {y: tensors}, {y: log-norm}."""
+    normaliser in the search, C-6).  Returns {y: tensors}, {y: log-norm}.  `options`: see compress."""
     R = {model.Ly: trivial_mps(model)}
     lognorm = {model.Ly: 0.0}
+    seed = [1]                                      # running count of truncated SVDs (seed of the random blocks)
     for y in range(model.Ly - 1, 0, -1):
-        R[y], lognorm[y] = compress(row_positions(model, y), R[y + 1], D, sweeps, gap_guard, stats)
+        R[y], lognorm[y] = compress(row_positions(model, y), R[y + 1], D, sweeps, gap_guard, stats, seed=seed,
+                                    **options)
     return R, lognorm
 
 

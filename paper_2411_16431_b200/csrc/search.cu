@@ -1080,7 +1080,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         }
         // The threshold is lowered (/ 64) while fewer than M + 1 boundaries lie above it and raised again (geometric
         // bisection) when more candidates than the merge buffers hold lie above it.
-        const int max_attempts = 16;
+        const int max_attempts = 40;
         double thr_few = -1.0, thr_many = -1.0;          // last thresholds with too few groups / too many survivors
         for (int attempt = 0; !seg && attempt < max_attempts; attempt++) {
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
@@ -1090,8 +1090,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           n1 = d2h(h, count.p);
           if (n1 > mcap) {                               // too many survivors for the merge buffers
             thr_many = thr;
-            if (thr_few <= 0.0 || !(thr_few > thr_many * (1.0 + 1e-9))) break;
-            thr = std::sqrt(thr_few) * std::sqrt(thr_many);
+            if (thr_few > 0.0 && !(thr_few > thr_many * (1.0 + 1e-9))) break;   // the two bounds met: no threshold fits
+            if (thr <= 0.0) break;                                              // every positive entry, still too many
+            thr = thr_few > 0.0 ? std::sqrt(thr_few) * std::sqrt(thr_many) : thr * 8.0;
             continue;
           }
           if (n1 == 0 && thr == 0.0) break;

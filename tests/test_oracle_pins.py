@@ -515,3 +515,121 @@ def test_merge_groups_are_boundaries():
     for k, s_ in zip(key.tolist(), score.tolist()):
         best[k] = max(best.get(k, -np.inf), s_)
     assert all(score[i] == best[key[i]] for i in surv)
+
+
+# ---------------------------------------------------------------- f2: paper-preferred schedule, randomized SVD, 2 chi -> chi
+def test_hash_uniform_is_splitmix64():
+    """The random block of the randomized SVD comes from SplitMix64's output function (public-domain reference
+    implementation by S. Vigna; its first output for state 0 is the published test vector 0xE220A8397B1DCDAF) applied
+    to a counter made of (seed, p', gamma, column): reproducible, layout-free, uniform on (-1, 1)."""
+    u0 = mps.hash_uniform(0, 1, 1, 1)[0, 0]
+    assert u0 == 2.0 * ((0xE220A8397B1DCDAF >> 11) * (1.0 / 9007199254740992.0)) - 1.0
+    # counter arithmetic against plain Python integers (instances.SplitMix64 is the same generator, written with ints)
+    seed, p, g, c = 7, 3, 5, 4
+    U = mps.hash_uniform(seed, p, g, c)
+    for (pp, gg, cc) in ((0, 0, 0), (2, 4, 3), (1, 0, 2)):
+        ctr = (seed * 0x100000001B3 + ((pp * 4096 + gg) * 1024 + cc)) & ((1 << 64) - 1)
+        ref = instances.SplitMix64(ctr)               # state = counter: next_u64 adds the golden gamma and mixes
+        assert U[pp * g + gg, cc] == 2.0 * ((ref.next_u64() >> 11) * (1.0 / 9007199254740992.0)) - 1.0
+    big = mps.hash_uniform(3, 64, 32, 48)
+    assert np.all(np.abs(big) < 1) and abs(big.mean()) < 5e-3 and abs(big.var() - 1 / 3) < 5e-3
+    assert np.array_equal(big, mps.hash_uniform(3, 64, 32, 48)) and not np.array_equal(big, mps.hash_uniform(4, 64, 32, 48))
+
+
+def test_randomized_svd_ritz_values_interlace_and_converge():
+    """Randomized range finder + subspace iteration (refs [43, 44]): the returned V is orthonormal, the
+    Ritz values never exceed the true singular values (Cauchy interlacing for a compression of Theta), approach them
+    from below as the number of iterations grows, and with enough iterations the retained subspace is LAPACK's."""
+    rng = np.random.default_rng(5)
+    pu, g, m = 12, 6, 90
+    U, _ = np.linalg.qr(rng.normal(size=(m, pu * g)))
+    W, _ = np.linalg.qr(rng.normal(size=(pu * g, pu * g)))
+    sv = 0.7 ** np.arange(pu * g)
+    Th = (U * sv) @ W.T
+    k, ks = 8, 8 + 6
+    prev = None
+    for iters in (1, 2, 4, 40):
+        V, s = mps.randomized_svd(Th, pu, g, ks, iters, seed=11)
+        assert np.abs(V.T @ V - np.eye(ks)).max() < 1e-12
+        assert np.all(s <= sv[:ks] * (1 + 1e-12))
+        if prev is not None:
+            assert np.all(s[:k] >= prev[:k] * (1 - 1e-12))
+        prev = s
+    assert np.allclose(s[:k], sv[:k], rtol=1e-10)
+    P = V[:, :k] @ V[:, :k].T
+    assert np.abs(P - W[:, :k] @ W[:, :k].T).max() < 1e-8
+    # one iteration already obeys the range-finder error bound in the spectral norm up to a modest factor
+    V1, _ = mps.randomized_svd(Th, pu, g, ks, 1, seed=11)
+    err = np.linalg.norm(Th - Th @ V1 @ V1.T, 2)
+    assert sv[ks] * (1 - 1e-12) <= err <= 10 * sv[ks]
+
+
+def test_truncate_mps_is_canonical_compression():
+    """Second step of 2 chi -> chi: D >= every bond leaves the state unchanged; a real cut keeps unit norm, bonds <= D,
+    loses at most sqrt(sum over bonds of the discarded Schmidt weight) (the textbook bound of canonical truncation) and
+    never beats the single-cut Eckart-Young optimum."""
+    rng = np.random.default_rng(9)
+    dims = [(1, 3, 6), (6, 4, 6), (6, 3, 5), (5, 2, 1)]
+    T = [rng.normal(size=d) * (0.5 ** np.arange(d[2]))[None, None, :] for d in dims]
+    v = mps.mps_to_dense(T)
+    nv = np.linalg.norm(v)
+    T[0] = T[0] / nv
+    v = v / nv
+    same, ln0 = mps.truncate_mps(T, 8)
+    assert abs(1 - abs((mps.mps_to_dense(same) * v).sum())) < 1e-12 and abs(ln0) < 1e-12
+    for D in (2, 3):
+        N, ln = mps.truncate_mps(T, D, gap_guard=False)
+        w = mps.mps_to_dense(N)
+        assert abs(np.linalg.norm(w) - 1) < 1e-12 and max(t.shape[2] for t in N) <= D
+        fid = abs((w * v).sum())
+        disc, cap = 0.0, 1.0
+        for cut in range(1, len(dims)):
+            sv = np.linalg.svd(v.reshape(int(np.prod(v.shape[:cut])), -1), compute_uv=False)
+            disc += (sv[D:] ** 2).sum()
+            cap = min(cap, np.sqrt((sv[:D] ** 2).sum()))
+        assert fid <= cap + 1e-12
+        assert np.linalg.norm(w * np.exp(ln) - v) <= np.sqrt(disc) * (1 + 1e-9) + 1e-12
+        assert ln <= 1e-12
+
+
+def test_interleaved_schedule_beats_plain_zipper():
+    """a variational sweep after every zipper step is the paper's preferred schedule, 'a full zipper
+    sweep first ... resulting in worse performance'.  On the P11 / P13 row problem: with no global pass the interleaved
+    schedule has a higher fidelity with the exact MPO x MPS product than the plain zipper, a longer sweep range does
+    not hurt, every variant respects the Eckart-Young cap, unit norm and bond <= D, and the two-step 2 chi -> chi
+    truncation is at least as good as the one-step zipper."""
+    m, Rex = _row_problem()
+    y = 1
+    pos = mps.row_positions(m, y)
+    exact = mps.mpo_mps_dense(pos, Rex[y + 1])
+    nex = np.linalg.norm(exact)
+    v = exact / nex
+    dims = v.shape
+
+    def infid(D, sweeps, **kw):
+        N, ln = mps.compress(pos, Rex[y + 1], D, sweeps, **kw)
+        w = mps.mps_to_dense(N)
+        assert abs(np.linalg.norm(w) - 1) < 1e-12 and max(t.shape[2] for t in N) <= D
+        return 1 - abs((w * v).sum()), ln
+
+    for D in (2, 3):
+        cap = 1.0
+        for cut in range(1, len(dims)):
+            sv = np.linalg.svd(v.reshape(int(np.prod(dims[:cut])), -1), compute_uv=False)
+            cap = min(cap, float(np.sqrt((sv[:D] ** 2).sum())))
+        z0, _ = infid(D, 0)
+        i1, _ = infid(D, 0, schedule=1, sweep_range=1)
+        i3, _ = infid(D, 0, schedule=1, sweep_range=3)
+        t0, _ = infid(D, 0, two_step=True)
+        assert i1 < 0.2 * z0 and i3 <= i1 * (1 + 1e-9) and t0 < z0
+        for f in (z0, i1, i3, t0):
+            assert f >= (1 - cap) - 1e-12
+        # with global passes on top every schedule lands at the same local optimum to the size of the truncation error
+        z2, lz2 = infid(D, 2)
+        i2, li2 = infid(D, 2, schedule=1, sweep_range=1)
+        assert abs(i2 - z2) <= 0.5 * z2 and abs(li2 - lz2) <= 10 * z2
+    # range 0 is the plain zipper; schedule 1 with exact D changes nothing
+    assert infid(3, 1, schedule=1, sweep_range=0)[0] == infid(3, 1)[0]
+    N0, l0 = mps.compress(pos, Rex[y + 1], 0, 0)
+    N1, l1 = mps.compress(pos, Rex[y + 1], 0, 0, schedule=1, svd_mode=1, two_step=True)
+    assert abs(1 - abs((mps.mps_to_dense(N0) * mps.mps_to_dense(N1)).sum())) < 1e-12 and abs(l0 - l1) < 1e-12
