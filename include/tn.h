@@ -77,6 +77,20 @@ enum {
   TN_OPT_MERGE_CAP = 10,  /* capacity of the merge buffers (survivors above the threshold resp. possible boundaries of a
                              cell; default 2^20, range 1..2^24).  A cell whose candidates fit neither route is selected
                              WITHOUT merging and counted in tn_stats.merge_fallback_cells                      */
+  /* ---- f2: the paper's preferred contraction schedule (Sec. III B 2; readings S21-S23).
+     The defaults (0) are the parity definition S1-S4: converged SVD, whole zipper first, then the passes. */
+  TN_OPT_SCHEDULE = 11,   /* 0 (default): whole zipper, then `sweeps` passes (the paper's variant (ii));
+                             1: every zipper step is followed by a variational sweep of the instantaneous stage of the
+                             zipper over TN_OPT_SWEEP_RANGE positions right of the centre and back, then `sweeps`
+                             global passes ("each step of the zipper procedure is followed by a sweep")  */
+  TN_OPT_SWEEP_RANGE = 12,/* positions to the right of the zipper's centre inside the local sweep (default 2; "a few
+                             tensors in the vicinity of the instantaneous centre")                              */
+  TN_OPT_SVD_MODE = 13,   /* 0 (default): converged truncated SVD (reading S1); 1: truncated randomized SVD with a fixed
+                             number of subspace iterations (refs [43, 44]): seeded, counter-based random
+                             block, reproducible run to run -- fewer Theta applies, accuracy left to the passes   */
+  TN_OPT_RSVD_ITERS = 14, /* subspace iterations of the randomized SVD (default 2)                             */
+  TN_OPT_TWO_STEP = 15,   /* 0 (default) / 1: zipper and passes at bond 2 D, then canonical truncation to D
+                             ("targeting 2 chi singular values ... further truncated to the target chi") */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */

@@ -14,6 +14,7 @@ EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_op
                     "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 OPT_MERGE_CAP = 10
+OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
 
 
 class TnError(RuntimeError):

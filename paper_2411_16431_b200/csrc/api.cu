@@ -245,6 +245,19 @@ int tn_set_option(tn_handle* h, int32_t key, double v) {
     case TN_OPT_SVD_CHEB: h->svd_cheb = v != 0.0; break;
     case TN_OPT_SVD_LOCK: h->svd_lock = v != 0.0; break;
     case TN_OPT_MERGE: h->merge = v != 0.0; break;
+    case TN_OPT_SCHEDULE:
+      if (v != 0.0 && v != 1.0) tn_throw(TN_ERR_ARG, "schedule must be 0 or 1");
+      h->schedule = (int)v; break;
+    case TN_OPT_SWEEP_RANGE:
+      if (v < 0 || v > 1e6) tn_throw(TN_ERR_ARG, "sweep range must be >= 0");
+      h->sweep_range = (int)v; break;
+    case TN_OPT_SVD_MODE:
+      if (v != 0.0 && v != 1.0) tn_throw(TN_ERR_ARG, "svd mode must be 0 or 1");
+      h->svd_mode = (int)v; break;
+    case TN_OPT_RSVD_ITERS:
+      if (v < 1 || v > 100) tn_throw(TN_ERR_ARG, "randomized SVD iterations must be in 1..100");
+      h->rsvd_iters = (int)v; break;
+    case TN_OPT_TWO_STEP: h->two_step = v != 0.0; break;
     case TN_OPT_MERGE_CAP:
       if (v < 1 || v > (double)(1 << 24)) tn_throw(TN_ERR_ARG, "merge cap must be in 1..2^24");
       h->merge_cap = (i64)v; break;
@@ -274,7 +287,7 @@ int tn_contract(tn_handle* h, int32_t D, int32_t sweeps) {
   if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
   if (!h->have_beta) tn_throw(TN_ERR_STATE, "tn_contract before tn_set_beta");
   if (sweeps < 0) tn_throw(TN_ERR_ARG, "sweeps < 0");
-  if (D > 1008) tn_throw(TN_ERR_ARG, "D > 1008 not supported");
+  if (D > 1008 || (h->two_step && D > 504)) tn_throw(TN_ERR_ARG, "D > 1008 (504 with TN_OPT_TWO_STEP) not supported");
   DeviceGuard dg(h);
   const unsigned long long mark = h->serial;
   try {

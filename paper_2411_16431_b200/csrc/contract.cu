@@ -552,11 +552,118 @@ void svd_trunc(Ctx& cx, const ThetaOp& op, int chi, int ks, double* Vz, double* 
   TN_CUDA(cudaMemcpyAsync(sig0_out, sig.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
 }
 
+// Truncated randomized SVD (TN_OPT_SVD_MODE = 1, refs [43, 44]): `iters` subspace iterations from a
+// seeded, counter-based random block, one Rayleigh-Ritz step, no convergence test (so no host round trip):
+//   Om <- orth(Omega);  iters x { Y <- orth(Theta Om);  Z <- Theta^T Y;  Om <- orth(Z) };  B = Om^T Z = W S X^T;  V = Om W.
+// Outputs as svd_trunc: Vz [n x chi] leading Ritz vectors, C [m x chi] = Theta Vz; columns >= keep are zero.
+void svd_rand(Ctx& cx, const ThetaOp& op, int chi, int ks, int pu, int g, double* Vz, double* C, double* sig0_out) {
+  tn_handle* h = cx.h;
+  const i64 m = op.m, n = op.n;
+  if (ks > 1024 || g > 4096) tn_throw(TN_ERR_ARG, "randomized SVD block of %d columns / bond %d: at most 1024 / 4096", ks, g);
+  DBuf<double> Om(h, (size_t)n * ks), Z(h, (size_t)n * ks), Y(h, (size_t)m * ks);
+  DBuf<double> B(h, (size_t)ks * ks), Bo(h, (size_t)ks * ks), Wt(h, (size_t)ks * ks), sig(h, ks);
+  fill_random_pgc(h, Om.p, pu, g, ks, cx.seed++);
+  cx.tic(&h->st.ms_orth_svd);
+  orth_columns(h, Om.p, n, ks, 3);
+  cx.toc();
+  for (int it = 0; it < std::max(1, h->rsvd_iters); it++) {
+    apply_N(cx, op, Om.p, Y.p, ks);
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Y.p, m, ks, 5);
+    cx.toc();
+    apply_T(cx, op, Y.p, Z.p, ks);
+    TN_CUDA(cudaMemcpyAsync(Om.p, Z.p, sizeof(double) * n * ks, cudaMemcpyDeviceToDevice, h->stream));
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Om.p, n, ks, 5);
+    cx.toc();
+    h->st.svd_iterations++;
+  }
+  cx.tic(&h->st.ms_orth_svd);
+  gemm_rm(h, true, false, ks, ks, (int)n, Om.p, ks, Z.p, ks, B.p, ks);
+  jacobi_rows(h, B.p, ks, ks, ks, Bo.p, Wt.p, sig.p);
+  k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, ks, chi, h->gap_guard, cx.d_keep, cx.d_stat);
+  TN_LAUNCH_CHECK(h);
+  k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
+  TN_LAUNCH_CHECK(h);
+  cx.toc();
+  gemm_rm(h, false, true, (int)n, ks, ks, Om.p, ks, Wt.p, ks, Z.p, ks);        // V = Om W
+  permute3(h, Vz, Z.p, 1, (int)n, chi, 0, ks, 1, 2, cx.d_keep);
+  apply_N(cx, op, Vz, C, chi);                                                  // connector = Theta V (exact for this V)
+  TN_CUDA(cudaMemcpyAsync(sig0_out, sig.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+}
+
 MpsTensor new_tensor(tn_handle* h, int dl, int p, int dr) {
   MpsTensor t;
   t.dl = dl; t.p = p; t.dr = dr;
   t.d = h->dalloc<double>((size_t)dl * p * dr);
   return t;
+}
+
+// C-1: QR chain left -> right on T in place (Fig. 8(c) "initial MPS in the left canonical form"); *rlast = the final 1 x 1 factor
+void left_canonicalize(Ctx& cx, std::vector<MpsTensor>& A, double* rlast) {
+  tn_handle* h = cx.h;
+  const int n = (int)A.size();
+  for (int j = 0; j < n; j++) {
+    const i64 rows = (i64)A[j].dl * A[j].p;
+    const int ar = A[j].dr;
+    DBuf<double> Q(h, (size_t)rows * ar), Rf(h, (size_t)ar * ar);
+    TN_CUDA(cudaMemcpyAsync(Q.p, A[j].d, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Q.p, rows, ar, 5);
+    cx.toc();
+    gemm_rm(h, true, false, ar, ar, (int)rows, Q.p, ar, A[j].d, ar, Rf.p, ar);
+    TN_CUDA(cudaMemcpyAsync(A[j].d, Q.p, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
+    if (j + 1 < n) {
+      const int cols = A[j + 1].p * A[j + 1].dr;
+      DBuf<double> T(h, (size_t)ar * cols);
+      gemm_rm(h, false, false, ar, cols, ar, Rf.p, ar, A[j + 1].d, cols, T.p, cols);
+      TN_CUDA(cudaMemcpyAsync(A[j + 1].d, T.p, sizeof(double) * ar * cols, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+      TN_CUDA(cudaMemcpyAsync(rlast, Rf.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    }
+  }
+}
+
+// Second step of the two-step truncation 2 chi -> chi: canonical compression of the unit-norm MPS N to
+// bond <= D (left-canonicalise, then LQ + small SVD at every bond right -> left; rank / gap rules as in the zipper).
+// N is replaced; *nu (device) receives the norm left after the cut.
+void truncate_mps(Ctx& cx, std::vector<MpsTensor>& N, int D, double* nu) {
+  tn_handle* h = cx.h;
+  const int n = (int)N.size();
+  DBuf<double> rl(h, 1);
+  left_canonicalize(cx, N, rl.p);
+  scale_by(h, N[n - 1].d, (i64)N[n - 1].dl * N[n - 1].p * N[n - 1].dr, rl.p, false);
+  for (int j = n - 1; j >= 1; j--) {
+    const int dl = N[j].dl, pc = N[j].p * N[j].dr;            // M = N[j] as [dl x pc]
+    const int kn = std::min(D, std::min(dl, pc));             // static new bond
+    DBuf<double> Qt(h, (size_t)pc * dl), L(h, (size_t)dl * dl), Lt(h, (size_t)dl * dl), Mo(h, (size_t)dl * dl);
+    DBuf<double> Wt(h, (size_t)dl * dl), sig(h, dl), T(h, (size_t)pc * dl);
+    permute3(h, Qt.p, N[j].d, 1, pc, dl, 0, 1, pc);           // Qt = M^T [pc x dl]
+    cx.tic(&h->st.ms_orth_svd);
+    orth_columns(h, Qt.p, pc, dl, 5);                         // M = L Qt^T with Qt^T right-canonical
+    gemm_rm(h, false, false, dl, dl, pc, N[j].d, pc, Qt.p, dl, L.p, dl);
+    permute3(h, Lt.p, L.p, 1, dl, dl, 0, 1, dl);
+    jacobi_rows(h, Lt.p, dl, dl, dl, Mo.p, Wt.p, sig.p);      // L = U S X^T:  Mo = S U^T,  Wt = X^T
+    k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, dl, kn, h->gap_guard, cx.d_keep, cx.d_stat);
+    TN_LAUNCH_CHECK(h);
+    k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
+    TN_LAUNCH_CHECK(h);
+    cx.toc();
+    gemm_rm(h, false, true, pc, dl, dl, Qt.p, dl, Wt.p, dl, T.p, dl);          // T = Qt X  [pc x dl]
+    MpsTensor nj = new_tensor(h, kn, N[j].p, N[j].dr);
+    permute3(h, nj.d, T.p, kn, pc, 1, 1, dl, 0, 0, cx.d_keep);                 // N'[j] = (first kn columns of T)^T, rows >= keep zero
+    // carry U S into the left neighbour: N[j-1] [rows x dl] . (Mo^T)[:, :kn]
+    const i64 rows = (i64)N[j - 1].dl * N[j - 1].p;
+    MpsTensor nl = new_tensor(h, N[j - 1].dl, N[j - 1].p, kn);
+    DBuf<double> Tl(h, (size_t)rows * kn);
+    gemm_rm(h, false, true, (int)rows, kn, dl, N[j - 1].d, dl, Mo.p, dl, Tl.p, kn);
+    permute3(h, nl.d, Tl.p, 1, (int)rows, kn, 0, kn, 1, 2, cx.d_keep);
+    h->dfree(N[j].d); h->dfree(N[j - 1].d);
+    N[j] = nj; N[j - 1] = nl;
+  }
+  const i64 n0 = (i64)N[0].dl * N[0].p * N[0].dr;
+  frob_norm(h, N[0].d, n0, nu);
+  scale_by(h, N[0].d, n0, nu, true);
 }
 
 // R_y = compress(T_y R_{y+1}; D, sweeps).  Returns the tensors of R_y (unit norm) and log of the norm removed.
@@ -574,28 +681,11 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
                             h->stream));
   }
   DBuf<double> rlast(h, 1);
-  for (int j = 0; j < n; j++) {
-    const i64 rows = (i64)A[j].dl * A[j].p;
-    const int ar = A[j].dr;
-    DBuf<double> Q(h, (size_t)rows * ar), Rf(h, (size_t)ar * ar);
-    TN_CUDA(cudaMemcpyAsync(Q.p, A[j].d, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
-    cx.tic(&h->st.ms_orth_svd);
-    orth_columns(h, Q.p, rows, ar, 5);
-    cx.toc();
-    gemm_rm(h, true, false, ar, ar, (int)rows, Q.p, ar, A[j].d, ar, Rf.p, ar);
-    TN_CUDA(cudaMemcpyAsync(A[j].d, Q.p, sizeof(double) * rows * ar, cudaMemcpyDeviceToDevice, h->stream));
-    if (j + 1 < n) {
-      const int cols = A[j + 1].p * A[j + 1].dr;
-      DBuf<double> T(h, (size_t)ar * cols);
-      gemm_rm(h, false, false, ar, cols, ar, Rf.p, ar, A[j + 1].d, cols, T.p, cols);
-      TN_CUDA(cudaMemcpyAsync(A[j + 1].d, T.p, sizeof(double) * ar * cols, cudaMemcpyDeviceToDevice, h->stream));
-    } else {
-      TN_CUDA(cudaMemcpyAsync(rlast.p, Rf.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
-    }
-  }
+  left_canonicalize(cx, A, rlast.p);
   // ---- static bond dimensions of the new MPS (zero-padded where the numerical rank is lower)
   std::vector<int> chi(n + 1, 1);
-  const int cap = exact ? h->exact_cap : D;
+  const bool two_step = !exact && h->two_step;
+  const int cap = exact ? h->exact_cap : (two_step ? 2 * D : D);   // bond kept by the zipper and the passes
   for (int j = n - 1; j >= 0; j--) {
     i64 mm = (i64)A[j].dl * pos[j].wl, nn = (i64)pos[j].pu * chi[j + 1];
     i64 full = std::min(mm, nn);
@@ -604,7 +694,6 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
                (long long)full, cap, y, j);
     chi[j] = (int)std::min<i64>(cap, full);
   }
-  // ---- C-2/C-3: zipper right -> left
   std::vector<double*> Renv(n, nullptr), Lenv(n, nullptr);
   std::vector<MpsTensor> N(n);
   // log-scales removed from the environments: lsR[j] = ls[j], lsL[j] = ls[n + j], ls0 = ls[2n] (reading S19)
@@ -613,16 +702,62 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
   TN_CUDA(cudaMemsetAsync(ls, 0, sizeof(double) * (2 * (size_t)n + 2), h->stream));
   double* d_sig0 = cx.d_scal + 1;
   double* d_safe = cx.d_scal + 2;
+  double* d_dummy = cx.d_scal + 3;
+  // ---- one-site variational steps (C-4; Fig. 8(d)): update the centre at q from both environments, move it on
+  auto step_right = [&](int q, bool move, bool track_ls) {     // centre q -> q + 1 (left environment extended)
+    const int g = chi[q], s2 = chi[q + 1];
+    ThetaOp op = build_op(cx, pos[q], true, A[q], Lenv[q], g);
+    DBuf<double> Z(h, (size_t)op.n * s2);
+    apply_T(cx, op, Renv[q], Z.p, s2);
+    if (move) {
+      cx.tic(&h->st.ms_orth_svd);
+      orth_columns(h, Z.p, op.n, s2, 5);
+      cx.toc();
+      if (Lenv[q + 1]) h->dfree(Lenv[q + 1]);
+      Lenv[q + 1] = h->dalloc<double>((size_t)op.m * s2);
+      apply_N(cx, op, Z.p, Lenv[q + 1], s2);
+      frob_norm(h, Lenv[q + 1], op.m * s2, d_sig0);
+      k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, track_ls ? ls + n + q : nullptr, track_ls ? ls + n + q + 1 : d_dummy, d_safe);
+      TN_LAUNCH_CHECK(h);
+      scale_by(h, Lenv[q + 1], op.m * s2, d_safe, true);
+    }
+    permute3(h, N[q].d, Z.p, g, pos[q].pu, s2, s2, (i64)g * s2, 1);
+    free_op(cx, op);
+  };
+  auto step_left = [&](int q, bool move) {                     // centre q -> q - 1 (right environment extended)
+    const int g = chi[q + 1], s2 = chi[q];
+    ThetaOp op = build_op(cx, pos[q], false, A[q], Renv[q], g);
+    DBuf<double> Z(h, (size_t)op.n * s2);
+    apply_T(cx, op, Lenv[q], Z.p, s2);
+    if (move) {
+      cx.tic(&h->st.ms_orth_svd);
+      orth_columns(h, Z.p, op.n, s2, 5);
+      cx.toc();
+      h->dfree(Renv[q - 1]);
+      Renv[q - 1] = h->dalloc<double>((size_t)op.m * s2);
+      apply_N(cx, op, Z.p, Renv[q - 1], s2);
+      frob_norm(h, Renv[q - 1], op.m * s2, d_sig0);
+      k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + q, ls + q - 1, d_safe);
+      TN_LAUNCH_CHECK(h);
+      scale_by(h, Renv[q - 1], op.m * s2, d_safe, true);
+    }
+    permute3(h, N[q].d, Z.p, s2, pos[q].pu, g, 1, (i64)g * s2, s2);
+    free_op(cx, op);
+  };
+  // ---- C-2/C-3: zipper right -> left
+  const bool interleaved = !exact && h->schedule == 1 && h->sweep_range > 0 && n > 1;
+  bool centre_swept = false;   // the centre tensor N[0] came out of a variational step (its scale sits in lsR[0] + lsL[0])
   Renv[n - 1] = h->dalloc<double>(1);
   TN_CUDA(cudaMemcpyAsync(Renv[n - 1], rlast.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
   for (int j = n - 1; j >= 0; j--) {
     const int g = chi[j + 1];
     ThetaOp op = build_op(cx, pos[j], false, A[j], Renv[j], g);
-    const int ks = exact ? (int)std::min(op.m, op.n)
-                         : (int)std::min<i64>((i64)chi[j] + h->oversample, std::min(op.m, op.n));
+    const i64 mn = std::min(op.m, op.n);
+    const int ks = exact ? (int)mn : (int)std::min<i64>((i64)chi[j] + h->oversample, mn);
     DBuf<double> Vz(h, (size_t)op.n * chi[j]);
     double* C = h->dalloc<double>((size_t)op.m * chi[j]);
-    svd_trunc(cx, op, chi[j], ks, Vz.p, C, d_sig0);
+    if (!exact && h->svd_mode == 1 && mn > cap) svd_rand(cx, op, chi[j], ks, pos[j].pu, g, Vz.p, C, d_sig0);
+    else svd_trunc(cx, op, chi[j], ks, Vz.p, C, d_sig0);
     N[j] = new_tensor(h, chi[j], pos[j].pu, g);
     permute3(h, N[j].d, Vz.p, chi[j], pos[j].pu, g, 1, (i64)g * chi[j], chi[j]);
     // connector <- connector / sigma_1, log sigma_1 carried beside it
@@ -636,72 +771,62 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
       h->dfree(C);
     }
     free_op(cx, op);
+    if (interleaved && j < n - 1) {
+      // ---- variational sweep of the instantaneous stage of the zipper over positions j .. kmax and
+      // back.  The block [connector . N_j ... N_{n-1}] approximates (A_j W_j) ... (A_{n-1} W_{n-1}) with its left legs
+      // (old bond, MPO bond) open; an orthonormal basis of the connector's range on those legs is the left
+      // environment of position j (reading S21): the connector already has the environment layout.
+      const int kmax = std::min(n - 1, j + h->sweep_range);
+      if (Lenv[j]) h->dfree(Lenv[j]);
+      if (j > 0) {
+        const i64 mc = (i64)A[j].dl * pos[j].wl;
+        Lenv[j] = h->dalloc<double>((size_t)mc * chi[j]);
+        TN_CUDA(cudaMemcpyAsync(Lenv[j], Renv[j - 1], sizeof(double) * mc * chi[j], cudaMemcpyDeviceToDevice, h->stream));
+        cx.tic(&h->st.ms_orth_svd);
+        orth_columns(h, Lenv[j], mc, chi[j], 5);
+        cx.toc();
+      } else {
+        Lenv[0] = h->dalloc<double>(1);
+        fill_value(h, Lenv[0], 1, 1.0);
+      }
+      for (int q = j; q < kmax; q++) step_right(q, true, false);
+      for (int q = kmax; q >= j; q--) step_left(q, q > 0);
+      if (j == 0) centre_swept = true;
+    }
   }
   // ---- C-4: one-site variational passes, alternating, first left -> right
   int centre = 0;
   if (!exact && sweeps > 0) {
+    if (Lenv[0]) h->dfree(Lenv[0]);
     Lenv[0] = h->dalloc<double>(1);
     fill_value(h, Lenv[0], 1, 1.0);
+    TN_CUDA(cudaMemsetAsync(ls + n, 0, sizeof(double) * n, h->stream));
     for (int sw = 0; sw < sweeps; sw++) {
       if (sw % 2 == 0) {
-        for (int j = 0; j < n; j++) {
-          const int g = chi[j], s = chi[j + 1];
-          ThetaOp op = build_op(cx, pos[j], true, A[j], Lenv[j], g);
-          DBuf<double> Z(h, (size_t)op.n * s);
-          apply_T(cx, op, Renv[j], Z.p, s);
-          if (j + 1 < n) {
-            cx.tic(&h->st.ms_orth_svd);
-            orth_columns(h, Z.p, op.n, s, 5);
-            cx.toc();
-            if (Lenv[j + 1]) h->dfree(Lenv[j + 1]);
-            Lenv[j + 1] = h->dalloc<double>((size_t)op.m * s);
-            apply_N(cx, op, Z.p, Lenv[j + 1], s);
-            frob_norm(h, Lenv[j + 1], op.m * s, d_sig0);
-            k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + n + j, ls + n + j + 1, d_safe);
-            TN_LAUNCH_CHECK(h);
-            scale_by(h, Lenv[j + 1], op.m * s, d_safe, true);
-          }
-          permute3(h, N[j].d, Z.p, g, pos[j].pu, s, s, (i64)g * s, 1);
-          free_op(cx, op);
-        }
+        for (int j = 0; j < n; j++) step_right(j, j + 1 < n, true);
         centre = n - 1;
       } else {
-        for (int j = n - 1; j >= 0; j--) {
-          const int g = chi[j + 1], s = chi[j];
-          ThetaOp op = build_op(cx, pos[j], false, A[j], Renv[j], g);
-          DBuf<double> Z(h, (size_t)op.n * s);
-          apply_T(cx, op, Lenv[j], Z.p, s);
-          if (j > 0) {
-            cx.tic(&h->st.ms_orth_svd);
-            orth_columns(h, Z.p, op.n, s, 5);
-            cx.toc();
-            h->dfree(Renv[j - 1]);
-            Renv[j - 1] = h->dalloc<double>((size_t)op.m * s);
-            apply_N(cx, op, Z.p, Renv[j - 1], s);
-            frob_norm(h, Renv[j - 1], op.m * s, d_sig0);
-            k_ls_step<<<1, 32, 0, h->stream>>>(d_sig0, ls + j, ls + j - 1, d_safe);
-            TN_LAUNCH_CHECK(h);
-            scale_by(h, Renv[j - 1], op.m * s, d_safe, true);
-          }
-          permute3(h, N[j].d, Z.p, s, pos[j].pu, g, 1, (i64)g * s, s);
-          free_op(cx, op);
-        }
+        for (int j = n - 1; j >= 0; j--) step_left(j, j > 0);
         centre = 0;
       }
     }
+    centre_swept = true;
   }
   // ---- norm of the centre tensor -> log-scale
   const i64 nc = (i64)N[centre].dl * N[centre].p * N[centre].dr;
   frob_norm(h, N[centre].d, nc, cx.d_scal);
   scale_by(h, N[centre].d, nc, cx.d_scal, true);
-  double nrm = 0.0;
+  if (two_step) truncate_mps(cx, N, D, d_dummy);   // 2 chi -> chi; the norm left after the cut joins the log-scale
+  else fill_value(h, d_dummy, 1, 1.0);
+  double nrm = 0.0, nu = 1.0;
   std::vector<double> lsh(2 * (size_t)n + 2);
   TN_CUDA(cudaMemcpyAsync(&nrm, cx.d_scal, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TN_CUDA(cudaMemcpyAsync(&nu, d_dummy, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   TN_CUDA(cudaMemcpyAsync(lsh.data(), ls, sizeof(double) * lsh.size(), cudaMemcpyDeviceToHost, h->stream));
   TN_CUDA(cudaStreamSynchronize(h->stream));
-  if (!(nrm > 0.0) || !std::isfinite(nrm)) tn_throw(TN_ERR_NUMERIC, "row %d: boundary MPS norm is %g", y, nrm);
-  const bool swept = !exact && sweeps > 0;
-  *lognorm = std::log(nrm) + (swept ? lsh[centre] + lsh[n + centre] : lsh[2 * (size_t)n]);
+  if (!(nrm > 0.0) || !std::isfinite(nrm) || !(nu > 0.0) || !std::isfinite(nu))
+    tn_throw(TN_ERR_NUMERIC, "row %d: boundary MPS norm is %g (after the 2 chi -> chi cut: %g)", y, nrm, nu);
+  *lognorm = std::log(nrm) + std::log(nu) + (centre_swept ? lsh[centre] + lsh[n + centre] : lsh[2 * (size_t)n]);
   if (!std::isfinite(*lognorm)) tn_throw(TN_ERR_NUMERIC, "row %d: log-norm is not finite", y);
   for (int j = 0; j < n; j++) {
     h->dfree(A[j].d);

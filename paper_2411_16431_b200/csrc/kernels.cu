@@ -115,6 +115,21 @@ __global__ void k_fill_random(double* X, i64 n, uint64_t seed) {
   i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) X[i] = 2.0 * ((mix64(seed * 0x100000001B3ull + (uint64_t)i) >> 11) * (1.0 / 9007199254740992.0)) - 1.0;
 }
+// Omega[(p', gamma)][col] = uniform(-1,1) from the counter (seed, p', gamma, col): independent of any memory layout, so
+// that the randomized SVD (TN_OPT_SVD_MODE = 1) draws the same block whatever the padding of the bonds
+__global__ void k_fill_random_pgc(double* X, int pu, int g, int ks, uint64_t seed) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)pu * g * ks) return;
+  const uint64_t c = (uint64_t)(t % ks), gg = (uint64_t)((t / ks) % g), pp = (uint64_t)(t / ((i64)ks * g));
+  const uint64_t ctr = seed * 0x100000001B3ull + ((pp * 4096ull + gg) * 1024ull + c);
+  X[t] = 2.0 * ((mix64(ctr) >> 11) * (1.0 / 9007199254740992.0)) - 1.0;
+}
+void fill_random_pgc(tn_handle* h, double* X, int pu, int g, int ks, uint64_t seed) {
+  const i64 n = (i64)pu * g * ks;
+  if (n <= 0) return;
+  k_fill_random_pgc<<<cdiv(n, 256), 256, 0, h->stream>>>(X, pu, g, ks, seed);
+  TN_LAUNCH_CHECK(h);
+}
 void fill_random(tn_handle* h, double* X, i64 n, uint64_t seed) {
   if (n <= 0) return;
   k_fill_random<<<cdiv(n, 256), 256, 0, h->stream>>>(X, n, seed);

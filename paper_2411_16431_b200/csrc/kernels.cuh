@@ -16,6 +16,8 @@ static inline int cdiv(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 // X[i] = uniform(-1,1) from a counter-based hash of (seed, i)
 void fill_random(tn_handle* h, double* X, i64 n, uint64_t seed);
 void fill_value(tn_handle* h, double* X, i64 n, double v);
+// X[(p', gamma)][col], p' < pu, gamma < g (<= 4096), col < ks (<= 1024): counter-based, layout-free (randomized SVD)
+void fill_random_pgc(tn_handle* h, double* X, int pu, int g, int ks, uint64_t seed);
 // out[i0][i1][i2] = in[i0*s0 + i1*s1 + i2*s2]; entries whose index along `mask_axis` (0..2, -1 = none)
 // is >= *keep (device int) are written as exact zeros.
 void permute3(tn_handle* h, double* out, const double* in, int n0, int n1, int n2, i64 s0, i64 s1, i64 s2,

@@ -50,15 +50,15 @@ def differ_by_component_flips(inst, s1, s2, comp=None):
     return all(np.unique(rel[comp == c]).size == 1 for c in np.unique(comp))
 
 
-def run_oracle(inst, beta, D, sweeps, M, merge=False):
+def run_oracle(inst, beta, D, sweeps, M, merge=False, oracle_opts=None):
     m = model.Model(inst).set_beta(beta)
-    R, ln = mps.contract(m, D, sweeps)
+    R, ln = mps.contract(m, D, sweeps, **(oracle_opts or {}))
     out = search.branch_and_bound(m, R, ln, M, merge=merge)
     return m, R, ln, out
 
 
-def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=False):
-    m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M, merge=merge)
+def compare(inst, beta, D, sweeps, M, tol, check_rows=True, options=(), merge=False, oracle_opts=None):
+    m, R, ln, ref = run_oracle(inst, beta, D, sweeps, M, merge=merge, oracle_opts=oracle_opts)
     with _tn(inst) as t:
         for key, val in options:
             t.set_option(key, val)
@@ -287,6 +287,62 @@ def test_merge_routes_and_counted_fallback(cap, expect_fallback):
         st = t.stats()
     assert st["merge_fallback_cells"] > 0
     assert np.array_equal(E, energy.energies(inst, states)) and np.all(np.diff(logp) <= 0)
+
+
+F2 = [  # (name, oracle options, CUDA options): the paper's preferred schedule and its ingredients
+    ("interleaved_r1", dict(schedule=1, sweep_range=1), [("OPT_SCHEDULE", 1), ("OPT_SWEEP_RANGE", 1)]),
+    ("interleaved_r2", dict(schedule=1, sweep_range=2), [("OPT_SCHEDULE", 1)]),
+    ("interleaved_all", dict(schedule=1, sweep_range=99), [("OPT_SCHEDULE", 1), ("OPT_SWEEP_RANGE", 99)]),
+    ("two_step", dict(two_step=True), [("OPT_TWO_STEP", 1)]),
+    ("randomized_2it", dict(svd_mode=1, rsvd_iters=2), [("OPT_SVD_MODE", 1)]),
+    ("randomized_1it", dict(svd_mode=1, rsvd_iters=1), [("OPT_SVD_MODE", 1), ("OPT_RSVD_ITERS", 1)]),
+    ("paper_preferred", dict(schedule=1, sweep_range=2, svd_mode=1, rsvd_iters=2, two_step=True),
+     [("OPT_SCHEDULE", 1), ("OPT_SVD_MODE", 1), ("OPT_TWO_STEP", 1)]),
+]
+F2_CASES = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, M)
+    (4, 4, 2, 4, 0.95, 2, 1.0, 6, 64),         # Zephyr-shaped miniature, ragged projectors
+    (3, 3, 3, 4, 0.9, 4, 1.0, 6, 64),          # Pegasus-shaped miniature: mediating positions inside the local sweeps
+    (3, 4, 1, 4, 1.0, 6, 2.0, 5, 16),
+]
+
+
+@pytest.mark.parametrize("name,oopts,copts", F2, ids=[f[0] for f in F2])
+@pytest.mark.parametrize("case", range(len(F2_CASES)))
+@pytest.mark.parametrize("sweeps", [0, 1])
+def test_f2_schedule_parity(name, oopts, copts, case, sweeps):
+    """TN_OPT_SCHEDULE / SVD_MODE / TWO_STEP against the oracle's switches of the same names: element by element at
+    1e-6, rows included.  The randomized SVD is deterministic given its counter-based random block, which both sides
+    generate from (seed, p', gamma, column) (oracle.mps.hash_uniform, k_fill_random_pgc)."""
+    import paper_2411_16431_b200 as tnb
+    Ly, Lx, S, ns, p, seed, beta, D, M = F2_CASES[case]
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    st = compare(inst, beta, D, sweeps, M, 1e-6, options=[(getattr(tnb, k), v) for k, v in copts], oracle_opts=oopts)
+    assert st["svd_unconverged"] == 0
+
+
+def test_f2_fast_mode_close_to_converged_mode():
+    """The fast mode (randomized SVD) is not the parity definition: it is compared with the converged
+    mode by R_y overlap and by the final list -- after one variational pass the two agree to the size of the
+    truncation error, with a fraction of the Theta applies."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(4, 4, 2, 4, p_keep=0.95, seed=2)
+    out = {}
+    for mode in (0, 1):
+        with _tn(inst) as t:
+            t.set_option(tnb.OPT_SVD_MODE, mode)
+            t.set_beta(1.0)
+            t.contract(6, 1)
+            rows = {y: t.mps(y) for y in range(1, inst.Ly)}
+            lz = t.log_z()
+            states, E, logp, pd = t.branch_and_bound(64)
+            out[mode] = (rows, lz, states, E, logp, t.stats())
+    trunc = out[0][5]["min_sigma_rel"]
+    assert 0 < trunc < 0.1
+    for y in range(1, inst.Ly):
+        assert 1 - abs(mps_overlap(out[0][0][y], out[1][0][y])) <= 10 * trunc ** 2 + 1e-12
+    assert abs(out[0][1] - out[1][1]) <= 10 * trunc * abs(out[0][1])
+    assert out[0][3].min() == out[1][3].min()                     # same best energy
+    assert out[1][5]["theta_apply_calls"] < out[0][5]["theta_apply_calls"]
 
 
 EDGE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, h): the degenerate shapes the method has
