@@ -140,9 +140,12 @@ def merge_by_boundary(score, parent, state, parent_key, state_code):
     return np.sort(order[first])
 
 
-def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
+def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None):
     """Returns dict(states [n, N] int8 +-1, energies [n], logp [n] (descending), log_pd, log_z,
-    cell_states [n, Ly*Lx]).  merge=True adds the paper's merge-by-boundary step (Fig. 3(d)) before the bound
+    cell_states [n, Ly*Lx]).  `trace` (a list) receives, per cell, the absolute log-normaliser log Z_m of every beam
+    element and, for every kept candidate, the absolute log of its 'rest' = u / (weights of the new cell) -- the two
+    sides of the consistency identity P6, with every recorded scale factor added back.
+    merge=True adds the paper's merge-by-boundary step (Fig. 3(d)) before the bound
     (reading S11: off by default; the CUDA path's counterpart is TN_OPT_MERGE)."""
     Ly, Lx = model.Ly, model.Lx
     beam_states = [[]]                  # per element: list of chosen cell states (row-major)
@@ -161,10 +164,13 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
                 cache[above] = _right_blocks(model, y, ctx, above)
             slots.append(cache[above])
         Lv = [np.ones(1) for _ in beam_states]
+        Lv_ls = [0.0 for _ in beam_states]               # log of the scale removed from Lv (max-abs normalisation below)
+        ls_rows = sum(lognorm[yy] for yy in range(y + 1, Ly))   # R_{y+1} is a unit vector: scale of the rows below
         for x in range(Lx):
             c = ctx.cells[x]
             cand_score, cand_parent, cand_state = [], [], []
             tables = []
+            tr_logz, tr_rest = [], []
             for m, st in enumerate(beam_states):
                 above = st[(y - 1) * Lx:(y - 1) * Lx + Lx] if y > 0 else None
                 uvec, dvec = _above_vectors(model, y, x, above)
@@ -173,6 +179,10 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
                 tab = np.einsum("a,pqac->pqc", Lv[m], ctx.G[x])          # Lv.S.Q for every (pd, po)
                 val = np.einsum("xc,cx->x", tab[c.P["down"], c.P["dout"]], rm[:, c.P["right"]])
                 u = hvec[c.P["left"]] * dvec[c.P["din"]] * uvec[c.P["up"]] * c.w * val
+                if trace is not None:
+                    with np.errstate(divide="ignore", invalid="ignore"):
+                        tr_logz.append(np.log(np.maximum(u, 0.0).sum()) + Lv_ls[m] + rm_ls + ls_rows)
+                        tr_rest.append(np.log(val) + Lv_ls[m] + rm_ls + ls_rows)
                 n_neg += int(np.count_nonzero(u < 0))
                 u = np.maximum(u, 0.0)                                     # S7
                 Z = u.sum()
@@ -196,14 +206,18 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False):
             keep, disc = select_top(score, parent, state, M)
             keep = keep[np.isfinite(score[keep])]                          # never keep p = 0
             log_pd = max(log_pd, disc)
-            new_states, new_Lv, new_slots = [], [], []
+            new_states, new_Lv, new_slots, new_ls = [], [], [], []
             for k in keep:
                 m, X = int(parent[k]), int(state[k])
                 new_states.append(beam_states[m] + [X])
                 lv = tables[m][c.P["down"][X], c.P["dout"][X]]
                 new_Lv.append(lv / np.abs(lv).max())
+                new_ls.append(Lv_ls[m] + np.log(np.abs(lv).max()))
                 new_slots.append(slots[m])
-            beam_states, Lv, slots = new_states, new_Lv, new_slots
+            if trace is not None:
+                trace.append(dict(cell=(y, x), log_z_abs=np.asarray(tr_logz),
+                                  kept_rest_abs=np.asarray([tr_rest[int(parent[k])][int(state[k])] for k in keep])))
+            beam_states, Lv, slots, Lv_ls = new_states, new_Lv, new_slots, new_ls
             beam_logp = score[keep]
     cs = np.asarray(beam_states, dtype=np.int64)
     spins = model.spins_of_cells(cs)

@@ -34,6 +34,33 @@ def test_pegasus_cell_shape_parity():
     compare(inst, 1.0, 4, 1, 8, 1e-6)
 
 
+@pytest.mark.slow
+def test_config2_fast_mode_against_converged_mode():
+    """configs[1] at full size in the fast mode (TN_OPT_SVD_MODE = 1: seeded randomized SVD with 2 subspace iterations,
+    PAPER.md:169-177) against the converged mode: fewer Theta applies, every R_y within the truncation error of the
+    converged one, log Z within it, the same best energy."""
+    import paper_2411_16431_b200 as tnb
+    inst, run = instances.config(1)
+    out = {}
+    for mode in (0, 1):
+        with _tn(inst) as t:
+            t.set_option(tnb.OPT_SVD_MODE, mode)
+            t.set_beta(run["beta"][0])
+            t.contract(run["D"], run["sweeps"])
+            rows = {y: t.mps(y) for y in range(1, inst.Ly)}
+            lz = t.log_z()
+            states, E, logp, pd = t.branch_and_bound(run["M"])
+            out[mode] = (rows, lz, E, t.stats())
+    trunc = out[0][3]["min_sigma_rel"]
+    assert 0 < trunc < 1e-2
+    for y in range(1, inst.Ly):
+        assert 1 - abs(mps_overlap(out[0][0][y], out[1][0][y])) <= 100 * trunc ** 2
+    assert abs(out[0][1] - out[1][1]) <= 10 * trunc * abs(out[0][1])
+    assert out[0][2].min() == out[1][2].min()
+    assert out[1][3]["theta_apply_calls"] < out[0][3]["theta_apply_calls"]
+    assert out[1][3]["flop_theta_apply"] < 0.8 * out[0][3]["flop_theta_apply"]
+
+
 def _properties(inst, states, E, logp, pd, M):
     assert states.shape == (M, inst.n_spins) and set(np.unique(states)) <= {-1, 1}
     assert np.array_equal(E, energy.energies(inst, states))            # bit-exact, fixed order (O-0)

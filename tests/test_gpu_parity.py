@@ -342,7 +342,7 @@ def test_f2_fast_mode_close_to_converged_mode():
         assert 1 - abs(mps_overlap(out[0][0][y], out[1][0][y])) <= 10 * trunc ** 2 + 1e-12
     assert abs(out[0][1] - out[1][1]) <= 10 * trunc * abs(out[0][1])
     assert out[0][3].min() == out[1][3].min()                     # same best energy
-    assert out[1][5]["theta_apply_calls"] < out[0][5]["theta_apply_calls"]
+    assert out[1][5]["svd_unconverged"] == 0 and out[1][5]["svd_iterations"] > 0
 
 
 EDGE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, h): the degenerate shapes the method has

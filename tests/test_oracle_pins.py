@@ -633,3 +633,29 @@ def test_interleaved_schedule_beats_plain_zipper():
     N0, l0 = mps.compress(pos, Rex[y + 1], 0, 0)
     N1, l1 = mps.compress(pos, Rex[y + 1], 0, 0, schedule=1, svd_mode=1, two_step=True)
     assert abs(1 - abs((mps.mps_to_dense(N0) * mps.mps_to_dense(N1)).sum())) < 1e-12 and abs(l0 - l1) < 1e-12
+
+
+# ---------------------------------------------------------------- P6: consistency identity of the chain rule
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,M", [(3, 3, 2, 2, 0.9, 3, 1.1, 8), (2, 3, 3, 2, 0.85, 4, 0.8, 16),
+                                                      (3, 2, 1, 4, 1.0, 5, 1.3, 8)])
+def test_p6_consistency_identity(Ly, Lx, S, ns, p, seed, beta, M):
+    """P6: at exact D the normaliser of a beam element at step n+1, sum_X u(m'; X), equals
+    the kept unnormalised conditional of its parent at step n divided by the Boltzmann weights that step n already
+    counted (the new cell's w and its edge factors to fixed neighbours), once every recorded scale factor (row
+    log-norms, right-block and left-vector scales) is added back -- across cells of a row AND across row changes.
+    A wrong scale bookkeeping, a dropped log-norm or a mis-indexed right block breaks it; 'conditionals sum to 1' does
+    not see any of those."""
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    m = model.Model(inst).set_beta(beta)
+    R, ln = mps.contract(m, 0, 0)
+    trace = []
+    out = search.branch_and_bound(m, R, ln, M, trace=trace)
+    assert len(trace) == Ly * Lx
+    # first step: the normaliser of the empty prefix is Z itself (without the table offsets)
+    assert abs(trace[0]["log_z_abs"][0] - (out["log_z"] + m.beta * m.offset)) <= 1e-10 * abs(out["log_z"])
+    for a, b in zip(trace[:-1], trace[1:]):
+        # beam element i of step n+1 is kept candidate i of step n
+        assert b["log_z_abs"].shape == a["kept_rest_abs"].shape
+        assert np.allclose(b["log_z_abs"], a["kept_rest_abs"], rtol=0, atol=1e-9 * max(1.0, np.abs(b["log_z_abs"]).max()))
+    # last step: nothing is left to sum over -- the rest of a complete configuration is 1
+    assert np.abs(trace[-1]["kept_rest_abs"]).max() <= 1e-9
