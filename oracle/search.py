@@ -140,14 +140,101 @@ def merge_by_boundary(score, parent, state, parent_key, state_code):
     return np.sort(order[first])
 
 
-def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None):
+class DropletBook:
+    """Excitation bookkeeping on top of the merge (Fig. 4): every beam element (main branch)
+    carries a list of droplets = low-energy excitations above it that do not modify its boundary.
+
+    A droplet is (dE, flips) with flips = {cell index: xor mask on that cell's state bits}.  When candidates merge
+    (same boundary), the most probable one is the main branch; every loser L gives the candidate droplet
+    diff(L, main) with dE = (logp_main - logp_L) / beta (same boundary => the ratio of the marginals is
+    exp(-beta dE) exactly for exact marginals), and every droplet d' already carried by L's parent gives the candidate
+    diff(L, main) xor d' with dE_L + dE(d') ('together with excitations above (b) and (b') accumulated in the previous
+    steps', Fig. 4 caption).  'To keep their number under control, we keep only those that are singly connected and
+    with a hamming distance between any pair of them above a specified threshold': candidates are walked in increasing
+    dE (ties: generation order = inherited ones first, then losers in the S8 order, each followed by its compositions)
+    and kept iff dE <= max_dE, the flipped spins form ONE connected piece of the interaction graph (edges with
+    J != 0), and the Hamming distance to every droplet already kept is >= min_hamming; at most max_count are kept
+    (reading S24)."""
+
+    def __init__(self, model, max_dE=1.0, min_hamming=1, max_count=8):
+        self.max_dE, self.min_hamming, self.max_count = float(max_dE), int(min_hamming), int(max_count)
+        inst = model.inst
+        ncell = model.Ly * model.Lx
+        self.nbits = model.nbits
+        self.spin_of = -np.ones((ncell, model.nbits), dtype=np.int64)       # (cell, bit) -> spin id
+        cell = inst.cell_y.astype(np.int64) * model.Lx + inst.cell_x
+        bit = inst.sub.astype(np.int64) * inst.n_s + inst.pos
+        self.spin_of[cell, bit] = np.arange(inst.n_spins)
+        self.adj = [[] for _ in range(inst.n_spins)]
+        for u, v, J in zip(inst.edge_u.tolist(), inst.edge_v.tolist(), inst.J.tolist()):
+            if J != 0.0:
+                self.adj[u].append(v)
+                self.adj[v].append(u)
+
+    def spins(self, flips):
+        out = []
+        for cidx, mask in flips.items():
+            for b in range(self.nbits):
+                if (mask >> b) & 1:
+                    out.append(int(self.spin_of[cidx, b]))
+        return out
+
+    def connected(self, flips):
+        sp = self.spins(flips)
+        if not sp:
+            return False
+        todo, seen, inset = [sp[0]], {sp[0]}, set(sp)
+        while todo:
+            u = todo.pop()
+            for v in self.adj[u]:
+                if v in inset and v not in seen:
+                    seen.add(v)
+                    todo.append(v)
+        return len(seen) == len(inset)
+
+    @staticmethod
+    def xor(f1, f2):
+        out = dict(f1)
+        for k, v in f2.items():
+            w = out.get(k, 0) ^ v
+            if w:
+                out[k] = w
+            else:
+                out.pop(k, None)
+        return out
+
+    @staticmethod
+    def hamming(f1, f2):
+        return sum(bin(v).count("1") for v in DropletBook.xor(f1, f2).values())
+
+    def select(self, cands):
+        """cands: list of (dE, flips) in generation order -> kept list (greedy in increasing dE)."""
+        order = sorted(range(len(cands)), key=lambda i: (cands[i][0], i))
+        kept = []
+        for i in order:
+            dE, fl = cands[i]
+            if len(kept) >= self.max_count:
+                break
+            if not (dE <= self.max_dE) or not fl or not self.connected(fl):
+                continue
+            if all(self.hamming(fl, k[1]) >= self.min_hamming for k in kept):
+                kept.append((dE, fl))
+        return kept
+
+
+def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None, droplets=None):
     """Returns dict(states [n, N] int8 +-1, energies [n], logp [n] (descending), log_pd, log_z,
     cell_states [n, Ly*Lx]).  `trace` (a list) receives, per cell, the absolute log-normaliser log Z_m of every beam
     element and, for every kept candidate, the absolute log of its 'rest' = u / (weights of the new cell) -- the two
     sides of the consistency identity P6, with every recorded scale factor added back.
     merge=True adds the paper's merge-by-boundary step (Fig. 3(d)) before the bound
-    (reading S11: off by default; the CUDA path's counterpart is TN_OPT_MERGE)."""
+    (reading S11: off by default; the CUDA path's counterpart is TN_OPT_MERGE).
+    droplets=dict(max_dE, min_hamming, max_count) (needs merge=True) adds the excitation bookkeeping of Fig. 4
+    (class DropletBook); the result then carries `droplets`: per returned state a list of (dE, flip mask [N] bool)."""
     Ly, Lx = model.Ly, model.Lx
+    book = DropletBook(model, **droplets) if droplets is not None else None
+    assert book is None or merge, "droplets need merge=True"
+    drops = [[]]                        # per beam element: list of (dE, flips)
     beam_states = [[]]                  # per element: list of chosen cell states (row-major)
     beam_logp = np.zeros(1)
     log_pd = -np.inf
@@ -199,12 +286,41 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None):
             state = np.concatenate(cand_state)
             if merge:
                 pk, sc = boundary_codes(model, y, x, beam_states)
+                if book is not None:
+                    all_score, all_parent, all_state = score, parent, state
+                    gkey = pk[parent] * (int(sc.max()) + 1) + sc[state]
+                    gorder = np.lexsort((state, parent, -score, gkey))     # groups contiguous, winner first, S8 inside
+                    gpos = np.empty(gorder.size, dtype=np.int64)
+                    gpos[gorder] = np.arange(gorder.size)
                 surv = merge_by_boundary(score, parent, state, pk, sc)
                 score, parent, state = score[surv], parent[surv], state[surv]
                 if stats is not None:
                     stats["merged_away"] = stats.get("merged_away", 0) + int(pk.size * sc.size - surv.size)
             keep, disc = select_top(score, parent, state, M)
             keep = keep[np.isfinite(score[keep])]                          # never keep p = 0
+            new_drops = []
+            if book is not None:
+                n_cell = y * Lx + x
+                for kk in keep:                                            # Fig. 4: losers of the winner's group
+                    w = int(surv[kk])
+                    mw, Xw, sw = int(all_parent[w]), int(all_state[w]), all_score[w]
+                    cands = list(drops[mw])                                # excitations the main branch already carries
+                    t = gpos[w] + 1
+                    while t < gorder.size and gkey[gorder[t]] == gkey[w]:
+                        l = int(gorder[t])
+                        dE = (sw - all_score[l]) / model.beta
+                        if not (dE <= book.max_dE):
+                            break                                          # sorted by score: the rest is further away
+                        ml, Xl = int(all_parent[l]), int(all_state[l])
+                        base = {k: a ^ b for k, (a, b) in enumerate(zip(beam_states[ml], beam_states[mw])) if a != b}
+                        if Xl != Xw:
+                            base[n_cell] = Xl ^ Xw
+                        cands.append((dE, base))
+                        for (d2, f2) in drops[ml]:
+                            if dE + d2 <= book.max_dE:
+                                cands.append((dE + d2, DropletBook.xor(base, f2)))
+                        t += 1
+                    new_drops.append(book.select(cands))
             log_pd = max(log_pd, disc)
             new_states, new_Lv, new_slots, new_ls = [], [], [], []
             for k in keep:
@@ -218,13 +334,25 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None):
                 trace.append(dict(cell=(y, x), log_z_abs=np.asarray(tr_logz),
                                   kept_rest_abs=np.asarray([tr_rest[int(parent[k])][int(state[k])] for k in keep])))
             beam_states, Lv, slots, Lv_ls = new_states, new_Lv, new_slots, new_ls
+            if book is not None:
+                drops = new_drops
             beam_logp = score[keep]
     cs = np.asarray(beam_states, dtype=np.int64)
     spins = model.spins_of_cells(cs)
     if stats is not None:
         stats["negative_u"] = n_neg
-    return dict(states=spins, energies=_energy.energies(model.inst, spins), logp=beam_logp,
-                log_pd=log_pd, log_z=log_z, cell_states=cs)
+    out = dict(states=spins, energies=_energy.energies(model.inst, spins), logp=beam_logp,
+               log_pd=log_pd, log_z=log_z, cell_states=cs)
+    if book is not None:
+        out["droplets"] = []
+        for lst in drops:
+            row = []
+            for dE, fl in lst:
+                mask = np.zeros(model.inst.n_spins, dtype=bool)
+                mask[book.spins(fl)] = True
+                row.append((dE, mask))
+            out["droplets"].append(row)
+    return out
 
 
 def exact_marginal_beam(model, E_all, M):

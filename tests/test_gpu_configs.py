@@ -89,6 +89,9 @@ def test_config5_full_size_properties():
     beta, N = run["beta"][0], inst.n_spins
     assert -beta * inst.E0 + np.log(2) - 1e-6 <= lz <= -beta * inst.E0 + N * np.log(2)
     assert st["min_sigma_rel"] < 1e-6
+    # beta = 4 on integer couplings: every bond is rank-deficient below D (nothing above 1e-14 sigma_1 is cut), so the
+    # contraction is exact to rounding and the chain rule logp = -beta E - log Z holds at every returned state
+    assert np.abs(logp + beta * E + lz).max() <= 1e-6 * abs(lz)
 
 
 @pytest.mark.slow
@@ -99,10 +102,15 @@ def test_config3_full_size_properties():
         t.contract(run["D"], run["sweeps"])
         lz = t.log_z()
         states, E, logp, pd = t.branch_and_bound(run["M"])
+        st = t.stats()
     _properties(inst, states, E, logp, pd, run["M"])
     beta = run["beta"][0]
     # every returned state is one term of Z:  log Z >= -beta E(s)  (up to the contraction error of a truncated MPS)
     assert lz >= -beta * E.min() - 1e-3 * abs(lz)
-    # exact chain rule at the returned states would give logp = -beta E - log Z; with D = 32 it holds approximately
+    # Chain rule at the returned states: exact marginals give logp = -beta E - log Z.  The product of conditionals
+    # telescopes row by row, so the residual is a sum of Ly - 1 log-ratios of boundary-MPS amplitudes, each off by at
+    # most the relative weight that row's worst cut discarded (min_sigma_rel = the largest smallest-retained sigma over
+    # all bonds, Fig. 12(b); measured at this config: 4.2e-3, residual 7.7e-3 nats).
     resid = logp + beta * E + lz
-    assert np.abs(resid).max() <= 0.05 * abs(beta * E.min())
+    assert 0 < st["min_sigma_rel"] < 0.02
+    assert np.abs(resid).max() <= 2 * (inst.Ly - 1) * st["min_sigma_rel"], (np.abs(resid).max(), st["min_sigma_rel"])

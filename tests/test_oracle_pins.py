@@ -659,3 +659,63 @@ def test_p6_consistency_identity(Ly, Lx, S, ns, p, seed, beta, M):
         assert np.allclose(b["log_z_abs"], a["kept_rest_abs"], rtol=0, atol=1e-9 * max(1.0, np.abs(b["log_z_abs"]).max()))
     # last step: nothing is left to sum over -- the rest of a complete configuration is 1
     assert np.abs(trace[-1]["kept_rest_abs"]).max() <= 1e-9
+
+
+# ---------------------------------------------------------------- f1: droplets (Fig. 4)
+@pytest.mark.parametrize("S,ns,seed,beta", [(2, 2, 3, 2.0), (1, 4, 8, 1.5)])
+def test_droplets_are_the_connected_low_energy_excitations(S, ns, seed, beta):
+    """Fig. 4: with exact marginals and no pruning the merge makes the ground state the main branch and
+    the book-kept droplets are EXACTLY the singly connected excitations above it within max_dE -- checked against
+    brute force over all 2^24 states: same flip sets, dE (from the ratio of marginals) = the exact energy difference
+    (O-0), lowest droplet = first excited state; combinations of droplets give further states of the spectrum."""
+    inst = instances.lattice(2, 3, S, ns, p_keep=1.0, seed=seed)
+    assert inst.n_spins == 24
+    m = model.Model(inst).set_beta(beta)
+    R, ln = mps.contract(m, 0, 0)
+    max_dE = 1.2
+    out = search.branch_and_bound(m, R, ln, 4096, merge=True,
+                                  droplets=dict(max_dE=max_dE, min_hamming=1, max_count=256))
+    E_all = brute.all_energies(inst)
+    gs = int(np.argmin(E_all))
+    assert out["states"].shape[0] == 1                       # the last cell has no boundary: everything merges
+    s0 = out["states"][0]
+    bits = ((1 - s0.astype(np.int64)) // 2)
+    assert int((bits << np.arange(24)).sum()) == gs and out["energies"][0] == E_all[gs]
+    drops = out["droplets"][0]
+    got = {}
+    for dE, mask in drops:
+        s1 = s0.copy()
+        s1[mask] *= -1
+        e1 = energy.energies(inst, s1[None])[0]
+        assert abs(dE - (e1 - out["energies"][0])) <= 1e-9   # ratio of exact marginals = Boltzmann factor
+        got[int((mask.astype(np.int64) << np.arange(24)).sum())] = dE
+    # brute force: all states within max_dE whose difference from the ground state is one connected piece
+    book = search.DropletBook(m)
+    want = set()
+    for idx in np.flatnonzero(E_all <= E_all[gs] + max_dE):
+        diff = int(idx) ^ gs
+        if diff == 0:
+            continue
+        sp = [i for i in range(24) if (diff >> i) & 1]
+        todo, seen, inset = [sp[0]], {sp[0]}, set(sp)
+        while todo:
+            u = todo.pop()
+            for v in book.adj[u]:
+                if v in inset and v not in seen:
+                    seen.add(v)
+                    todo.append(v)
+        if len(seen) == len(inset):
+            want.add(diff)
+    assert want and set(got) == want
+    first_excited = np.partition(E_all, 1)[1] - E_all[gs]
+    assert abs(min(got.values()) - first_excited) <= 1e-9
+    # the filters: a large Hamming threshold keeps fewer, pairwise distant droplets; max_count caps the list
+    far = search.branch_and_bound(m, R, ln, 4096, merge=True,
+                                  droplets=dict(max_dE=max_dE, min_hamming=3, max_count=256))["droplets"][0]
+    assert 0 < len(far) <= len(drops)
+    for i in range(len(far)):
+        for j in range(i):
+            assert int((far[i][1] ^ far[j][1]).sum()) >= 3
+    few = search.branch_and_bound(m, R, ln, 4096, merge=True,
+                                  droplets=dict(max_dE=max_dE, min_hamming=1, max_count=3))["droplets"][0]
+    assert [d for d, _ in few] == sorted(d for d, _ in drops)[:3]
