@@ -91,6 +91,12 @@ enum {
   TN_OPT_RSVD_ITERS = 14, /* subspace iterations of the randomized SVD (default 2)                             */
   TN_OPT_TWO_STEP = 15,   /* 0 (default) / 1: zipper and passes at bond 2 D, then canonical truncation to D
                              ("targeting 2 chi singular values ... further truncated to the target chi") */
+  /* ---- f1: droplets = excitation bookkeeping on top of the merge (Fig. 4; reading S24) */
+  TN_OPT_DROPLETS = 16,             /* 0 (default) / 1 (needs TN_OPT_MERGE): every main branch carries the low-energy
+                                       excitations that merged into it; read them with tn_droplets               */
+  TN_OPT_DROPLET_MAX_DE = 17,       /* energy cutoff of a droplet above its main branch (default 1.0)          */
+  TN_OPT_DROPLET_MIN_HAMMING = 18,  /* minimal pairwise Hamming distance of the droplets kept on one branch (default 1) */
+  TN_OPT_DROPLET_MAX_COUNT = 19,    /* droplets kept per branch (default 8, range 1..32)                        */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */
@@ -130,6 +136,7 @@ typedef struct {
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
   int64_t merge_fallback_cells; /* cells at which TN_OPT_MERGE could not merge (merge buffers too small at every threshold
                                 tried) and the selection ran unmerged; 0 = every cell followed Fig. 3(d)          */
+  int64_t droplet_overflow;  /* boundary groups whose droplet candidates exceeded the kernel's buffer (1024): 0 = none     */
   double flop_orth_svd;      /* algorithmic FLOP of the orthonormalisations: 2 Cholesky-QR rounds of 4 m k^2 each per call
                                 (Gram + apply; the rounds actually run are decided on the device, 1..5)             */
   double flop_search_rblocks;/* algorithmic FLOP of the right-block GEMMs (part of flop_search)                      */
@@ -187,6 +194,12 @@ int tn_mps_tensor(tn_handle*, int32_t y, int32_t j, double* out /* HOST dl*p*dr 
  * Ties: logp desc, then parent rank asc, then cell state asc (reading S8). */
 int tn_branch_and_bound(tn_handle*, int32_t M, int32_t* n_out, int8_t* states, double* energies,
                         double* logp, double* log_p_discarded);
+
+/* tn_droplets (f1, Fig. 4): the excitations book-kept above returned state `rank` of the last
+ * tn_branch_and_bound (needs TN_OPT_MERGE and TN_OPT_DROPLETS; TN_ERR_STATE otherwise).  *n <= TN_OPT_DROPLET_MAX_COUNT;
+ * dE HOST [max_count]: energy of main (+) flip above main, from the ratio of the marginals (increasing); flips HOST
+ * [max_count][n_spins] int8: 1 = the droplet flips that spin.  Either output may be NULL. */
+int tn_droplets(tn_handle*, int32_t rank, int32_t* n, double* dE, int8_t* flips);
 
 int tn_get_stats(tn_handle*, tn_stats* out /* HOST */);
 

@@ -11,10 +11,11 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_droplets", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 OPT_MERGE_CAP = 10
 OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
+OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT = 16, 17, 18, 19
 
 
 class TnError(RuntimeError):
@@ -30,7 +31,7 @@ class TnStats(C.Structure):
         "bytes_theta_apply", "flop_search", "bytes_search_cond", "bytes_search_select", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
             "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged",
-            "merge_fallback_cells")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
+            "merge_fallback_cells", "droplet_overflow")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -64,6 +65,7 @@ def lib():
         L.tn_branch_and_bound.argtypes = [C.c_void_p, C.c_int32, p_i32, p_i8, p_f64, p_f64, p_f64]
         L.tn_get_stats.argtypes = [C.c_void_p, C.POINTER(TnStats)]
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
+        L.tn_droplets.argtypes = [C.c_void_p, C.c_int32, p_i32, p_f64, p_i8]
         L.tn_fp64_peak.argtypes = [p_f64]
         L.tn_kernel_bench.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int64, C.c_int32, p_f64]
         L.tn_kernel_check.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, p_f64, p_f64, p_f64]
@@ -160,6 +162,15 @@ def tn_branch_and_bound(handle, M, n_spins):
                                      _ptr(logp, C.c_double), C.byref(pd)))
     k = n.value
     return states[:k], energies[:k], logp[:k], pd.value
+
+
+def tn_droplets(handle, rank, n_spins, max_count=32):
+    """Returns (dE [n], flips [n, n_spins] int8) of the droplets above returned state `rank` (include/tn.h)."""
+    n = C.c_int32()
+    dE = np.empty(max_count, dtype=np.float64)
+    flips = np.empty((max_count, n_spins), dtype=np.int8)
+    _check(lib().tn_droplets(handle, int(rank), C.byref(n), _ptr(dE, C.c_double), _ptr(flips, C.c_int8)))
+    return dE[:n.value].copy(), flips[:n.value].copy()
 
 
 def tn_energy(handle, states, n_spins=None):
@@ -262,6 +273,9 @@ class TensorNetwork:
 
     def branch_and_bound(self, M):
         return tn_branch_and_bound(self.handle, M, self.n_spins)
+
+    def droplets(self, rank):
+        return tn_droplets(self.handle, rank, self.n_spins)
 
     def energy(self, states):
         return tn_energy(self.handle, states, self.n_spins)

@@ -258,6 +258,16 @@ int tn_set_option(tn_handle* h, int32_t key, double v) {
       if (v < 1 || v > 100) tn_throw(TN_ERR_ARG, "randomized SVD iterations must be in 1..100");
       h->rsvd_iters = (int)v; break;
     case TN_OPT_TWO_STEP: h->two_step = v != 0.0; break;
+    case TN_OPT_DROPLETS: h->droplets = v != 0.0; break;
+    case TN_OPT_DROPLET_MAX_DE:
+      if (!(v >= 0.0) || !std::isfinite(v)) tn_throw(TN_ERR_ARG, "droplet energy cutoff must be finite and >= 0");
+      h->droplet_max_dE = v; break;
+    case TN_OPT_DROPLET_MIN_HAMMING:
+      if (v < 0 || v > 1e6) tn_throw(TN_ERR_ARG, "droplet Hamming threshold out of range");
+      h->droplet_min_hamming = (int)v; break;
+    case TN_OPT_DROPLET_MAX_COUNT:
+      if (v < 1 || v > 32) tn_throw(TN_ERR_ARG, "droplets per branch must be in 1..32");
+      h->droplet_max_count = (int)v; break;
     case TN_OPT_MERGE_CAP:
       if (v < 1 || v > (double)(1 << 24)) tn_throw(TN_ERR_ARG, "merge cap must be in 1..2^24");
       h->merge_cap = (i64)v; break;
@@ -364,6 +374,19 @@ int tn_branch_and_bound(tn_handle* h, int32_t M, int32_t* n_out, int8_t* states,
     throw;
   }
   trim_free_list(h);
+  TN_API_END
+}
+
+int tn_droplets(tn_handle* h, int32_t rank, int32_t* n, double* dE, int8_t* flips) {
+  TN_API_BEGIN
+  if (!h || !n) tn_throw(TN_ERR_ARG, "NULL argument");
+  if (h->drop_K == 0) tn_throw(TN_ERR_STATE, "tn_droplets: the last tn_branch_and_bound did not run with TN_OPT_MERGE and TN_OPT_DROPLETS");
+  if (rank < 0 || rank >= (int)h->drop_cnt.size()) tn_throw(TN_ERR_ARG, "rank out of range");
+  const int k = h->drop_cnt[rank];
+  *n = k;
+  if (dE) std::copy(h->drop_dE.begin() + (size_t)rank * h->drop_K, h->drop_dE.begin() + (size_t)rank * h->drop_K + k, dE);
+  if (flips) std::copy(h->drop_flips.begin() + (size_t)rank * h->drop_K * h->n_spins,
+                       h->drop_flips.begin() + ((size_t)rank * h->drop_K + k) * h->n_spins, flips);
   TN_API_END
 }
 

@@ -262,6 +262,7 @@ __global__ void k_beam_scale(const double* logp, const double* Z, int nb, double
   }
   mx = sh[0];
   for (int i = threadIdx.x; i < nb; i += blockDim.x) scale[i] = Z[i] > 0.0 ? exp(logp[i] - mx) / Z[i] : 0.0;
+  if (threadIdx.x == 0) scale[nb] = mx;   // key r = v fcd scale_m  <=>  score = log r + mx
 }
 
 // ---- top-M radix selection on r = v * fcd * scale (monotone in the score) ------------------------
@@ -523,6 +524,39 @@ __device__ __forceinline__ bool mcand_before(const MCand& x, const MCand& y) {
   if (x.parent != y.parent) return x.parent < y.parent;
   return x.state < y.state;
 }
+struct MergeLegs { const int *Pr, *Pd, *Po; int n_r, n_d, n_o, use_r, use_d, use_o; };
+__device__ __forceinline__ unsigned long long merge_gid(const MergeLegs& lg, const int* pid, int m, int a, int b, int cl) {
+  unsigned long long g = (unsigned long long)pid[m];
+  g = g * (unsigned long long)(lg.use_r ? lg.n_r : 1) + (unsigned long long)(lg.use_r ? lg.Pr[a] : 0);
+  g = g * (unsigned long long)(lg.use_d ? lg.n_d : 1) + (unsigned long long)(lg.use_d ? lg.Pd[b] : 0);
+  g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
+  return g;
+}
+// Droplet mode (TN_OPT_DROPLETS): every c_hi variant at or above the bound is a candidate (the interior variants are
+// the losers that become droplets), and with `gbest` the bound is per boundary group: dfac x the group's best key.
+__global__ void __launch_bounds__(256) k_sel_prefilter_all(SelArgs a, int lgA, int lgCl, double thr, double dfac,
+                                                           const unsigned long long* gbest, const int* pid, MergeLegs lg,
+                                                           Raw* out, unsigned* count, unsigned cap) {
+  const int m = blockIdx.y, nchunk = gridDim.x;
+  const i64 c0 = a.per_m * blockIdx.x / nchunk, c1 = a.per_m * (blockIdx.x + 1) / nchunk;
+  const double* v = a.V + (i64)m * a.per_m;
+  const double sc = a.scale[m];
+  for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
+    const double x = v[q];
+    if (!(x > 0.0)) continue;
+    const int i = (int)(q >> lgA), aa = (int)(q & (a.nA - 1)), cl = i & (a.nCl - 1), b = i >> lgCl;
+    double bound = thr;
+    if (gbest) bound = __longlong_as_double((long long)gbest[merge_gid(lg, pid, m, aa, b, cl)]) * dfac * (1.0 - 1e-12);
+    const double vs = x * sc;
+    for (int ch = 0; ch < a.nCh; ch++) {
+      const double r = vs * sel_fcd(a, m, cl, ch);
+      if (r > 0.0 && r >= bound) {
+        unsigned idx = atomicAdd(count, 1u);
+        if (idx < cap) out[idx] = Raw{m, i, aa, ch};
+      }
+    }
+  }
+}
 __global__ void __launch_bounds__(256) k_sel_prefilter_merge(SelArgs a, int lgA, double thr, const double* fmx, Raw* out,
                                                              unsigned* count, unsigned cap) {
   const int m = blockIdx.y, nchunk = gridDim.x;
@@ -552,7 +586,6 @@ __global__ void __launch_bounds__(256) k_sel_prefilter_merge(SelArgs a, int lgA,
     }
   }
 }
-struct MergeLegs { const int *Pr, *Pd, *Po; int n_r, n_d, n_o, use_r, use_d, use_o; };
 __global__ void k_merge_score(SelArgs a, const Raw* raw, unsigned n, unsigned npad, const double* logp, const double* Z,
                               int ns, int S, const int* pid, MergeLegs lg, MCand* out) {
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -576,13 +609,6 @@ __global__ void k_merge_score(SelArgs a, const Raw* raw, unsigned n, unsigned np
 // of r = v * scale_m * max_ch fcd (positive doubles order like integers; r is monotone in the score); pass 2: among
 // the entries that attain the maximum of their group, atomicMin of (parent << 32 | cell state) = the S8 tie-break;
 // pass 3: one candidate per non-empty group with its exact score.
-__device__ __forceinline__ unsigned long long merge_gid(const MergeLegs& lg, const int* pid, int m, int a, int b, int cl) {
-  unsigned long long g = (unsigned long long)pid[m];
-  g = g * (unsigned long long)(lg.use_r ? lg.n_r : 1) + (unsigned long long)(lg.use_r ? lg.Pr[a] : 0);
-  g = g * (unsigned long long)(lg.use_d ? lg.n_d : 1) + (unsigned long long)(lg.use_d ? lg.Pd[b] : 0);
-  g = g * (unsigned long long)(lg.use_o ? lg.n_o : 1) + (unsigned long long)(lg.use_o ? lg.Po[cl] : 0);
-  return g;
-}
 __device__ __forceinline__ unsigned merge_state(int a, int b, int cl, int ch, int ns, int S) {
   unsigned state = (unsigned)a;
   if (S >= 2) state |= (unsigned)b << ns;
@@ -688,12 +714,227 @@ static void bitonic_sort(tn_handle* h, T* c, unsigned n) {   // n a power of two
 }
 
 // first (= most probable, S8 order) member of every group of the sorted list
-__global__ void k_merge_first(const MCand* c, unsigned n, Cand* out, unsigned* count) {
+__global__ void k_merge_first(const MCand* c, unsigned n, Cand* out, unsigned* count, double sthr = -INFINITY,
+                              unsigned* count_thr = nullptr) {
   unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
   const MCand x = c[t];
   if (x.g == ~0ull) return;
-  if (t == 0 || c[t - 1].g != x.g) out[atomicAdd(count, 1u)] = Cand{x.score, x.parent, x.state};
+  if (t == 0 || c[t - 1].g != x.g) {
+    out[atomicAdd(count, 1u)] = Cand{x.score, x.parent, x.state};
+    if (count_thr && x.score >= sthr) atomicAdd(count_thr, 1u);   // winners at or above the selection bound itself
+  }
+}
+
+// ---- droplets (Fig. 4; reading S24) ---------------------------------------------------------
+// One CTA per new beam element i (= kept winner of a boundary group).  Candidates: the droplets its parent carries,
+// then every loser of its group within max_dE (sorted list `mc`: groups contiguous, S8 order inside), each followed by
+// its compositions with the droplets of the loser's parent.  They are sorted by (dE, generation order) and kept
+// greedily iff the flipped spins are one connected piece of the interaction graph and the Hamming distance to every
+// droplet already kept is >= min_hamming, up to max_count.
+struct DropArgs {
+  const MCand* mc; unsigned n_mc;                 // sorted survivors of this cell's merge
+  const Cand* beam; int nkeep;                    // new beam (sorted): parent, state, score
+  const unsigned* st_old; int ncell, cellidx;     // old beam states
+  const int* pid; MergeLegs lg; int ns, S, nCl;
+  const unsigned* pool_old; const double* dE_old; const int* cnt_old;   // [m][K][ncell], [m][K], [m]
+  unsigned* pool_new; double* dE_new; int* cnt_new;
+  int K; double max_dE, beta; int min_hamming;
+  const int* spin_of; int nbits;                  // [ncell][nbits]
+  const int *adj_ptr, *adj; int n_spins;
+  unsigned long long* overflow;
+};
+struct DCand { double dE; int seq, lparent, ldrop; unsigned lstate; };
+constexpr int DROP_CMAX = 1024;
+__global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
+  extern __shared__ unsigned char dsm_raw[];
+  DCand* cand = reinterpret_cast<DCand*>(dsm_raw);                       // DROP_CMAX
+  unsigned* fm = reinterpret_cast<unsigned*>(cand + DROP_CMAX);          // ncell
+  unsigned* inF = fm + a.ncell;                                          // (n_spins + 31) / 32
+  unsigned* reach = inF + (a.n_spins + 31) / 32;
+  int* list = reinterpret_cast<int*>(reach + (a.n_spins + 31) / 32);     // n_spins
+  __shared__ int s_n, s_scan[128], s_stop, s_cnt, s_changed, s_red[128];
+  const int i = blockIdx.x, tid = threadIdx.x;
+  const Cand w = a.beam[i];
+  const unsigned smask = (1u << a.ns) - 1, hmask = (1u << (a.ns / 2)) - 1;
+  const int wa = (int)(w.state & smask), wb = a.S == 1 ? wa : (int)((w.state >> a.ns) & smask);
+  const int wcl = a.S == 3 ? (int)((w.state >> (2 * a.ns)) & hmask) : 0;
+  const unsigned long long gw = merge_gid(a.lg, a.pid, w.parent, wa, wb, wcl);
+  // group start: lower bound of gw in the sorted list
+  unsigned lo = 0, hi = a.n_mc;
+  while (lo < hi) { unsigned mid = (lo + hi) >> 1; if (a.mc[mid].g < gw) lo = mid + 1; else hi = mid; }
+  // ---- candidates
+  const int nin = a.cnt_old[w.parent];
+  for (int k = tid; k < nin; k += 128) cand[k] = DCand{a.dE_old[(i64)w.parent * a.K + k], k, -1, k, 0u};
+  if (tid == 0) { s_n = nin; s_stop = 0; }
+  __syncthreads();
+  for (unsigned base = lo + 1; !s_stop; base += 128) {
+    const unsigned t = base + tid;
+    int mine = 0;
+    double dE = 0.0;
+    MCand l;
+    bool valid = false;
+    if (t < a.n_mc) {
+      l = a.mc[t];
+      if (l.g == gw) {
+        dE = (w.score - l.score) / a.beta;
+        valid = dE <= a.max_dE;
+      }
+    }
+    if (valid) {
+      mine = 1;
+      const int nl = a.cnt_old[l.parent];
+      for (int k = 0; k < nl; k++) mine += (dE + a.dE_old[(i64)l.parent * a.K + k] <= a.max_dE) ? 1 : 0;
+    }
+    s_scan[tid] = mine;
+    __syncthreads();
+    if (tid == 0) {
+      int run = s_n;
+      bool stop = false;
+      for (int q = 0; q < 128; q++) { const int c = s_scan[q]; s_scan[q] = run; run += c; if (c == 0) stop = true; }
+      s_n = run;
+      if (stop) s_stop = 1;
+    }
+    __syncthreads();
+    if (valid) {
+      int o = s_scan[tid];
+      if (o < DROP_CMAX) cand[o] = DCand{dE, o, l.parent, -1, l.state};
+      o++;
+      const int nl = a.cnt_old[l.parent];
+      for (int k = 0; k < nl; k++) {
+        const double d2 = dE + a.dE_old[(i64)l.parent * a.K + k];
+        if (d2 <= a.max_dE) { if (o < DROP_CMAX) cand[o] = DCand{d2, o, l.parent, k, l.state}; o++; }
+      }
+    }
+    __syncthreads();
+  }
+  int n = s_n;
+  if (n > DROP_CMAX) { if (tid == 0) atomicAdd(a.overflow, 1ull); n = DROP_CMAX; }
+  int np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  for (int k = n + tid; k < np2; k += 128) cand[k] = DCand{INFINITY, 0x7fffffff, -1, -1, 0u};
+  __syncthreads();
+  for (int k = 2; k <= np2; k <<= 1)
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int e = tid; e < np2; e += 128) {
+        const int o = e ^ j;
+        if (o > e) {
+          const DCand x = cand[e], y = cand[o];
+          const bool xy = x.dE < y.dE || (x.dE == y.dE && x.seq < y.seq);   // x before y
+          const bool up = (e & k) == 0;
+          if (up ? !xy : xy) { cand[e] = y; cand[o] = x; }
+        }
+      }
+      __syncthreads();
+    }
+  // ---- greedy selection
+  const int nw = (a.n_spins + 31) / 32;
+  int kept = 0;
+  unsigned* mine_pool = a.pool_new + (i64)i * a.K * a.ncell;
+  for (int c = 0; c < n && kept < a.K; c++) {
+    const DCand d = cand[c];
+    // flip mask over cells
+    int pop = 0;
+    for (int k = tid; k < a.ncell; k += 128) {
+      unsigned v = 0u;
+      if (k <= a.cellidx) {
+        if (d.lparent >= 0) {
+          v = k < a.cellidx ? (a.st_old[(i64)d.lparent * a.ncell + k] ^ a.st_old[(i64)w.parent * a.ncell + k])
+                            : (d.lstate ^ w.state);
+        }
+        if (d.ldrop >= 0) v ^= a.pool_old[((i64)(d.lparent >= 0 ? d.lparent : w.parent) * a.K + d.ldrop) * a.ncell + k];
+      }
+      fm[k] = v;
+      pop += __popc(v);
+    }
+    s_red[tid] = pop;
+    for (int k = tid; k < nw; k += 128) { inF[k] = 0u; reach[k] = 0u; }
+    __syncthreads();
+    if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
+    __syncthreads();
+    const int nflip = s_cnt;
+    if (nflip == 0) { __syncthreads(); continue; }
+    // Hamming distance to the kept ones
+    bool ok = true;
+    for (int j = 0; j < kept && ok; j++) {
+      int hd = 0;
+      for (int k = tid; k < a.ncell; k += 128) hd += __popc(fm[k] ^ mine_pool[(i64)j * a.ncell + k]);
+      __syncthreads();
+      s_red[tid] = hd;
+      __syncthreads();
+      if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
+      __syncthreads();
+      if (s_cnt < a.min_hamming) ok = false;
+    }
+    if (ok) {
+      // connectivity: list of flipped spins, label propagation from the first one
+      if (tid == 0) s_cnt = 0;
+      __syncthreads();
+      for (int k = tid; k < a.ncell; k += 128) {
+        unsigned v = fm[k];
+        while (v) {
+          const int bit = __ffs(v) - 1;
+          v &= v - 1;
+          const int sp = a.spin_of[k * a.nbits + bit];
+          list[atomicAdd(&s_cnt, 1)] = sp;
+          atomicOr(&inF[sp >> 5], 1u << (sp & 31));
+        }
+      }
+      __syncthreads();
+      if (tid == 0) { int mn = list[0]; for (int q = 1; q < nflip; q++) mn = min(mn, list[q]); reach[mn >> 5] |= 1u << (mn & 31); }
+      __syncthreads();
+      for (int round = 0; round < nflip; round++) {
+        if (tid == 0) s_changed = 0;
+        __syncthreads();
+        for (int q = tid; q < nflip; q += 128) {
+          const int u = list[q];
+          if (!((reach[u >> 5] >> (u & 31)) & 1u)) continue;
+          for (int e = a.adj_ptr[u]; e < a.adj_ptr[u + 1]; e++) {
+            const int v = a.adj[e];
+            if (((inF[v >> 5] >> (v & 31)) & 1u) && !((reach[v >> 5] >> (v & 31)) & 1u)) {
+              atomicOr(&reach[v >> 5], 1u << (v & 31));
+              s_changed = 1;
+            }
+          }
+        }
+        __syncthreads();
+        const int ch = s_changed;
+        __syncthreads();
+        if (!ch) break;
+      }
+      int rc = 0;
+      for (int k = tid; k < nw; k += 128) rc += __popc(reach[k]);
+      s_red[tid] = rc;
+      __syncthreads();
+      if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
+      __syncthreads();
+      if (s_cnt != nflip) ok = false;
+    }
+    if (ok) {
+      for (int k = tid; k < a.ncell; k += 128) mine_pool[(i64)kept * a.ncell + k] = fm[k];
+      if (tid == 0) a.dE_new[(i64)i * a.K + kept] = d.dE;
+      kept++;
+    }
+    __syncthreads();
+  }
+  if (tid == 0) a.cnt_new[i] = kept;
+}
+// cells selected without merging: the children inherit their parent's droplets unchanged
+__global__ void k_droplets_inherit(const Cand* beam, int nkeep, int K, int ncell, const unsigned* pool_old, const double* dE_old,
+                                   const int* cnt_old, unsigned* pool_new, double* dE_new, int* cnt_new) {
+  const int i = blockIdx.x, p = beam[i].parent, n = cnt_old[p];
+  for (i64 k = threadIdx.x; k < (i64)n * ncell; k += blockDim.x) pool_new[(i64)i * K * ncell + k] = pool_old[(i64)p * K * ncell + k];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) dE_new[(i64)i * K + k] = dE_old[(i64)p * K + k];
+  if (threadIdx.x == 0) cnt_new[i] = n;
+}
+// flips[(i, k)][spin] = 1 if droplet k of state i flips that spin
+__global__ void k_droplets_unpack(const unsigned* pool, int nstate, int K, int ncell, int n_spins, const int* cell_of,
+                                  const int* bit_of, int8_t* out) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)nstate * K * n_spins) return;
+  const int sp = (int)(t % n_spins);
+  const i64 ik = t / n_spins;
+  out[t] = (int8_t)((pool[ik * ncell + cell_of[sp]] >> bit_of[sp]) & 1u);
 }
 __global__ void k_fill_sentinel(Cand* c, unsigned from, unsigned to) {
   unsigned t = from + blockIdx.x * blockDim.x + threadIdx.x;
@@ -826,10 +1067,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   DBuf<unsigned> stA(h, (size_t)M * ncell), stB(h, (size_t)M * ncell);
   DBuf<double> lpA(h, M), lpB(h, M), LvA(h, (size_t)M * ldLv), LvB(h, (size_t)M * ldLv);
   DBuf<int> slA(h, M), slB(h, M), hrow(h, M), vrow(h, (size_t)M * Lx), drow(h, (size_t)M * Lx);
-  DBuf<double> Z(h, M), scale(h, M), pd(h, 1), fc(h, (size_t)M * 16);
+  DBuf<double> Z(h, M), scale(h, (size_t)M + 1), pd(h, 1), fc(h, (size_t)M * 16);
   DBuf<unsigned long long> nneg(h, 1);
   DBuf<SelState> sel(h, 1);
-  DBuf<unsigned> hist(h, 4096), count(h, 1);
+  DBuf<unsigned> hist(h, 4096), count(h, 2);
   DBuf<Raw> raw(h, cap);
   const unsigned ccap = 1u << 22;                   // compact candidate list of the prefilter pass
   DBuf<double> ckeys(h, ccap), fmx(h, (size_t)M * 16);
@@ -840,6 +1081,44 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   DBuf<MCand> mcand(h, h->merge ? mcap2 : 1);
   DBuf<Cand> mcands(h, h->merge ? mcap2 + 4096 : 1);
   DBuf<int> pid(h, M), chbest(h, h->merge ? (size_t)M * 16 : 1);
+  // ---- droplets (Fig. 4): double-buffered pools [beam element][K][cell] of xor masks, their dE and counts
+  const bool drops = h->merge && h->droplets;
+  const int dK = drops ? h->droplet_max_count : 1, nbits = S * ns;
+  const size_t dpool = drops ? (size_t)M * dK * ncell : 1;
+  DBuf<unsigned> dpA(h, dpool), dpB(h, dpool);
+  DBuf<double> ddA(h, (size_t)M * dK), ddB(h, (size_t)M * dK);
+  DBuf<int> dcA(h, M), dcB(h, M), d_spin_of(h, drops ? (size_t)ncell * nbits : 1), d_adj_ptr(h, drops ? (size_t)h->n_spins + 1 : 1);
+  DBuf<int> d_adj(h, drops ? 2 * (size_t)h->n_edges + 1 : 1);
+  DBuf<unsigned long long> d_dover(h, 1);
+  unsigned* dp_cur = dpA.p; unsigned* dp_nxt = dpB.p;
+  double* dd_cur = ddA.p; double* dd_nxt = ddB.p;
+  int* dc_cur = dcA.p; int* dc_nxt = dcB.p;
+  size_t drop_smem = 0;
+  if (drops) {
+    if (h->n_spins > 16384) tn_throw(TN_ERR_ARG, "TN_OPT_DROPLETS supports up to 16384 spins");
+    std::vector<int> spin_of((size_t)ncell * nbits, 0), aptr((size_t)h->n_spins + 1, 0), adj;
+    for (int i = 0; i < h->n_spins; i++) spin_of[(size_t)h->cell_of[i] * nbits + h->bit_of[i]] = i;
+    for (i64 e = 0; e < h->n_edges; e++)
+      if (h->J[e] != 0.0) { aptr[h->edge_u[e] + 1]++; aptr[h->edge_v[e] + 1]++; }
+    for (int i = 0; i < h->n_spins; i++) aptr[i + 1] += aptr[i];
+    adj.assign((size_t)aptr[h->n_spins] + 1, 0);
+    std::vector<int> fill(aptr.begin(), aptr.end() - 1);
+    for (i64 e = 0; e < h->n_edges; e++)
+      if (h->J[e] != 0.0) { adj[fill[h->edge_u[e]]++] = h->edge_v[e]; adj[fill[h->edge_v[e]]++] = h->edge_u[e]; }
+    TN_CUDA(cudaMemcpyAsync(d_spin_of.p, spin_of.data(), sizeof(int) * spin_of.size(), cudaMemcpyHostToDevice, h->stream));
+    TN_CUDA(cudaMemcpyAsync(d_adj_ptr.p, aptr.data(), sizeof(int) * aptr.size(), cudaMemcpyHostToDevice, h->stream));
+    TN_CUDA(cudaMemcpyAsync(d_adj.p, adj.data(), sizeof(int) * adj.size(), cudaMemcpyHostToDevice, h->stream));
+    TN_CUDA(cudaMemsetAsync(dpA.p, 0, sizeof(unsigned) * dpool, h->stream));
+    TN_CUDA(cudaMemsetAsync(dpB.p, 0, sizeof(unsigned) * dpool, h->stream));
+    TN_CUDA(cudaMemsetAsync(dcA.p, 0, sizeof(int) * M, h->stream));
+    TN_CUDA(cudaMemsetAsync(d_dover.p, 0, sizeof(unsigned long long), h->stream));
+    TN_CUDA(cudaStreamSynchronize(h->stream));   // the host vectors above go out of scope
+    drop_smem = sizeof(DCand) * DROP_CMAX + sizeof(unsigned) * ((size_t)ncell + 2 * ((h->n_spins + 31) / 32)) +
+                sizeof(int) * (size_t)h->n_spins;
+    TN_SMEM_OPT_IN(h, k_droplets, 200 * 1024);
+    if (drop_smem > 200 * 1024) tn_throw(TN_ERR_ARG, "TN_OPT_DROPLETS: lattice too large for the droplet kernel");
+  }
+  const double dfac = drops ? std::exp(-h->beta * h->droplet_max_dE) * (1.0 - 1e-9) : 1.0;
   DBuf<unsigned long long> gbest(h, 2 * (size_t)mcap + 2);   // [mcap] group maxima, [mcap] tie-breaks, [1] positive-entry count
   DBuf<Cand> cand(h, npad);
   unsigned* st_cur = stA.p; unsigned* st_nxt = stB.p;
@@ -1005,6 +1284,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       bool direct = total * c.nCh <= (i64)h->select_direct_max;       // few candidates: radix passes straight on V
       bool cand_sorted = false;                                       // set by the merge route (cand.p final and sorted)
       unsigned np2 = 2;
+      unsigned n_mc = 0;   // entries of the sorted survivor list mcand of this cell (droplet mode)
       if (h->merge) {
         // ---- parent part of the boundary: dense ids of the projected forward legs of rows y-1, y (host, tiny)
         std::vector<unsigned> hst((size_t)nb * ncell);
@@ -1040,6 +1320,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         const bool seg = gposs <= (double)mcap;
         bool ok = false;
         unsigned n1 = 0, ng = 0;
+        int lgClm = 0;
+        while ((1 << lgClm) < c.nCl) lgClm++;
+        const double mxlp = drops ? d2h(h, scale.p + nb) : 0.0;
         if (seg) {
           // ---- few possible boundaries (always so in the last column and the last row): segmented arg-max over all of V
           const i64 ngroups = (i64)gposs;
@@ -1054,14 +1337,34 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           const int nch2 = (int)std::max<i64>(1, std::min<i64>(64, per_m / 4096));
           k_merge_seg<1><<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, fmx.p, chbest.p, pid.p, lg, ns, S, gbest.p, gt, npos);
           TN_LAUNCH_CHECK(h);
-          k_merge_seg<2><<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, fmx.p, chbest.p, pid.p, lg, ns, S, gbest.p, gt, npos);
-          TN_LAUNCH_CHECK(h);
-          k_merge_seg_emit<<<cdiv(ngroups, 256), 256, 0, h->stream>>>(sa, gbest.p, gt, ngroups, lp_cur, Z.p, ns, S, mcands.p, count.p);
-          TN_LAUNCH_CHECK(h);
           h->st.bytes_search_select += 2.0 * 8.0 * nb * (double)per_m;
-          ng = d2h(h, count.p);
-          n1 = (unsigned)std::min<unsigned long long>(d2h(h, npos), 0xffffffffull);
-          ok = true;
+          if (!drops) {
+            k_merge_seg<2><<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, fmx.p, chbest.p, pid.p, lg, ns, S, gbest.p, gt, npos);
+            TN_LAUNCH_CHECK(h);
+            k_merge_seg_emit<<<cdiv(ngroups, 256), 256, 0, h->stream>>>(sa, gbest.p, gt, ngroups, lp_cur, Z.p, ns, S, mcands.p, count.p);
+            TN_LAUNCH_CHECK(h);
+            ng = d2h(h, count.p);
+            n1 = (unsigned)std::min<unsigned long long>(d2h(h, npos), 0xffffffffull);
+            ok = true;
+          } else {
+            // droplet mode: every candidate within max_dE of its group's best (all c_hi variants) is needed as a loser
+            k_sel_prefilter_all<<<dim3(nch2, nb), 256, 0, h->stream>>>(sa, lgA, lgCl, 0.0, dfac, gbest.p, pid.p, lg, craw.p, count.p, mcap);
+            TN_LAUNCH_CHECK(h);
+            n1 = d2h(h, count.p);
+            if (n1 <= mcap && n1 > 0) {
+              n_mc = n1;
+              unsigned mp2 = 2;
+              while (mp2 < n1 + 1) mp2 <<= 1;
+              k_merge_score<<<cdiv(mp2, 256), 256, 0, h->stream>>>(sa, craw.p, n1, mp2, lp_cur, Z.p, ns, S, pid.p, lg, mcand.p);
+              TN_LAUNCH_CHECK(h);
+              bitonic_sort<MCand, LessM>(h, mcand.p, mp2);
+              TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+              k_merge_first<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, mcands.p, count.p);
+              TN_LAUNCH_CHECK(h);
+              ng = d2h(h, count.p);
+              ok = true;
+            }
+          }
         }
         double thr = 0.0;                                // few candidates: take every positive entry
         if (!seg && !direct) {
@@ -1084,7 +1387,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         double thr_few = -1.0, thr_many = -1.0;          // last thresholds with too few groups / too many survivors
         for (int attempt = 0; !seg && attempt < max_attempts; attempt++) {
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
-          k_sel_prefilter_merge<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, thr, fmx.p, craw.p, count.p, mcap);
+          if (drops)
+            k_sel_prefilter_all<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, lgClm, thr * dfac, dfac, nullptr, pid.p, lg, craw.p, count.p, mcap);
+          else
+            k_sel_prefilter_merge<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, thr, fmx.p, craw.p, count.p, mcap);
           h->st.bytes_search_select += 8.0 * nb * (double)per_m * (attempt == 0 && !direct ? 1.0 + 2.0 / 64.0 : 1.0);
           TN_LAUNCH_CHECK(h);
           n1 = d2h(h, count.p);
@@ -1101,11 +1407,16 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           k_merge_score<<<cdiv(mp2, 256), 256, 0, h->stream>>>(sa, craw.p, n1, mp2, lp_cur, Z.p, ns, S, pid.p, lg, mcand.p);
           TN_LAUNCH_CHECK(h);
           bitonic_sort<MCand, LessM>(h, mcand.p, mp2);
-          TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
-          k_merge_first<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, mcands.p, count.p);
+          TN_CUDA(cudaMemsetAsync(count.p, 0, 2 * sizeof(unsigned), h->stream));
+          k_merge_first<<<cdiv(mp2, 256), 256, 0, h->stream>>>(mcand.p, mp2, mcands.p, count.p,
+                                                               drops && thr > 0.0 ? std::log(thr) + mxlp : -INFINITY,
+                                                               drops ? count.p + 1 : nullptr);
           TN_LAUNCH_CHECK(h);
           ng = d2h(h, count.p);
-          if (ng >= (unsigned)M + 1 || thr == 0.0) { ok = true; break; }
+          n_mc = n1;
+          // droplet mode: the list reaches down to thr * dfac, but M + 1 WINNERS must lie at or above thr itself
+          const unsigned ng_sel = drops ? d2h(h, count.p + 1) : ng;
+          if (ng_sel >= (unsigned)M + 1 || thr == 0.0) { ok = true; break; }
           thr_few = thr;                                 // fewer than M + 1 boundaries above the bound: lower it
           if (thr_many > 0.0) thr = std::sqrt(thr_few) * std::sqrt(thr_many);
           else thr = thr > 1e-290 ? thr / 64.0 : 0.0;
@@ -1213,6 +1524,20 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       k_new_beam<<<nkeep, 128, 0, h->stream>>>(cand_final, nkeep, M, st_cur, st_nxt, ncell, cellidx, sl_cur, sl_nxt, lp_nxt,
                                                LG.p, npp, Dr, ldLv, Lv_nxt, c.Pd, c.Po, c.n_o, ns, S, pd.p);
       TN_LAUNCH_CHECK(h);
+      if (drops) {
+        if (cand_sorted && n_mc > 0) {
+          MergeLegs lgd{c.Pr, c.Pd, c.Po, c.n_r, c.n_d, c.n_o, x + 1 < Lx, y + 1 < Ly, S == 3 && x + 1 < Lx && y + 1 < Ly};
+          DropArgs da{mcand.p, n_mc, cand_final, nkeep, st_cur, ncell, cellidx, pid.p, lgd, ns, S, c.nCl,
+                      dp_cur, dd_cur, dc_cur, dp_nxt, dd_nxt, dc_nxt, dK, h->droplet_max_dE, h->beta, h->droplet_min_hamming,
+                      d_spin_of.p, nbits, d_adj_ptr.p, d_adj.p, h->n_spins, d_dover.p};
+          k_droplets<<<nkeep, 128, drop_smem, h->stream>>>(da);
+          TN_LAUNCH_CHECK(h);
+        } else {
+          k_droplets_inherit<<<nkeep, 128, 0, h->stream>>>(cand_final, nkeep, dK, ncell, dp_cur, dd_cur, dc_cur, dp_nxt, dd_nxt, dc_nxt);
+          TN_LAUNCH_CHECK(h);
+        }
+        std::swap(dp_cur, dp_nxt); std::swap(dd_cur, dd_nxt); std::swap(dc_cur, dc_nxt);
+      }
       std::swap(st_cur, st_nxt); std::swap(lp_cur, lp_nxt); std::swap(Lv_cur, Lv_nxt); std::swap(sl_cur, sl_nxt);
       nb = nkeep;
       t_s.stop();
@@ -1233,6 +1558,23 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
   TN_CUDA(cudaMemcpyAsync(&pdv, pd.p, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   unsigned long long neg = 0;
   TN_CUDA(cudaMemcpyAsync(&neg, nneg.p, sizeof(neg), cudaMemcpyDeviceToHost, h->stream));
+  h->drop_cnt.clear(); h->drop_dE.clear(); h->drop_flips.clear();
+  h->drop_K = 0;
+  if (drops) {
+    DBuf<int8_t> dfl(h, (size_t)nb * dK * h->n_spins);
+    k_droplets_unpack<<<cdiv((i64)nb * dK * h->n_spins, 256), 256, 0, h->stream>>>(dp_cur, nb, dK, ncell, h->n_spins, h->d_cell_of,
+                                                                                  h->d_bit_of, dfl.p);
+    TN_LAUNCH_CHECK(h);
+    h->drop_K = dK;
+    h->drop_cnt.resize(nb); h->drop_dE.resize((size_t)nb * dK); h->drop_flips.resize((size_t)nb * dK * h->n_spins);
+    TN_CUDA(cudaMemcpyAsync(h->drop_cnt.data(), dc_cur, sizeof(int) * nb, cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaMemcpyAsync(h->drop_dE.data(), dd_cur, sizeof(double) * nb * dK, cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaMemcpyAsync(h->drop_flips.data(), dfl.p, (size_t)nb * dK * h->n_spins, cudaMemcpyDeviceToHost, h->stream));
+    unsigned long long over = 0;
+    TN_CUDA(cudaMemcpyAsync(&over, d_dover.p, sizeof(over), cudaMemcpyDeviceToHost, h->stream));
+    TN_CUDA(cudaStreamSynchronize(h->stream));
+    h->st.droplet_overflow += (int64_t)over;
+  }
   TN_CUDA(cudaStreamSynchronize(h->stream));
   *n_out = nb;
   if (log_pd_out) *log_pd_out = pdv;

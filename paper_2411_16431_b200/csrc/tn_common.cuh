@@ -84,6 +84,12 @@ struct tn_handle {
   int D = 0, sweeps = 0;
   // options
   int merge = 0;            // TN_OPT_MERGE: merge candidates by boundary before the bound (Fig. 3(d))
+  int droplets = 0, droplet_min_hamming = 1, droplet_max_count = 8;   // TN_OPT_DROPLETS ... (Fig. 4)
+  double droplet_max_dE = 1.0;
+  std::vector<int> drop_cnt;          // results of the last tn_branch_and_bound: droplets per returned state,
+  std::vector<double> drop_dE;        //   [state][K] excitation energies,
+  std::vector<int8_t> drop_flips;     //   [state][K][n_spins] flip masks
+  int drop_K = 0;
   i64 merge_cap = 1ll << 20;  // TN_OPT_MERGE_CAP: survivors / boundary groups the merge buffers hold
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
   int schedule = 0, sweep_range = 2, svd_mode = 0, rsvd_iters = 2, two_step = 0;   // f2 (TN_OPT_SCHEDULE ...)

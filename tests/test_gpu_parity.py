@@ -345,6 +345,61 @@ def test_f2_fast_mode_close_to_converged_mode():
     assert out[1][5]["svd_unconverged"] == 0 and out[1][5]["svd_iterations"] > 0
 
 
+DROPS = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, max_dE, min_hamming, max_count)
+    (2, 3, 2, 2, 1.0, 3, 2.0, 0, 0, 64, 1.2, 1, 16),          # the brute-force pin's lattice (exact D)
+    (3, 3, 3, 2, 0.85, 7, 0.9, 0, 0, 32, 1.5, 1, 8),          # mediating tensors: c_hi variants are interior droplets
+    (4, 4, 2, 4, 0.95, 2, 1.0, 6, 1, 64, 1.0, 2, 8),          # truncated D, ragged projectors, Hamming filter
+    (3, 3, 3, 4, 0.9, 4, 1.0, 6, 2, 64, 0.8, 1, 4),           # 4096 states per cell, list capped at 4
+    (3, 4, 1, 4, 1.0, 6, 2.0, 5, 1, 16, 2.0, 3, 8),
+]
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,beta,D,sweeps,M,max_dE,min_h,max_count", DROPS)
+@pytest.mark.parametrize("route", ["segmented", "threshold"])
+def test_droplets_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, max_dE, min_h, max_count, route):
+    """TN_OPT_DROPLETS (Fig. 4) against the oracle's DropletBook: for every returned state the same
+    droplets -- identical flip masks, dE within the tolerance that the log-probabilities carry -- through both merge
+    routes (segmented arg-max with per-group bounds; threshold + sort, forced by a small TN_OPT_MERGE_CAP)."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    tol = 1e-9 if D == 0 else 1e-6
+    m = model.Model(inst).set_beta(beta)
+    R, ln = mps.contract(m, D, sweeps)
+    ref = search.branch_and_bound(m, R, ln, M, merge=True,
+                                  droplets=dict(max_dE=max_dE, min_hamming=min_h, max_count=max_count))
+    with _tn(inst) as t:
+        for k, v in ((tnb.OPT_MERGE, 1), (tnb.OPT_DROPLETS, 1), (tnb.OPT_DROPLET_MAX_DE, max_dE),
+                     (tnb.OPT_DROPLET_MIN_HAMMING, min_h), (tnb.OPT_DROPLET_MAX_COUNT, max_count),
+                     (tnb.OPT_SELECT_DIRECT_MAX, 0)):
+            t.set_option(k, v)
+        if route == "threshold":
+            t.set_option(tnb.OPT_MERGE_CAP, 4096)
+        t.set_beta(beta)
+        t.contract(D, sweeps)
+        states, E, logp, pd = t.branch_and_bound(M)
+        st = t.stats()
+        got = [t.droplets(r) for r in range(states.shape[0])]
+    assert st["merge_fallback_cells"] == 0 and st["droplet_overflow"] == 0
+    check_lists(inst, ref, states, E, logp, pd, tol)
+    dtol = 4 * tol * np.abs(ref["logp"]).max() / beta
+    total = 0
+    for r in range(states.shape[0]):
+        if not np.array_equal(states[r], ref["states"][r]):
+            continue                                           # a tie inside the tolerance (check_lists accepted it)
+        dE, flips = got[r]
+        want = ref["droplets"][r]
+        assert len(dE) == len(want), (r, len(dE), len(want))
+        for k, (wE, wmask) in enumerate(want):
+            assert abs(dE[k] - wE) <= dtol, (r, k, dE[k], wE)
+            assert np.array_equal(flips[k].astype(bool), wmask), (r, k)
+            s1 = states[r].copy()
+            s1[wmask] *= -1
+            if D == 0:                                         # exact marginals: dE IS the energy of the excitation
+                assert abs(energy.energies(inst, s1[None])[0] - E[r] - dE[k]) <= 1e-8
+        total += len(want)
+    assert total > 0
+
+
 EDGE = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, h): the degenerate shapes the method has
     (1, 3, 2, 2, 1.0, 1, 1.0, 0, 0, 8, "uniform"),       # one row: no boundary MPS at all
     (1, 1, 3, 2, 1.0, 1, 1.0, 0, 0, 8, "uniform"),       # one cell
