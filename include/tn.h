@@ -97,6 +97,8 @@ enum {
   TN_OPT_DROPLET_MAX_DE = 17,       /* energy cutoff of a droplet above its main branch (default 1.0)          */
   TN_OPT_DROPLET_MIN_HAMMING = 18,  /* minimal pairwise Hamming distance of the droplets kept on one branch (default 1) */
   TN_OPT_DROPLET_MAX_COUNT = 19,    /* droplets kept per branch (default 8, range 1..32)                        */
+  TN_OPT_MERGE_SEGMENTED = 20,      /* 1 (default) / 0: allow the segmented arg-max route of the merge (taken when the possible
+                                       boundaries of a cell fit TN_OPT_MERGE_CAP); 0 forces threshold + sort everywhere   */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */

@@ -16,6 +16,7 @@ OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SE
 OPT_MERGE_CAP = 10
 OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
 OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT = 16, 17, 18, 19
+OPT_MERGE_SEGMENTED = 20
 
 
 class TnError(RuntimeError):

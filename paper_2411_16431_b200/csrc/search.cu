@@ -1317,7 +1317,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         TN_LAUNCH_CHECK(h);
         // number of POSSIBLE boundaries of the candidates of this cell
         const double gposs = (double)ids.size() * (lg.use_r ? lg.n_r : 1) * (lg.use_d ? lg.n_d : 1) * (lg.use_o ? lg.n_o : 1);
-        const bool seg = gposs <= (double)mcap;
+        const bool seg = h->merge_segmented && gposs <= (double)mcap;
         bool ok = false;
         unsigned n1 = 0, ng = 0;
         int lgClm = 0;
@@ -1395,9 +1395,13 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           TN_LAUNCH_CHECK(h);
           n1 = d2h(h, count.p);
           if (n1 > mcap) {                               // too many survivors for the merge buffers
-            thr_many = thr;
+            if (thr <= 0.0) {                                                   // every positive entry, still too many:
+              if (thr_few <= 0.0) break;                                        //   nothing to bisect against
+              thr_many = thr_few * 1e-80;                                       //   the bound lies somewhere below thr_few
+            } else {
+              thr_many = thr;
+            }
             if (thr_few > 0.0 && !(thr_few > thr_many * (1.0 + 1e-9))) break;   // the two bounds met: no threshold fits
-            if (thr <= 0.0) break;                                              // every positive entry, still too many
             thr = thr_few > 0.0 ? std::sqrt(thr_few) * std::sqrt(thr_many) : thr * 8.0;
             continue;
           }
@@ -1419,7 +1423,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           if (ng_sel >= (unsigned)M + 1 || thr == 0.0) { ok = true; break; }
           thr_few = thr;                                 // fewer than M + 1 boundaries above the bound: lower it
           if (thr_many > 0.0) thr = std::sqrt(thr_few) * std::sqrt(thr_many);
-          else thr = thr > 1e-290 ? thr / 64.0 : 0.0;
+          else thr = (attempt < 3 && thr > 1e-290) ? thr / 64.0 : 0.0;       // a few steps down, then every positive entry
         }
         if (ok) {
           if (ng == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);

@@ -268,8 +268,10 @@ def test_merge_by_boundary_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, sa
 @pytest.mark.parametrize("cap,expect_fallback", [(1 << 20, False), (512, False), (8, True)])
 def test_merge_routes_and_counted_fallback(cap, expect_fallback):
     """TN_OPT_MERGE has two routes: a segmented arg-max over all candidates when the possible boundaries of a cell fit
-    the merge buffers (TN_OPT_MERGE_CAP), else threshold + sort with a bisected threshold.  cap = 512 forces the
-    threshold route with bisection on most cells of this lattice; both must reproduce the oracle's merge=True.  A cell
+    the merge buffers (TN_OPT_MERGE_CAP), else threshold + sort with a bisected threshold.  cap = 512 sends the middle
+    cells of this lattice (up to 16384 possible boundaries) through the threshold route with fewer buffer slots than
+    the sampled bound leaves survivors (bisection), the rest through the segmented one; both must reproduce the
+    oracle's merge=True.  A cell
     that fits neither route (cap = 8) is selected unmerged and COUNTED in merge_fallback_cells -- never silently."""
     import paper_2411_16431_b200 as tnb
     inst = instances.lattice(4, 4, 2, 4, p_keep=0.95, seed=2)
@@ -359,7 +361,7 @@ DROPS = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M, max_dE, min_hamm
 def test_droplets_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, max_dE, min_h, max_count, route):
     """TN_OPT_DROPLETS (Fig. 4) against the oracle's DropletBook: for every returned state the same
     droplets -- identical flip masks, dE within the tolerance that the log-probabilities carry -- through both merge
-    routes (segmented arg-max with per-group bounds; threshold + sort, forced by a small TN_OPT_MERGE_CAP)."""
+    routes (segmented arg-max with per-group bounds; threshold + sort, forced by TN_OPT_MERGE_SEGMENTED = 0)."""
     import paper_2411_16431_b200 as tnb
     inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
     tol = 1e-9 if D == 0 else 1e-6
@@ -373,7 +375,7 @@ def test_droplets_parity(Ly, Lx, S, ns, p, seed, beta, D, sweeps, M, max_dE, min
                      (tnb.OPT_SELECT_DIRECT_MAX, 0)):
             t.set_option(k, v)
         if route == "threshold":
-            t.set_option(tnb.OPT_MERGE_CAP, 4096)
+            t.set_option(tnb.OPT_MERGE_SEGMENTED, 0)
         t.set_beta(beta)
         t.contract(D, sweeps)
         states, E, logp, pd = t.branch_and_bound(M)
