@@ -56,6 +56,8 @@ def parse_args():
                     help="N = 1 with --replicas transforms: run the 8 maps as concurrent replicas on this many "
                          "CUDA streams (one host thread per stream)")
     ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
+    ap.add_argument("--droplets", action="store_true",
+                    help="TN_OPT_DROPLETS on top of --merge: book-keep the excitations above every main branch (Fig. 4)")
     ap.add_argument("--transform", type=int, default=0,
                     help="lattice transformation 0..7 (PAPER.md:270; instances.transformed; Zephyr-shaped configs only)")
     return ap.parse_args()
@@ -449,8 +451,13 @@ def run_ours(args):
 
     def make_tn(ins):
         t = tnb.TensorNetwork(ins)
-        if args.merge:
+        if args.merge or args.droplets:
             t.set_option(tnb.OPT_MERGE, 1)
+        if args.droplets:
+            t.set_option(tnb.OPT_DROPLETS, 1)
+            t.set_option(tnb.OPT_DROPLET_MAX_COUNT, 32)
+            t.set_option(tnb.OPT_DROPLET_MAX_DE, 0.01 * abs(float(inst.E0)) if "E0" in inst else 1.0)
+            t.set_option(tnb.OPT_DROPLET_MIN_HAMMING, max(1, inst.n_spins // 4) if "E0" in inst else 1)
         return t
 
     def step(t, b, r):
@@ -497,6 +504,16 @@ def run_ours(args):
     barrier()
     st = t.stats()                                               # stage timers of the last timed step
     log_z = t.log_z()
+    drop_states = None
+    if args.droplets:                                            # main branches and their single-droplet excitations
+        states0 = outs[0]
+        ex = [states0]
+        for r in range(states0.shape[0]):
+            dE, flips = t.droplets(r)
+            if len(dE):
+                ex.append((states0[r][None, :].astype(np.int32) * (1 - 2 * flips.astype(np.int32))).astype(np.int8))
+        drop_states = np.concatenate(ex, axis=0)
+        drop_E = t.energy(drop_states)                           # O-0 energies on the device (tn_energy)
     alone = kernel_alone(t, inst, run) if rank == 0 else None
     t.close()
 
@@ -558,6 +575,12 @@ def run_ours(args):
         line["replicas"] = replicas
     if "E0" in inst:
         line["planted"] = diversity_report(inst, states, E)
+    if drop_states is not None:
+        Ed = drop_E
+        line["droplets"] = {"main_branches": int(states.shape[0]), "states_with_single_droplets": int(drop_states.shape[0]),
+                            "droplet_overflow": int(st["droplet_overflow"])}
+        if "E0" in inst:
+            line["droplets"]["planted"] = diversity_report(inst, drop_states, Ed)
     if e2e_ms is not None:
         line["e2e"] = {"value": whole_job_value(e2e_ms, K, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h}
