@@ -58,6 +58,8 @@ def parse_args():
     ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
     ap.add_argument("--droplets", action="store_true",
                     help="TN_OPT_DROPLETS on top of --merge: book-keep the excitations above every main branch (Fig. 4)")
+    ap.add_argument("--droplet-max-de", type=float, default=2.0, help="TN_OPT_DROPLET_MAX_DE (energy units of J)")
+    ap.add_argument("--droplet-min-hamming", type=int, default=2, help="TN_OPT_DROPLET_MIN_HAMMING")
     ap.add_argument("--transform", type=int, default=0,
                     help="lattice transformation 0..7 (PAPER.md:270; instances.transformed; Zephyr-shaped configs only)")
     return ap.parse_args()
@@ -455,9 +457,9 @@ def run_ours(args):
             t.set_option(tnb.OPT_MERGE, 1)
         if args.droplets:
             t.set_option(tnb.OPT_DROPLETS, 1)
-            t.set_option(tnb.OPT_DROPLET_MAX_COUNT, 32)
-            t.set_option(tnb.OPT_DROPLET_MAX_DE, 0.01 * abs(float(inst.E0)) if "E0" in inst else 1.0)
-            t.set_option(tnb.OPT_DROPLET_MIN_HAMMING, max(1, inst.n_spins // 4) if "E0" in inst else 1)
+            t.set_option(tnb.OPT_DROPLET_MAX_COUNT, 16)
+            t.set_option(tnb.OPT_DROPLET_MAX_DE, args.droplet_max_de)
+            t.set_option(tnb.OPT_DROPLET_MIN_HAMMING, args.droplet_min_hamming)
         return t
 
     def step(t, b, r):

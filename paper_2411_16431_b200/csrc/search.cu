@@ -38,10 +38,11 @@ struct LdPA {   // A(m; i=(b,cl), k) = LG[m][(Pd b * n_o + Po cl)][k]
     return LG[((i64)m * npp + Pd[b] * n_o + Po[cl]) * Dr + k];
   }
 };
-struct LdPB {   // B(m; k, a) = RM[slot m][k][Pr a]
-  const double* RM; const int *slot, *Pr; int Dr, n_r;
+struct LdPB {   // B(m; k, a) = RM[slot m][k][Pr a] * cs[m][a]: the column weights h wA ride on the small operand, so the
+                // epilogue of the conditional GEMM has only row-wise factors left (it was issue-bound on per-element loads)
+  const double* RM; const int *slot, *Pr; int Dr, n_r; const double* cs; int nA;
   __device__ __forceinline__ double operator()(int m, int k, int a) const {
-    return RM[((i64)slot[m] * Dr + k) * n_r + Pr[a]];
+    return RM[((i64)slot[m] * Dr + k) * n_r + Pr[a]] * cs[(i64)m * nA + a];
   }
 };
 struct StPV {
@@ -49,7 +50,8 @@ struct StPV {
   int nA, nB, nCl, tshift; i64 per_m;
   __device__ __forceinline__ void operator()(int m, int, int i, int a, double acc) const {
     int b = i / nCl, cl = i % nCl;
-    double w = hS[(i64)hrow[m] * nA + a] * wA[a] * X[(a >> tshift) * nB + b] * vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl];
+    // (the column weights hS wA are already inside the B operand, LdPB)
+    double w = X[(a >> tshift) * nB + b] * vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl];
     V[(i64)m * per_m + (i64)i * nA + a] = acc * w;
   }
 };
@@ -61,33 +63,35 @@ struct ArPV {
   }
 };
 struct EpPV {   // stores V and, fused, collects Z_m = sum max(v, 0) fc[m][cl] and the count of negative entries
-  double* V; const double *cs, *X, *vS, *Yc, *fc; const int *vrow, *slot;
+  double* V; const double *X, *vS, *Yc, *fc; const int *vrow, *slot;
   double* zpart; unsigned long long* nneg;
   int nA, nB, nCl, tshift, ntile; i64 per_m;
   static constexpr bool kReduce = true;
-  struct Row { double* p; const double* x; const double* c; double w, f, z; unsigned neg; };
+  struct Row { double* p; const double* x; double w, f, z; unsigned neg; };
   __device__ __forceinline__ Row row(int m, int i) const {
     const int b = i / nCl, cl = i % nCl;
-    return Row{V + (i64)m * per_m + (i64)i * nA, X + b, cs + (i64)m * nA, vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl],
+    return Row{V + (i64)m * per_m + (i64)i * nA, X + b, vS[(i64)vrow[slot[m]] * nB + b] * Yc[b * nCl + cl],
                fc[(i64)m * nCl + cl], 0.0, 0u};
   }
-  __device__ __forceinline__ void tally(Row& r, double v) const {
-    if (v > 0.0) r.z += v * r.f;
-    else if (v < 0.0) r.neg++;
+  __device__ __forceinline__ void tally(Row& r, double v) const {   // the row factor fc[m][cl] is applied once, in collect
+    r.z += fmax(v, 0.0);
+    r.neg += v >= 0.0 ? 0u : 1u;   // negatives AND NaNs are counted (reading S7), as in the k_beam_Z route
   }
   __device__ __forceinline__ void put(Row& r, int, int a, double v) const {
-    const double o = v * r.w * r.c[a] * r.x[(a >> tshift) * nB];
+    const double o = v * (r.w * r.x[(a >> tshift) * nB]);
     r.p[a] = o;
     tally(r, o);
   }
   __device__ __forceinline__ void put2(Row& r, int, int a, double v0, double v1) const {
-    const double o0 = v0 * r.w * r.c[a] * r.x[(a >> tshift) * nB], o1 = v1 * r.w * r.c[a + 1] * r.x[((a + 1) >> tshift) * nB];
+    const double t0 = r.w * r.x[(a >> tshift) * nB];
+    const double t1 = tshift > 0 && !(a & 1) ? t0 : r.w * r.x[((a + 1) >> tshift) * nB];   // a even: same a_hi
+    const double o0 = v0 * t0, o1 = v1 * t1;
     if (((nA | a) & 1) == 0) *reinterpret_cast<double2*>(r.p + a) = make_double2(o0, o1);
     else { r.p[a] = o0; r.p[a + 1] = o1; }
     tally(r, o0);
     tally(r, o1);
   }
-  __device__ __forceinline__ void collect(const Row& r, double& z, unsigned& n) const { z += r.z; n += r.neg; }
+  __device__ __forceinline__ void collect(const Row& r, double& z, unsigned& n) const { z += r.z * r.f; n += r.neg; }
   __device__ __forceinline__ void tile_done(int m, int tile, double z, unsigned n) const {
     zpart[(i64)m * ntile + tile] = z;
     if (n) atomicAdd(nneg, (unsigned long long)n);
@@ -1230,10 +1234,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         k_colscale<<<cdiv((i64)nb * c.nA, 256), 256, 0, h->stream>>>(c.BhS, c.wA, hrow.p, nb, c.nA, cs.p);
         TN_LAUNCH_CHECK(h);
         ArPV ar{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
-        LdPB be{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r};
+        LdPB be{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r, cs.p, c.nA};
         const int ntile = (Mg + 127) / 128;
         DBuf<double> zpart(h, (size_t)nb * std::max(ntile, 64));
-        EpPV ep{V.p, cs.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
+        EpPV ep{V.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
                 c.nA, c.nB, c.nCl, c.tshift, ntile, per_m};
         if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
           // Z and the negative count came out of the GEMM epilogue: no extra pass over V
@@ -1383,7 +1387,7 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         }
         // The threshold is lowered (/ 64) while fewer than M + 1 boundaries lie above it and raised again (geometric
         // bisection) when more candidates than the merge buffers hold lie above it.
-        const int max_attempts = 40;
+        const int max_attempts = 14;   // every attempt is one pass over V
         double thr_few = -1.0, thr_many = -1.0;          // last thresholds with too few groups / too many survivors
         for (int attempt = 0; !seg && attempt < max_attempts; attempt++) {
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
