@@ -764,10 +764,10 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
   const int wa = (int)(w.state & smask), wb = a.S == 1 ? wa : (int)((w.state >> a.ns) & smask);
   const int wcl = a.S == 3 ? (int)((w.state >> (2 * a.ns)) & hmask) : 0;
   const unsigned long long gw = merge_gid(a.lg, a.pid, w.parent, wa, wb, wcl);
-  // group start: lower bound of gw in the sorted list
+  // group start: lower bound of gw in the sorted list (the winner itself is the first entry of its group)
   unsigned lo = 0, hi = a.n_mc;
   while (lo < hi) { unsigned mid = (lo + hi) >> 1; if (a.mc[mid].g < gw) lo = mid + 1; else hi = mid; }
-  // ---- candidates
+  // ---- candidates, in generation order: inherited, then every loser followed by its compositions
   const int nin = a.cnt_old[w.parent];
   for (int k = tid; k < nin; k += 128) cand[k] = DCand{a.dE_old[(i64)w.parent * a.K + k], k, -1, k, 0u};
   if (tid == 0) { s_n = nin; s_stop = 0; }
@@ -782,7 +782,7 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
       l = a.mc[t];
       if (l.g == gw) {
         dE = (w.score - l.score) / a.beta;
-        valid = dE <= a.max_dE;
+        valid = dE <= a.max_dE;                     // sorted by score: the first loser beyond the cutoff ends the walk
       }
     }
     if (valid) {
@@ -818,7 +818,7 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
   while (np2 < n) np2 <<= 1;
   for (int k = n + tid; k < np2; k += 128) cand[k] = DCand{INFINITY, 0x7fffffff, -1, -1, 0u};
   __syncthreads();
-  for (int k = 2; k <= np2; k <<= 1)
+  for (int k = 2; k <= np2; k <<= 1)                 // bitonic sort by (dE, generation order)
     for (int j = k >> 1; j > 0; j >>= 1) {
       for (int e = tid; e < np2; e += 128) {
         const int o = e ^ j;
@@ -831,7 +831,8 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
       }
       __syncthreads();
     }
-  // ---- greedy selection
+  // ---- greedy selection.  Every value that thread 0 publishes through s_cnt is copied to a register by all threads
+  // and followed by a barrier before s_cnt is reused (the control flow below must stay uniform over the CTA).
   const int nw = (a.n_spins + 31) / 32;
   int kept = 0;
   unsigned* mine_pool = a.pool_new + (i64)i * a.K * a.ncell;
@@ -857,21 +858,23 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
     if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
     __syncthreads();
     const int nflip = s_cnt;
-    if (nflip == 0) { __syncthreads(); continue; }
+    __syncthreads();
+    if (nflip == 0) continue;
     // Hamming distance to the kept ones
     bool ok = true;
     for (int j = 0; j < kept && ok; j++) {
       int hd = 0;
       for (int k = tid; k < a.ncell; k += 128) hd += __popc(fm[k] ^ mine_pool[(i64)j * a.ncell + k]);
-      __syncthreads();
       s_red[tid] = hd;
       __syncthreads();
       if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
       __syncthreads();
-      if (s_cnt < a.min_hamming) ok = false;
+      const int hdist = s_cnt;
+      __syncthreads();
+      if (hdist < a.min_hamming) ok = false;
     }
     if (ok) {
-      // connectivity: list of flipped spins, label propagation from the first one
+      // connectivity: list of flipped spins, label propagation from the lowest one
       if (tid == 0) s_cnt = 0;
       __syncthreads();
       for (int k = tid; k < a.ncell; k += 128) {
@@ -912,7 +915,9 @@ __global__ void __launch_bounds__(128) k_droplets(DropArgs a) {
       __syncthreads();
       if (tid == 0) { int t = 0; for (int q = 0; q < 128; q++) t += s_red[q]; s_cnt = t; }
       __syncthreads();
-      if (s_cnt != nflip) ok = false;
+      const int nreach = s_cnt;
+      __syncthreads();
+      if (nreach != nflip) ok = false;
     }
     if (ok) {
       for (int k = tid; k < a.ncell; k += 128) mine_pool[(i64)kept * a.ncell + k] = fm[k];

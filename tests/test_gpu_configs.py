@@ -114,3 +114,34 @@ def test_config3_full_size_properties():
     resid = logp + beta * E + lz
     assert 0 < st["min_sigma_rel"] < 0.02
     assert np.abs(resid).max() <= 2 * (inst.Ly - 1) * st["min_sigma_rel"], (np.abs(resid).max(), st["min_sigma_rel"])
+
+
+@pytest.mark.slow
+def test_config5_droplets_at_full_size():
+    """configs[4] (loop-planted 12x12 Zephyr-shaped, M = 1024) with merge + droplets: the run that exposed a shared-memory
+    race in k_droplets at scale.  The merge leaves ONE main branch (the last cell has no boundary), it is a planted
+    ground state, and every book-kept droplet is a real excitation: flipping its spins raises the energy by exactly
+    dE (integer couplings; the beta = 4 contraction is exact to rounding), dE ascending, pairwise Hamming >= 2."""
+    import paper_2411_16431_b200 as tnb
+    inst, run = instances.config(4)
+    beta = run["beta"][0]
+    with _tn(inst) as t:
+        for k, v in ((tnb.OPT_MERGE, 1), (tnb.OPT_DROPLETS, 1), (tnb.OPT_DROPLET_MAX_COUNT, 16),
+                     (tnb.OPT_DROPLET_MAX_DE, 2.0), (tnb.OPT_DROPLET_MIN_HAMMING, 2)):
+            t.set_option(k, v)
+        t.set_beta(beta)
+        t.contract(run["D"], run["sweeps"])
+        states, E, logp, pd = t.branch_and_bound(run["M"])
+        st = t.stats()
+        dE, flips = t.droplets(0)
+        assert states.shape[0] == 1 and E[0] == inst.E0
+        assert len(dE) > 0 and np.all(np.diff(dE) >= -1e-9) and dE.max() <= 2.0 + 1e-9
+        ex = (states[0][None, :].astype(np.int32) * (1 - 2 * flips.astype(np.int32))).astype(np.int8)
+        Eex = t.energy(ex)
+    assert np.array_equal(Eex, energy.energies(inst, ex))
+    assert np.abs((Eex - E[0]) - dE).max() <= 1e-6
+    for i in range(len(dE)):
+        assert flips[i].sum() > 0
+        for j in range(i):
+            assert int((flips[i] != flips[j]).sum()) >= 2
+    assert st["merge_fallback_cells"] <= 8               # counted, never silent (cells whose survivors exceed 2^20)
