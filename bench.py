@@ -56,6 +56,14 @@ def parse_args():
                     help="N = 1 with --replicas transforms: run the 8 maps as concurrent replicas on this many "
                          "CUDA streams (one host thread per stream)")
     ap.add_argument("--merge", action="store_true", help="TN_OPT_MERGE: merge candidates by boundary (paper Fig. 3(d))")
+    ap.add_argument("--svd-mode", default="converged", choices=["converged", "randomized"],
+                    help="TN_OPT_SVD_MODE: converged truncated SVD (parity definition, default) or the paper's seeded "
+                         "randomized SVD with 2 subspace iterations (PAPER.md:169-177)")
+    ap.add_argument("--schedule", default="zipper-then-sweeps", choices=["zipper-then-sweeps", "interleaved"],
+                    help="TN_OPT_SCHEDULE: variant (ii) of PAPER.md:179 (default) or a sweep after every zipper step")
+    ap.add_argument("--two-step", action="store_true", help="TN_OPT_TWO_STEP: zipper and passes at 2 D, then cut to D")
+    ap.add_argument("--headline-fast", action="store_true",
+                    help="add a second one-step record of configs[3] in the fast mode (--svd-mode randomized)")
     ap.add_argument("--droplets", action="store_true",
                     help="TN_OPT_DROPLETS on top of --merge: book-keep the excitations above every main branch (Fig. 4)")
     ap.add_argument("--droplet-max-de", type=float, default=2.0, help="TN_OPT_DROPLET_MAX_DE (energy units of J)")
@@ -453,6 +461,7 @@ def run_ours(args):
 
     def make_tn(ins):
         t = tnb.TensorNetwork(ins)
+        set_contract_options(tnb, t, args)
         if args.merge or args.droplets:
             t.set_option(tnb.OPT_MERGE, 1)
         if args.droplets:
@@ -589,6 +598,9 @@ def run_ours(args):
     # ---- the north_star target workload: ONE timed step of configs[3] (N = 5400, D = 64, M = 1024, 3 passes, beta = 2)
     if world == 1 and not args.no_headline and args.config != 3:
         line["headline"] = headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local)
+        if args.headline_fast:
+            line["headline_fast"] = headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local,
+                                                    svd_mode="randomized")
     if world == 1 and not args.no_cpu_baseline:
         smp = OracleSample(base_inst if not transform else inst, run, beta, ORACLE_SAMPLE[args.config])
         tm = smp.step()
@@ -599,7 +611,17 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local):
+def set_contract_options(tnb, t, args, svd_mode=None):
+    mode = svd_mode or args.svd_mode
+    if mode == "randomized":
+        t.set_option(tnb.OPT_SVD_MODE, 1)
+    if args.schedule == "interleaved":
+        t.set_option(tnb.OPT_SCHEDULE, 1)
+    if args.two_step:
+        t.set_option(tnb.OPT_TWO_STEP, 1)
+
+
+def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local, svd_mode=None):
     """One timed step (after a tables-only warm-up of the handle) of BASELINE.json configs[3] at beta = 2: the
     ~5400-spin D = 64, M = 1024 instance of north_star, with its own stage table, roofline and clocks.  A single step:
     `steps` = 1, `warmup` = 0 -- a record inside the driver-observed run, not the line's `value`."""
@@ -608,6 +630,7 @@ def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_sr
     beta = run["beta"][bi]
     sampler = ClockSampler(local)
     t = tnb.TensorNetwork(inst)
+    set_contract_options(tnb, t, args, svd_mode)
     if args.merge:
         t.set_option(tnb.OPT_MERGE, 1)
     sampler.start()
@@ -618,7 +641,9 @@ def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_sr
     clocks = sampler.stop()
     states, E, logp, pd = outs
     stages, roofline = stage_report(st, ci, fp64_peak, peaks, peak_src)
-    return {"config": config_record(ci, inst, run, beta, args.merge, 0, 1), "steps": 1, "warmup": 0,
+    return {"config": dict(config_record(ci, inst, run, beta, args.merge, 0, 1), svd_mode=svd_mode or args.svd_mode,
+                           schedule=args.schedule, two_step=bool(args.two_step)), "steps": 1, "warmup": 0,
+            "svd_iterations": int(st["svd_iterations"]), "theta_apply_calls": int(st["theta_apply_calls"]),
             "value": ms * 1e-3, "unit": UNIT, "ms_per_step": ms, "contract_ms": round(st["ms_contract"], 3),
             "search_ms": round(st["ms_search"], 3), "best_energy": float(E.min()), "log_z": float(lz),
             "log_p_discarded": float(pd), "min_sigma_rel": st["min_sigma_rel"], "negative_u": int(st["negative_u"]),
