@@ -61,6 +61,7 @@ def parse_args():
                          "randomized SVD with 2 subspace iterations (PAPER.md:169-177)")
     ap.add_argument("--schedule", default="zipper-then-sweeps", choices=["zipper-then-sweeps", "interleaved"],
                     help="TN_OPT_SCHEDULE: variant (ii) of PAPER.md:179 (default) or a sweep after every zipper step")
+    ap.add_argument("--oversample", type=int, default=None, help="TN_OPT_OVERSAMPLE (extra block columns of the SVD)")
     ap.add_argument("--two-step", action="store_true", help="TN_OPT_TWO_STEP: zipper and passes at 2 D, then cut to D")
     ap.add_argument("--headline-fast", action="store_true",
                     help="add a second one-step record of configs[3] in the fast mode (--svd-mode randomized)")
@@ -619,6 +620,8 @@ def set_contract_options(tnb, t, args, svd_mode=None):
         t.set_option(tnb.OPT_SCHEDULE, 1)
     if args.two_step:
         t.set_option(tnb.OPT_TWO_STEP, 1)
+    if args.oversample is not None:
+        t.set_option(tnb.OPT_OVERSAMPLE, args.oversample)
 
 
 def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local, svd_mode=None):

@@ -38,13 +38,21 @@ struct LdPA {   // A(m; i=(b,cl), k) = LG[m][(Pd b * n_o + Po cl)][k]
     return LG[((i64)m * npp + Pd[b] * n_o + Po[cl]) * Dr + k];
   }
 };
-struct LdPB {   // B(m; k, a) = RM[slot m][k][Pr a] * cs[m][a]: the column weights h wA ride on the small operand, so the
-                // epilogue of the conditional GEMM has only row-wise factors left (it was issue-bound on per-element loads)
-  const double* RM; const int *slot, *Pr; int Dr, n_r; const double* cs; int nA;
+struct LdPB {   // B(m; k, a) = RMc[m][k][a] = RM[slot m][k][Pr a] * hS[hrow m][a] * wA[a], materialised densely by k_rmc once per
+                // cell: the column weights ride on the small operand (the epilogue of the conditional GEMM has only
+                // row-wise factors left) and the B tile is read with coalesced loads instead of three dependent gathers
+  const double* RMc; int Dr, nA;
   __device__ __forceinline__ double operator()(int m, int k, int a) const {
-    return RM[((i64)slot[m] * Dr + k) * n_r + Pr[a]] * cs[(i64)m * nA + a];
+    return __ldg(RMc + ((i64)m * Dr + k) * nA + a);
   }
 };
+__global__ void k_rmc(const double* RM, const int* slot, const int* Pr, const double* hS, const double* wA, const int* hrow,
+                      int nb, int Dr, int n_r, int nA, double* RMc) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)nb * Dr * nA) return;
+  const int a = (int)(t % nA), k = (int)((t / nA) % Dr), m = (int)(t / ((i64)nA * Dr));
+  RMc[t] = RM[((i64)slot[m] * Dr + k) * n_r + Pr[a]] * (hS[(i64)hrow[m] * nA + a] * wA[a]);
+}
 struct StPV {
   double* V; const double *hS, *wA, *X, *vS, *Yc; const int *hrow, *vrow, *slot;
   int nA, nB, nCl, tshift; i64 per_m;
@@ -97,13 +105,6 @@ struct EpPV {   // stores V and, fused, collects Z_m = sum max(v, 0) fc[m][cl] a
     if (n) atomicAdd(nneg, (unsigned long long)n);
   }
 };
-// cs[m][a] = hS[hrow[m]][a] * wA[a]
-__global__ void k_colscale(const double* hS, const double* wA, const int* hrow, int nb, int nA, double* cs) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nb * nA) return;
-  int m = t / nA, a = t % nA;
-  cs[t] = hS[(i64)hrow[m] * nA + a] * wA[a];
-}
 struct LdHA {   // A(i=(b',b''), kk=(b,cl)) = G[(Pd b * n_o + Po cl)][i]
   const double* G; const int *Pd, *Po; int nCl, n_o; i64 DD;
   __device__ __forceinline__ double operator()(int, int i, int kk) const {
@@ -1235,11 +1236,11 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
         h->st.flop_search_cond += 2.0 * nb * (double)Mg * Ng * Dr;
         h->st.bytes_search_cond += 8.0 * nb * (double)per_m;
-        DBuf<double> cs(h, (size_t)nb * c.nA);
-        k_colscale<<<cdiv((i64)nb * c.nA, 256), 256, 0, h->stream>>>(c.BhS, c.wA, hrow.p, nb, c.nA, cs.p);
+        DBuf<double> RMc(h, (size_t)nb * Dr * c.nA);
+        k_rmc<<<cdiv((i64)nb * Dr * c.nA, 256), 256, 0, h->stream>>>(rt[x].RM, sl_cur, c.Pr, c.BhS, c.wA, hrow.p, nb, Dr, c.n_r, c.nA, RMc.p);
         TN_LAUNCH_CHECK(h);
         ArPV ar{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
-        LdPB be{rt[x].RM, sl_cur, c.Pr, Dr, c.n_r, cs.p, c.nA};
+        LdPB be{RMc.p, Dr, c.nA};
         const int ntile = (Mg + 127) / 128;
         DBuf<double> zpart(h, (size_t)nb * std::max(ntile, 64));
         EpPV ep{V.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
