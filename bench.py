@@ -8,7 +8,9 @@ the largest config whose `--steps 20 --warmup 5` run fits the driver's per-arm t
 kernel is in its streaming regime, the Theta-core is 8.6 GB >> L2).  The north_star target workload, configs[3]
 (Pegasus-shaped 15x15x24, N = 5400, D = 64, M = 1024, three variational passes, beta = 2), takes about two minutes per
 step, so the same JSON line carries a `headline` record of ONE timed step of it (own stage table, roofline and clocks;
-`--no-headline` skips it, N = 1 only).
+`--no-headline` skips it, N = 1 only), and a second one, `headline_fast`, of the same workload with the paper's own
+truncated randomized SVD (seeded, reproducible, parity-tested against the oracle's switch on small
+lattices; `--no-headline-fast` skips it).  The line's `value` is always the converged (parity-defining) mode.
 A step = tn_set_beta + tn_contract(D, sweeps) + tn_branch_and_bound(M) on an instance that is already resident in HBM
 (tn_create done before the timed region).  The `e2e` arm repeats the measurement with tn_create (host -> device copy
 of the instance) and tn_destroy inside the timed region; results always come back to caller-allocated host buffers.
@@ -63,8 +65,9 @@ def parse_args():
                     help="TN_OPT_SCHEDULE: variant (ii) of PAPER.md:179 (default) or a sweep after every zipper step")
     ap.add_argument("--oversample", type=int, default=None, help="TN_OPT_OVERSAMPLE (extra block columns of the SVD)")
     ap.add_argument("--two-step", action="store_true", help="TN_OPT_TWO_STEP: zipper and passes at 2 D, then cut to D")
-    ap.add_argument("--headline-fast", action="store_true",
-                    help="add a second one-step record of configs[3] in the fast mode (--svd-mode randomized)")
+    ap.add_argument("--no-headline-fast", action="store_true",
+                    help="skip the second one-step record of configs[3], taken in the paper's own mode (seeded randomized "
+                         "SVD, --svd-mode randomized)")
     ap.add_argument("--droplets", action="store_true",
                     help="TN_OPT_DROPLETS on top of --merge: book-keep the excitations above every main branch (Fig. 4)")
     ap.add_argument("--droplet-max-de", type=float, default=2.0, help="TN_OPT_DROPLET_MAX_DE (energy units of J)")
@@ -599,7 +602,7 @@ def run_ours(args):
     # ---- the north_star target workload: ONE timed step of configs[3] (N = 5400, D = 64, M = 1024, 3 passes, beta = 2)
     if world == 1 and not args.no_headline and args.config != 3:
         line["headline"] = headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local)
-        if args.headline_fast:
+        if not args.no_headline_fast and args.svd_mode == "converged":
             line["headline_fast"] = headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local,
                                                     svd_mode="randomized")
     if world == 1 and not args.no_cpu_baseline:
