@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (0-based)")
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (0-based); 5 = the 50 x 50 square lattice of the paper's App. B")
     ap.add_argument("--beta-index", type=int, default=0, help="which beta of the config's sweep")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -110,8 +110,8 @@ def sub_lattice(inst, rows, cols):
 
 # (rows, cols, beam) of the oracle sample per config: None = the whole instance.  Pegasus-shaped cells have 2^24
 # states: every oracle operation on one cell costs seconds, so the sample there is a 2 x 2 block with one beam element.
-ORACLE_SAMPLE = {0: None, 1: None, 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64)}
-ORACLE_SAMPLE_SMALL = {0: None, 1: (2, 6, 256), 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64)}   # reference arm, many steps
+ORACLE_SAMPLE = {0: None, 1: None, 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64), 5: None}
+ORACLE_SAMPLE_SMALL = {0: None, 1: (2, 6, 256), 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64), 5: (10, 50, 256)}   # reference arm, many steps
 
 
 class OracleSample:

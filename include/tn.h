@@ -31,7 +31,8 @@
  *
  * Geometry accepted by tn_create (BASELINE.json "Pegasus-/Zephyr-shaped" synthetic lattices):
  *   a cell is a chain of S = subs_per_cell (1..3) sub-clusters of n_s = spins_per_sub spins
- *   (n_s even, 2..8); lo = positions [0, n_s/2), hi = [n_s/2, n_s).  Allowed edges:
+ *   (2..8, even; with S == 1 any n_s in 1..8 -- n_s = 1 is the square lattice of App. B, one spin
+ *   per site); lo = positions [0, n_s/2), hi = [n_s/2, n_s).  Allowed edges:
  *     inside a sub-cluster: any pair;   sub s hi -- sub s+1 lo  (same cell);
  *     horizontal (x,y)-(x+1,y): sub 0 -- sub 0;  vertical (x,y)-(x,y+1): sub v -- sub v with
  *     v = min(1, S-1);  diagonal (x,y)-(x+1,y+1) (S == 3 only): sub 2 lo -- sub 2 hi.

@@ -102,7 +102,7 @@ def lattice(Ly, Lx, S, n_s, p_keep=1.0, seed=0, h="uniform", h_scale=1.0, name="
     """Random-coupling instance (classes I/II of PAPER.md:225-226 on the synthetic shape).
 
     h: "uniform" -> h_i ~ U[-h_scale, h_scale]; "zero" -> h = 0 (class I)."""
-    assert n_s % 2 == 0 and 1 <= S <= 3
+    assert 1 <= S <= 3 and (n_s % 2 == 0 or S == 1)      # S = 1 has no lo / hi halves: any n_s (square lattice: n_s = 1)
     rng = SplitMix64(seed)
     eu, ev, J = [], [], []
     for (u, v) in candidate_edges(Ly, Lx, S, n_s):
@@ -227,6 +227,10 @@ CONFIGS = [
          beta=[1.0, 2.0, 4.0], D=64, M=1024, sweeps=3),
     dict(name="cfg5_zephyr_12x12x16_planted", kind="loops", Ly=12, Lx=12, S=2, n_s=8,
          beta=[4.0], D=32, M=1024, sweeps=1),
+    # not a BASELINE.json config: the square-lattice workload of App. B (nearest neighbours, one spin per
+    # site, class I couplings, chi = 16, M = 256, beta = 4, 50 x 50 sites) -- SURVEY.md section 8(f) f4, first half
+    dict(name="appB_square_50x50", kind="lattice", Ly=50, Lx=50, S=1, n_s=1, p_keep=1.0, h="zero",
+         beta=[4.0], D=16, M=256, sweeps=1),
 ]
 
 

@@ -141,8 +141,9 @@ int tn_create(tn_handle** out, int32_t n_spins, int64_t n_edges, const int32_t* 
     if (n_spins <= 0 || n_edges < 0 || Ly <= 0 || Lx <= 0) tn_throw(TN_ERR_ARG, "non-positive size");
     if ((n_edges > 0 && (!edge_u || !edge_v || !J)) || !cell_y || !cell_x || !sub || !pos)
       tn_throw(TN_ERR_ARG, "NULL input array");
-    if (S < 1 || S > 3 || ns < 2 || ns > 8 || (ns & 1))
-      tn_throw(TN_ERR_GEOMETRY, "subs_per_cell must be 1..3 and spins_per_sub even in 2..8 (got %d, %d)", S, ns);
+    if (S < 1 || S > 3 || ns < 1 || ns > 8 || (S > 1 && (ns & 1)))
+      tn_throw(TN_ERR_GEOMETRY, "subs_per_cell must be 1..3 and spins_per_sub in 1..8, even unless subs_per_cell == 1 "
+               "(got %d, %d)", S, ns);
     if ((i64)n_spins != (i64)Ly * Lx * S * ns)
       tn_throw(TN_ERR_GEOMETRY, "n_spins = %d but the cluster map has Ly*Lx*S*n_s = %lld slots", n_spins,
                (long long)Ly * Lx * S * ns);

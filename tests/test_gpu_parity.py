@@ -116,6 +116,8 @@ EXACT = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, M)
     (2, 3, 1, 4, 1.0, 1, 1.5, 16),
     (2, 3, 2, 2, 0.9, 7, 0.9, 8),
     (3, 3, 3, 2, 0.85, 7, 0.9, 32),
+    (4, 5, 1, 1, 1.0, 2, 1.0, 16),             # square lattice, one spin per site (App. B; f4 workload)
+    (3, 4, 1, 3, 0.9, 5, 0.8, 16),             # S = 1 with an odd number of spins per cell
 ]
 
 
@@ -138,6 +140,7 @@ TRUNC = [  # (Ly, Lx, S, n_s, p_keep, seed, beta, D, sweeps, M)
     (3, 3, 3, 4, 0.9, 4, 1.0, 6, 2, 64),       # Pegasus-shaped miniature: 4096 states per cell, mediating tensors
     (4, 3, 3, 2, 0.85, 9, 1.5, 4, 3, 32),
     (3, 3, 1, 4, 1.0, 6, 2.0, 5, 1, 16),
+    (10, 10, 1, 1, 1.0, 3, 1.0, 4, 1, 64),     # square lattice 10 x 10, chi = 4: truncating, 100 cells of one spin
 ]
 
 
@@ -540,3 +543,12 @@ def test_error_codes():
     with pytest.raises(tnb.TnError) as e:
         tnb.TensorNetwork(bad)
     assert e.value.code == -2              # TN_ERR_GEOMETRY
+
+
+@pytest.mark.slow
+def test_square_lattice_workload_of_appendix_b():
+    """App. B: nearest-neighbour square lattice, one spin per site, J ~ U[-1,1] (class I), chi = 16, M = 256,
+    beta = 4 -- here 16 x 16 sites (the oracle needs a minute for it), element by element against the oracle.  The
+    king's lattice of the same appendix (both diagonals) is outside the accepted geometry."""
+    inst = instances.lattice(16, 16, 1, 1, p_keep=1.0, seed=1, h="zero")
+    compare(inst, 4.0, 16, 1, 256, 1e-6)

@@ -719,3 +719,20 @@ def test_droplets_are_the_connected_low_energy_excitations(S, ns, seed, beta):
     few = search.branch_and_bound(m, R, ln, 4096, merge=True,
                                   droplets=dict(max_dE=max_dE, min_hamming=1, max_count=3))["droplets"][0]
     assert [d for d, _ in few] == sorted(d for d, _ in drops)[:3]
+
+
+# ---------------------------------------------------------------- f4 (partial): square lattice, one spin per site
+def test_square_lattice_against_brute_force():
+    """App. B PAPER.md:446-454 workload shape: S = 1, n_s = 1 (cells of a single spin, bond dimension 2 everywhere).
+    P1 / P2 / P3 / P7 on a 4 x 5 lattice: log Z of the exact contraction = brute force, the no-prune beam returns the
+    brute-force order, logp = -beta E - log Z."""
+    inst = instances.lattice(4, 5, 1, 1, p_keep=1.0, seed=2)
+    E_all = brute.all_energies(inst)
+    m = model.Model(inst).set_beta(1.3)
+    R, ln = mps.contract(m, 0, 0)
+    out = search.branch_and_bound(m, R, ln, 1 << 12)
+    lz = brute.log_z(E_all, 1.3)
+    assert abs(out["log_z"] - lz) <= 1e-12 * abs(lz)
+    low = np.sort(E_all)[:64]
+    assert np.allclose(out["energies"][:64], low, rtol=0, atol=1e-12)
+    assert np.allclose(out["logp"], -1.3 * out["energies"] - lz, rtol=0, atol=1e-9)
