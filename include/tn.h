@@ -100,6 +100,8 @@ enum {
   TN_OPT_DROPLET_MAX_COUNT = 19,    /* droplets kept per branch (default 8, range 1..32)                        */
   TN_OPT_MERGE_SEGMENTED = 20,      /* 1 (default) / 0: allow the segmented arg-max route of the merge (taken when the possible
                                        boundaries of a cell fit TN_OPT_MERGE_CAP); 0 forces threshold + sort everywhere   */
+  TN_OPT_SVD_DIRECT = 21,           /* 1 (default) / 0: where Theta is tiny (n <= 128, n m + n^2 <= 24000 entries) form it explicitly
+                                       and take its SVD by one-sided Jacobi in one kernel instead of iterating            */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */
@@ -139,6 +141,7 @@ typedef struct {
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
   int64_t merge_fallback_cells; /* cells at which TN_OPT_MERGE could not merge (merge buffers too small at every threshold
                                 tried) and the selection ran unmerged; 0 = every cell followed Fig. 3(d)          */
+  int64_t svd_direct;        /* truncated SVDs taken by the direct route (TN_OPT_SVD_DIRECT)                              */
   int64_t droplet_overflow;  /* boundary groups whose droplet candidates exceeded the kernel's buffer (1024): 0 = none     */
   double flop_orth_svd;      /* algorithmic FLOP of the orthonormalisations: 2 Cholesky-QR rounds of 4 m k^2 each per call
                                 (Gram + apply; the rounds actually run are decided on the device, 1..5)             */

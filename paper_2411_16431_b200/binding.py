@@ -17,6 +17,7 @@ OPT_MERGE_CAP = 10
 OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
 OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT = 16, 17, 18, 19
 OPT_MERGE_SEGMENTED = 20
+OPT_SVD_DIRECT = 21
 
 
 class TnError(RuntimeError):
@@ -32,7 +33,7 @@ class TnStats(C.Structure):
         "bytes_theta_apply", "flop_search", "bytes_search_cond", "bytes_search_select", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
             "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged",
-            "merge_fallback_cells", "droplet_overflow")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
+            "merge_fallback_cells", "svd_direct", "droplet_overflow")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -592,6 +592,37 @@ void svd_rand(Ctx& cx, const ThetaOp& op, int chi, int ks, int pu, int g, double
   TN_CUDA(cudaMemcpyAsync(sig0_out, sig.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
 }
 
+// Tiny Theta (both dimensions of the order of 100: every position of the one-spin-per-site square lattice, the first
+// and last positions of any row, config 1): the matrix is formed explicitly by one apply to the identity and decomposed
+// by the one-sided Jacobi kernel -- an exact SVD in ~6 launches, no iteration and no host round trip, where the subspace
+// iteration needs ~40 launches and a device -> host flag per step.  Same outputs as svd_trunc.
+__global__ void k_eye(double* X, int n) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < n * n) X[t] = (t / n == t % n) ? 1.0 : 0.0;
+}
+bool svd_direct_fits(i64 m, i64 n) { return n <= 128 && m <= 4096 && n * m + n * n <= 24000; }
+void svd_direct(Ctx& cx, const ThetaOp& op, int chi, double* Vz, double* C, double* sig0_out) {
+  tn_handle* h = cx.h;
+  const int m = (int)op.m, n = (int)op.n;
+  DBuf<double> X(h, (size_t)n * n), Th(h, (size_t)m * n), ThT(h, (size_t)n * m), Mo(h, (size_t)n * m), Wt(h, (size_t)n * n), sig(h, n);
+  cx.seed++;                                                     // one seed per truncated SVD, whichever route takes it
+  k_eye<<<cdiv((i64)n * n, 256), 256, 0, h->stream>>>(X.p, n);
+  TN_LAUNCH_CHECK(h);
+  apply_N(cx, op, X.p, Th.p, n);                                 // Theta [m x n]
+  cx.tic(&h->st.ms_orth_svd);
+  permute3(h, ThT.p, Th.p, 1, n, m, 0, 1, n);                    // Theta^T [n x m]
+  jacobi_rows(h, ThT.p, m, n, m, Mo.p, Wt.p, sig.p);             // rows of V^T Theta^T orthogonal: Wt = V^T, Mo = (Theta V)^T
+  k_rank_decide<<<1, 32, 0, h->stream>>>(sig.p, std::min(m, n), chi, h->gap_guard, cx.d_keep, cx.d_stat);
+  TN_LAUNCH_CHECK(h);
+  k_commit_stat<<<1, 32, 0, h->stream>>>(cx.d_stat);
+  TN_LAUNCH_CHECK(h);
+  cx.toc();
+  permute3(h, Vz, Wt.p, 1, n, chi, 0, 1, n, 2, cx.d_keep);
+  permute3(h, C, Mo.p, 1, m, chi, 0, 1, m, 2, cx.d_keep);
+  TN_CUDA(cudaMemcpyAsync(sig0_out, sig.p, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  h->st.svd_direct++;
+}
+
 MpsTensor new_tensor(tn_handle* h, int dl, int p, int dr) {
   MpsTensor t;
   t.dl = dl; t.p = p; t.dr = dr;
@@ -757,6 +788,7 @@ std::vector<MpsTensor> compress(Ctx& cx, int y, const std::vector<MpsTensor>& Ao
     DBuf<double> Vz(h, (size_t)op.n * chi[j]);
     double* C = h->dalloc<double>((size_t)op.m * chi[j]);
     if (!exact && h->svd_mode == 1 && mn > cap) svd_rand(cx, op, chi[j], ks, pos[j].pu, g, Vz.p, C, d_sig0);
+    else if (h->svd_direct && svd_direct_fits(op.m, op.n)) svd_direct(cx, op, chi[j], Vz.p, C, d_sig0);
     else svd_trunc(cx, op, chi[j], ks, Vz.p, C, d_sig0);
     N[j] = new_tensor(h, chi[j], pos[j].pu, g);
     permute3(h, N[j].d, Vz.p, chi[j], pos[j].pu, g, 1, (i64)g * chi[j], chi[j]);

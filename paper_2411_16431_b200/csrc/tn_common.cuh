@@ -94,6 +94,7 @@ struct tn_handle {
   i64 merge_cap = 1ll << 20;  // TN_OPT_MERGE_CAP: survivors / boundary groups the merge buffers hold
   int gap_guard = 1, svd_maxit = 40, oversample = 16, exact_cap = 512, svd_cheb = 1, svd_lock = 1;
   int schedule = 0, sweep_range = 2, svd_mode = 0, rsvd_iters = 2, two_step = 0;   // f2 (TN_OPT_SCHEDULE ...)
+  int svd_direct = 1;       // TN_OPT_SVD_DIRECT: explicit Theta + Jacobi SVD where Theta is tiny
   int svd_skip_first = 0;   // predictor (contract.cu): skip the first Rayleigh-Ritz step of the next truncated SVD
   double svd_tol = 1e-11;
   i64 select_direct_max = 1ll << 22;
