@@ -111,7 +111,7 @@ def sub_lattice(inst, rows, cols):
 # (rows, cols, beam) of the oracle sample per config: None = the whole instance.  Pegasus-shaped cells have 2^24
 # states: every oracle operation on one cell costs seconds, so the sample there is a 2 x 2 block with one beam element.
 ORACLE_SAMPLE = {0: None, 1: None, 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64), 5: None}
-ORACLE_SAMPLE_SMALL = {0: None, 1: (2, 6, 256), 2: (2, 2, 1), 3: (2, 2, 1), 4: (2, 4, 64), 5: (10, 50, 256)}   # reference arm, many steps
+ORACLE_SAMPLE_SMALL = {0: None, 1: (2, 6, 256), 2: (2, 1, 1), 3: (2, 1, 1), 4: (2, 4, 64), 5: (10, 50, 256)}   # reference arm, many steps
 
 
 class OracleSample:
@@ -529,7 +529,7 @@ def run_ours(args):
                 ex.append((states0[r][None, :].astype(np.int32) * (1 - 2 * flips.astype(np.int32))).astype(np.int8))
         drop_states = np.concatenate(ex, axis=0)
         drop_E = t.energy(drop_states)                           # O-0 energies on the device (tn_energy)
-    alone = kernel_alone(t, inst, run) if rank == 0 else None
+    alone = kernel_alone(t, inst, run) if (rank == 0 and run["D"] > 0) else None
     t.close()
 
     # ---- e2e: host buffers in, host buffers out, tn_create / tn_destroy inside the timed region
