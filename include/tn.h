@@ -141,6 +141,8 @@ typedef struct {
                                 parity with a converged SVD (reading S1) is not guaranteed at those bonds  */
   int64_t merge_fallback_cells; /* cells at which TN_OPT_MERGE could not merge (merge buffers too small at every threshold
                                 tried) and the selection ran unmerged; 0 = every cell followed Fig. 3(d)          */
+  int64_t select_tie_overflow; /* cells whose tie group at the beam cut exceeded the candidate list and was collected completely */
+  int64_t select_tie_dropped;  /* cells whose tie group exceeded even 2^24 candidates: an arbitrary subset of it was kept     */
   int64_t svd_direct;        /* truncated SVDs taken by the direct route (TN_OPT_SVD_DIRECT)                              */
   int64_t droplet_overflow;  /* boundary groups whose droplet candidates exceeded the kernel's buffer (1024): 0 = none     */
   double flop_orth_svd;      /* algorithmic FLOP of the orthonormalisations: 2 Cholesky-QR rounds of 4 m k^2 each per call

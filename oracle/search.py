@@ -297,6 +297,13 @@ def branch_and_bound(model, R, lognorm, M, stats=None, merge=False, trace=None, 
                 if stats is not None:
                     stats["merged_away"] = stats.get("merged_away", 0) + int(pk.size * sc.size - surv.size)
             keep, disc = select_top(score, parent, state, M)
+            if stats is not None and keep.size == M and np.isfinite(disc):
+                # bookkeeping for the parity tests: a cut that falls INSIDE a group of (numerically) tied candidates --
+                # which members survive is then decided by rounding noise, and everything downstream that depends on
+                # the identity of the survivors (later discarded probabilities, states of tied ranks) is not unique
+                last = score[keep[-1]]
+                if last - disc <= 1e-9 * max(1.0, abs(last)):
+                    stats["tied_cuts"] = stats.get("tied_cuts", 0) + 1
             keep = keep[np.isfinite(score[keep])]                          # never keep p = 0
             new_drops = []
             if book is not None:

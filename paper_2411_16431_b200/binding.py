@@ -33,7 +33,7 @@ class TnStats(C.Structure):
         "bytes_theta_apply", "flop_search", "bytes_search_cond", "bytes_search_select", "min_sigma_rel")] + [(n, C.c_int64) for n in (
             "svd_iterations", "kernel_launches", "negative_u", "rows_contracted", "bytes_device", "jacobi_calls",
             "jacobi_sweeps", "theta_apply_calls", "cheb_steps", "svd_locked_cols", "merged_away", "svd_unconverged",
-            "merge_fallback_cells", "svd_direct", "droplet_overflow")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
+            "merge_fallback_cells", "select_tie_overflow", "select_tie_dropped", "svd_direct", "droplet_overflow")] + [(n, C.c_double) for n in ("flop_orth_svd", "flop_search_rblocks", "flop_search_cond")]
 
     def asdict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -13,6 +13,7 @@
 #include <algorithm>
 #include <cfloat>
 #include <map>
+#include <memory>
 
 namespace {
 
@@ -488,16 +489,6 @@ __device__ __forceinline__ bool cand_before(const Cand& x, const Cand& y) {   //
   if (x.score != y.score) return x.score > y.score;
   if (x.parent != y.parent) return x.parent < y.parent;
   return x.state < y.state;
-}
-__global__ void k_bitonic_step(Cand* c, unsigned n, unsigned k, unsigned j) {
-  unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  unsigned l = i ^ j;
-  if (l > i) {
-    Cand x = c[i], y = c[l];
-    bool up = (i & k) == 0;
-    if (up ? cand_before(y, x) : cand_before(x, y)) { c[i] = y; c[l] = x; }
-  }
 }
 __global__ void __launch_bounds__(1024) k_bitonic_smem(Cand* c, unsigned n) {
   extern __shared__ Cand sc[];
@@ -1291,6 +1282,12 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       const i64 total = (i64)nb * per_m;
       const int gsel = (int)std::min<i64>((i64)h->sms * 8, (total + 255) / 256);
       unsigned ncand = 0;
+      // Ties at the cut beyond the candidate list (degenerate instances: integer couplings, J = 0): up to tie_cap candidates
+      // are collected completely and sorted, so that the S8 order decides and the result is reproducible run to run;
+      // beyond that an arbitrary subset of the tie group is taken and the cell is counted in select_tie_dropped.
+      const unsigned tie_cap = 1u << 24;
+      std::unique_ptr<DBuf<Raw>> rawL;
+      std::unique_ptr<DBuf<Cand>> candL;
       bool direct = total * c.nCh <= (i64)h->select_direct_max;       // few candidates: radix passes straight on V
       bool cand_sorted = false;                                       // set by the merge route (cand.p final and sorted)
       unsigned np2 = 2;
@@ -1496,7 +1493,19 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
           k_csel_compact<<<gc, 256, 0, h->stream>>>(ckeys.p, craw.p, n1, sel.p, raw.p, count.p, cap);
           TN_LAUNCH_CHECK(h);
-          ncand = std::min(d2h(h, count.p), cap);
+          ncand = d2h(h, count.p);
+          if (ncand > cap) {   // more ties at the cut than the list holds: collect ALL of them (deterministic, S8 order)
+            if (ncand <= tie_cap) {
+              rawL.reset(new DBuf<Raw>(h, ncand));
+              TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+              k_csel_compact<<<gc, 256, 0, h->stream>>>(ckeys.p, craw.p, n1, sel.p, rawL->p, count.p, ncand);
+              TN_LAUNCH_CHECK(h);
+              h->st.select_tie_overflow++;
+            } else {
+              h->st.select_tie_dropped++;
+              ncand = cap;
+            }
+          }
         }
       }
       if (direct && !cand_sorted) {
@@ -1513,25 +1522,38 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
         k_sel_collect<<<gsel, 256, 0, h->stream>>>(sa, sel.p, raw.p, count.p, cap);
         TN_LAUNCH_CHECK(h);
-        ncand = std::min(d2h(h, count.p), cap);
+        ncand = d2h(h, count.p);
+        if (ncand > cap) {     // more ties at the cut than the list holds: collect ALL of them (deterministic, S8 order)
+          if (ncand <= tie_cap) {
+            rawL.reset(new DBuf<Raw>(h, ncand));
+            TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
+            k_sel_collect<<<gsel, 256, 0, h->stream>>>(sa, sel.p, rawL->p, count.p, ncand);
+            TN_LAUNCH_CHECK(h);
+            h->st.select_tie_overflow++;
+          } else {
+            h->st.select_tie_dropped++;
+            ncand = cap;
+          }
+        }
       }
       if (ncand == 0) tn_throw(TN_ERR_NUMERIC, "cell (%d,%d): every candidate has zero probability", y, x);
       Cand* cand_final = cand_sorted ? mcands.p : cand.p;
       if (!cand_sorted) {
       while (np2 < ncand + 1) np2 <<= 1;   // at least one sentinel so that cand[M] exists when ncand <= M
       while (np2 <= (unsigned)M) np2 <<= 1;
-      if (np2 > npad) np2 = npad;
-      k_sel_score<<<cdiv(np2, 256), 256, 0, h->stream>>>(sa, raw.p, ncand, np2, lp_cur, Z.p, ns, S, cand.p);
+      if (rawL) {                          // tie overflow: the complete tie group, in buffers of its own
+        candL.reset(new DBuf<Cand>(h, np2));
+        cand_final = candL->p;
+      } else if (np2 > npad) {
+        np2 = npad;
+      }
+      k_sel_score<<<cdiv(np2, 256), 256, 0, h->stream>>>(sa, rawL ? rawL->p : raw.p, ncand, np2, lp_cur, Z.p, ns, S, cand_final);
       TN_LAUNCH_CHECK(h);
       if (np2 <= 4096) {
-        k_bitonic_smem<<<1, 1024, np2 * sizeof(Cand), h->stream>>>(cand.p, np2);
+        k_bitonic_smem<<<1, 1024, np2 * sizeof(Cand), h->stream>>>(cand_final, np2);
         TN_LAUNCH_CHECK(h);
       } else {
-        for (unsigned k = 2; k <= np2; k <<= 1)
-          for (unsigned j = k >> 1; j > 0; j >>= 1) {
-            k_bitonic_step<<<cdiv(np2, 256), 256, 0, h->stream>>>(cand.p, np2, k, j);
-            TN_LAUNCH_CHECK(h);
-          }
+        bitonic_sort<Cand, LessC>(h, cand_final, np2);   // tiled: a handful of launches instead of log^2 n
       }
       }
       const int nkeep = (int)std::min<unsigned>(ncand, (unsigned)M);

@@ -130,7 +130,8 @@ def run_case(name):
         out = search.branch_and_bound(m, R, ln, run["M"], stats=st)
         data.update(log_z=np.float64(out["log_z"]), logp=out["logp"], log_pd=np.float64(out["log_pd"]),
                     cell_states=out["cell_states"].astype(np.int32), energies=out["energies"],
-                    states=out["states"].astype(np.int8), negative_u=np.int64(st.get("negative_u", 0)))
+                    states=out["states"].astype(np.int8), negative_u=np.int64(st.get("negative_u", 0)),
+                    tied_cuts=np.int64(st.get("tied_cuts", 0)))
     t3 = time.perf_counter()
     rng = np.random.default_rng(20241116)
     for y in range(1, inst.Ly):

@@ -77,7 +77,8 @@ def test_parity_with_stored_oracle_rows(path):
             states, E, logp, pd = t.branch_and_bound(run["M"])
         st = t.stats()
     if run["M"] > 0:
-        ref = dict(logp=data["logp"], states=data["states"], log_pd=float(data["log_pd"]))
+        ref = dict(logp=data["logp"], states=data["states"], log_pd=float(data["log_pd"]),
+                   tied_cuts=int(data["tied_cuts"]) if "tied_cuts" in data else 0)
         check_lists(inst, ref, states, E, logp, pd, tol)
     assert st["svd_unconverged"] == 0
     print("%s: worst Schmidt-value deviation %.2e sigma_1, worst sampled-amplitude deviation %.2e max|amp|, "
