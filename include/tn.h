@@ -229,6 +229,16 @@ int tn_kernel_check(tn_handle*, int32_t op, int64_t m, int32_t n, int32_t k, con
  *   TN_CHECK_ORTH: orthonormalisation of a random [m x n] block (k unused). */
 int tn_kernel_bench(tn_handle*, int32_t op, int64_t m, int32_t n, int64_t k, int32_t iters, double* ms_per_call);
 
+/* tn_gemm_t_static: ALLOCATION-FREE variant of the Theta-core^T x skinny apply (a2, Fig. 7), for callers
+ * that cannot call cudaMalloc (CUDA graph capture, tight serving loops):  C [k x n] = A [m x k]^T . B [m x n],  all three
+ * DEVICE pointers, row-major with leading dimensions lda >= k, ldb >= n, ldc >= n (lda, ldb even; A, B 16-byte aligned),
+ * n <= 96.  Needs no handle.  The split-over-m workspace lives in a file-scope device array of 2^20 doubles (8 MiB, held by
+ * every GPU that loads the library): sizes with 2 k n > 2^20 return TN_ERR_ARG.  The call queues two kernels on
+ * `cuda_stream` (NULL = default stream) and returns without synchronising; it calls no cudaMalloc / cudaFree.  Every call
+ * shares the scratch array: calls that overlap on the GPU (other streams, parallel graph branches) race on it. */
+int tn_gemm_t_static(void* cuda_stream, int64_t m, int32_t n, int64_t k, const double* dA, int64_t lda, const double* dB,
+                     int64_t ldb, double* dC, int64_t ldc);
+
 /* tn_fp64_peak: measured FP64 tensor-core (mma.sync m8n8k4 f64 = SASS DMMA) peak of the current device
  * in TFLOP/s, from a register-resident chain (about 10 ms); the roofline denominator of the GEMM stages
  * ("FP64 tensor peak to be measured first").  Needs no handle. */

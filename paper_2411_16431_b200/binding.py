@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_droplets", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_droplets", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_gemm_t_static", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 OPT_MERGE_CAP = 10
 OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
@@ -69,6 +69,8 @@ def lib():
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
         L.tn_droplets.argtypes = [C.c_void_p, C.c_int32, p_i32, p_f64, p_i8]
         L.tn_fp64_peak.argtypes = [p_f64]
+        L.tn_gemm_t_static.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p,
+                                       C.c_int64, C.c_void_p, C.c_int64]
         L.tn_kernel_bench.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int64, C.c_int32, p_f64]
         L.tn_kernel_check.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, p_f64, p_f64, p_f64]
         L.tn_last_error.restype = C.c_char_p
@@ -210,6 +212,12 @@ def tn_kernel_bench(handle, op, m, n, k, iters=10) -> float:
     v = C.c_double(0.0)
     _check(lib().tn_kernel_bench(handle, int(op), int(m), int(n), int(k), int(iters), C.byref(v)))
     return v.value
+
+
+def tn_gemm_t_static(cuda_stream, m, n, k, dA, lda, dB, ldb, dC, ldc):
+    """C [k x n] = A [m x k]^T . B [m x n] on DEVICE pointers (ints), allocation-free (include/tn.h); asynchronous."""
+    _check(lib().tn_gemm_t_static(C.c_void_p(cuda_stream), int(m), int(n), int(k), C.c_void_p(dA), int(lda),
+                                  C.c_void_p(dB), int(ldb), C.c_void_p(dC), int(ldc)))
 
 
 def tn_fp64_peak() -> float:

@@ -447,6 +447,14 @@ int tn_kernel_bench(tn_handle* h, int32_t op, int64_t m, int32_t n, int64_t k, i
   TN_API_END
 }
 
+int tn_gemm_t_static(void* cuda_stream, int64_t m, int32_t n, int64_t k, const double* dA, int64_t lda, const double* dB,
+                     int64_t ldb, double* dC, int64_t ldc) {
+  TN_API_BEGIN
+  need_device();
+  gemm_t_static_run(cuda_stream, m, n, k, dA, lda, dB, ldb, dC, ldc);
+  TN_API_END
+}
+
 int tn_get_stats(tn_handle* h, tn_stats* out) {
   TN_API_BEGIN
   if (!h || !out) tn_throw(TN_ERR_ARG, "NULL argument");

@@ -167,6 +167,9 @@ void search_logz(tn_handle* h);
 void search_run(tn_handle* h, int M, int* n_out, int8_t* states, double* energies, double* logp,
                 double* log_pd);
 void energy_run(tn_handle* h, int n, const int8_t* states, double* energies);
+// ---- tsgemm.cu: allocation-free Theta-core^T x skinny apply on device pointers (static device scratch)
+void gemm_t_static_run(void* stream, i64 m, int n, i64 k, const double* A, i64 lda, const double* B, i64 ldb, double* C,
+                       i64 ldc);
 // ---- orth.cu
 void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A, const double* B, double* C);
 void kernel_bench_run(tn_handle* h, int op, i64 m, int n, i64 k, int iters, double* ms_per_call);

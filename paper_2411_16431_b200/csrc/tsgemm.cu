@@ -240,3 +240,86 @@ bool tsgemm_batched(tn_handle* h, bool trans, i64 M, int N, i64 K, const double*
   tsb.n = nbatch; tsb.sB = sB; tsb.sC = sC;
   return tsgemm_impl(h, trans, M, N, K, A, lda, B, ldb, C, ldc, tsb);
 }
+
+// =====================================================================================================================
+// Allocation-free entry point (tn_gemm_t_static, include/tn.h): C[k x n] = A[m x k]^T . B[m x n], the "Theta-core^T x
+// skinny" apply with its split-over-the-reduction workspace in a file-scope device array instead of a device allocation:
+// for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).
+//   * The scratch is TN_STATIC_SCRATCH_DOUBLES doubles (8 MiB); every GPU that loads the library holds it until exit.
+//   * In HOST code the array's name is a host-side stand-in, not a device address: its device address is looked up once per
+//     device, with that device current, by cudaGetSymbolAddress below, and that pointer is what the kernels get.
+//   * Every call shares the array and it keeps the last call's contents.  Nothing has to start at zero: every workspace
+//     entry the reduction reads is written first by the GEMM kernel of the same call (each split CTA stores its whole
+//     in-range tile, zero or not).  Calls that overlap on the GPU (different streams, or graph branches) RACE on it.
+//   * No cudaMalloc / cudaFree / allocating library routine, no synchronisation: two kernels are queued on the stream.
+// =====================================================================================================================
+static constexpr size_t TN_STATIC_SCRATCH_DOUBLES = (size_t)1 << 20;
+static __device__ __align__(256) double g_ts_static_scratch[TN_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+
+struct DevOnly { int device; };   // what TN_SMEM_OPT_IN needs from a handle
+
+template <int NT>
+void launch_ts_static(int dev, cudaStream_t st, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc,
+                      i64 Mout, int N, i64 Kred, int nsplit, double* scratch) {
+  constexpr int WARPS = 8, BM = 16 * WARPS, NP = 8 * NT;
+  constexpr int LDA = smem_ld(BM), LDB = smem_ld(NP);
+  constexpr size_t smem = sizeof(double) * TS_STAGES * (TS_BK * LDA + TS_BK * LDB);
+  DevOnly d{dev};
+  TN_SMEM_OPT_IN(&d, (k_tsgemm<NT, WARPS, true>), smem);
+  const i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
+  nsplit = (int)((Kred + kper - 1) / kper);
+  dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit, 1u);
+  k_tsgemm<NT, WARPS, true><<<grid, WARPS * 32, smem, st>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper,
+                                                           nsplit > 1 ? scratch : nullptr, 1, 0, 0);
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) tn_throw(TN_ERR_CUDA, "tn_gemm_t_static: launch failed: %s", cudaGetErrorString(e));
+  if (nsplit > 1) {
+    k_ts_reduce<<<dim3((unsigned)((Mout * N + 255) / 256), 1u), 256, 0, st>>>(scratch, nsplit, Mout, N, C, ldc, 0);
+    e = cudaPeekAtLastError();
+    if (e != cudaSuccess) tn_throw(TN_ERR_CUDA, "tn_gemm_t_static: reduce launch failed: %s", cudaGetErrorString(e));
+  }
+}
+
+}  // namespace
+
+void gemm_t_static_run(void* stream, i64 m, int n, i64 k, const double* A, i64 lda, const double* B, i64 ldb, double* C,
+                       i64 ldc) {
+  if (!A || !B || !C || m < 1 || n < 1 || k < 1) tn_throw(TN_ERR_ARG, "tn_gemm_t_static: NULL pointer or non-positive size");
+  if (n > 96) tn_throw(TN_ERR_ARG, "tn_gemm_t_static: n = %d > 96 columns", n);
+  if (lda < k || ldb < n || ldc < n || (lda & 1) || (ldb & 1) || !aligned16(A) || !aligned16(B))
+    tn_throw(TN_ERR_ARG, "tn_gemm_t_static: lda >= k, ldb >= n, ldc >= n, lda and ldb even, A and B 16-byte aligned are required");
+  if ((size_t)k * (size_t)n * 2 > TN_STATIC_SCRATCH_DOUBLES)
+    tn_throw(TN_ERR_ARG, "tn_gemm_t_static: k * n = %lld exceeds the static scratch (two partial products of k * n doubles "
+             "must fit %zu doubles = %zu MiB); use tn_kernel_check / the handle-based path for larger outputs",
+             (long long)(k * n), TN_STATIC_SCRATCH_DOUBLES, TN_STATIC_SCRATCH_DOUBLES * sizeof(double) >> 20);
+  int dev = 0;
+  TN_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) tn_throw(TN_ERR_ARG, "tn_gemm_t_static: device ordinal %d not supported", dev);
+  // set-up, once per device, with that device current: device address of the scratch array and the SM count
+  static double* scratch_dev[64] = {nullptr};
+  static int sms_dev[64] = {0};
+  if (!scratch_dev[dev]) {
+    double* p = nullptr;
+    TN_CUDA(cudaGetSymbolAddress((void**)&p, g_ts_static_scratch));
+    if (!p) tn_throw(TN_ERR_CUDA, "tn_gemm_t_static: cudaGetSymbolAddress returned NULL");
+    TN_CUDA(cudaDeviceGetAttribute(&sms_dev[dev], cudaDevAttrMultiProcessorCount, dev));
+    scratch_dev[dev] = p;
+  }
+  // split over the reduction (rows of A): enough CTAs for two waves, at least 128 rows per split, bounded by the scratch
+  const i64 tiles = (k + 127) / 128;
+  i64 want = (2 * (i64)sms_dev[dev] + tiles - 1) / tiles;
+  want = std::min<i64>(want, std::max<i64>(1, m / 128));
+  want = std::min<i64>(want, 64);
+  want = std::min<i64>(want, (i64)(TN_STATIC_SCRATCH_DOUBLES / ((size_t)k * n)));
+  const int nsplit = (int)std::max<i64>(1, want);
+  cudaStream_t st = (cudaStream_t)stream;
+  switch ((n + 7) / 8) {
+#define TN_TS_CASE(NT_) case NT_: launch_ts_static<NT_>(dev, st, A, lda, B, ldb, C, ldc, k, n, m, nsplit, scratch_dev[dev]); break;
+    TN_TS_CASE(1) TN_TS_CASE(2) TN_TS_CASE(3) TN_TS_CASE(4) TN_TS_CASE(5) TN_TS_CASE(6)
+    TN_TS_CASE(7) TN_TS_CASE(8) TN_TS_CASE(9) TN_TS_CASE(10) TN_TS_CASE(11) TN_TS_CASE(12)
+#undef TN_TS_CASE
+    default: tn_throw(TN_ERR_ARG, "tn_gemm_t_static: n = %d", n);
+  }
+}
