@@ -736,3 +736,77 @@ def test_square_lattice_against_brute_force():
     low = np.sort(E_all)[:64]
     assert np.allclose(out["energies"][:64], low, rtol=0, atol=1e-12)
     assert np.allclose(out["logp"], -1.3 * out["energies"] - lz, rtol=0, atol=1e-9)
+
+
+# ---------------------------------------------------------------- f4: LBP local dimensional reduction (Sec. IV)
+def _brute_cell_marginals(inst, E_all, beta):
+    nb = inst.S * inst.n_s
+    ncell = inst.Ly * inst.Lx
+    lw = -beta * (E_all - E_all.min())
+    p = np.exp(lw)
+    p /= p.sum()
+    p = p.reshape((1 << nb,) * ncell)                    # axis 0 = LAST cell (highest bits)
+    out = []
+    for cidx in range(ncell):
+        ax = tuple(a for a in range(ncell) if a != ncell - 1 - cidx)
+        out.append(p.sum(axis=ax))
+    return out
+
+
+def _drop_edges(inst, pairs):
+    """instance without the inter-cell edges between the given pairs of cells ((y, x), (y, x))"""
+    cell = inst.cell_y.astype(int) * inst.Lx + inst.cell_x
+    bad = {frozenset((a[0] * inst.Lx + a[1], b[0] * inst.Lx + b[1])) for a, b in pairs}
+    keep = np.array([frozenset((cell[u], cell[v])) not in bad for u, v in zip(inst.edge_u, inst.edge_v)])
+    d = dict(inst)
+    d.update(edge_u=inst.edge_u[keep], edge_v=inst.edge_v[keep], J=inst.J[keep])
+    return instances.Instance(d)
+
+
+def test_lbp_is_exact_on_trees():
+    """'Such iterations converge to exact results for problems defined on a tree': Eqs. (11)-(13) on a
+    star of Pegasus-shaped cells that carries all three kinds of inter-cell couplings (horizontal, vertical, diagonal)
+    and on a chain of Zephyr-shaped cells reproduce the brute-force cell marginals once the iteration count reaches the
+    diameter of the tree, and do NOT before (so the iteration really propagates)."""
+    from oracle import lbp
+    full = instances.lattice(2, 2, 3, 2, p_keep=1.0, seed=4)
+    star = _drop_edges(full, [((0, 1), (1, 1)), ((1, 0), (1, 1))])
+    assert star.n_spins == 24 and len(star.J) < len(full.J)
+    beta = 0.9
+    ex = _brute_cell_marginals(star, brute.all_energies(star), beta)
+    m = model.Model(star).set_beta(beta)
+    nu = lbp.messages(m, 2)                                        # diameter of the star: 2
+    for cidx in range(4):
+        lp = lbp.log_marginals(m, nu, cidx // 2, cidx % 2)
+        assert np.abs(np.exp(lp) - ex[cidx]).max() <= 1e-13
+        st, l2 = lbp.select(m, nu, cidx // 2, cidx % 2, 5)
+        assert np.array_equal(st, np.lexsort((np.arange(64), -ex[cidx]))[:5]) and np.all(np.diff(l2) <= 0)
+    chain = instances.lattice(1, 4, 2, 2, p_keep=1.0, seed=9)
+    exc = _brute_cell_marginals(chain, brute.all_energies(chain), 1.3)
+    mc = model.Model(chain).set_beta(1.3)
+    err = []
+    for it in (1, 2, 3, 6):
+        nuc = lbp.messages(mc, it)
+        err.append(max(np.abs(np.exp(lbp.log_marginals(mc, nuc, 0, x)) - exc[x]).max() for x in range(4)))
+    assert err[0] > 1e-4 and err[1] > 1e-6 and err[2] <= 1e-13 and err[3] <= 1e-13
+
+
+def test_lbp_on_loops_is_normalised_and_close_at_high_temperature():
+    """On a lattice with loops LBP is an approximation: the marginals are normalised, the error against
+    brute force vanishes with beta (the loop corrections are high order in beta: the shortest loop of cells has four
+    edge matrices) and is visible at beta = 1."""
+    from oracle import lbp
+    inst = instances.lattice(2, 3, 2, 2, p_keep=1.0, seed=6)
+    E_all = brute.all_energies(inst)
+    errs = {}
+    for beta in (0.05, 1.0):
+        ex = _brute_cell_marginals(inst, E_all, beta)
+        m = model.Model(inst).set_beta(beta)
+        nu = lbp.messages(m, 10)
+        e = 0.0
+        for cidx in range(6):
+            lp = lbp.log_marginals(m, nu, cidx // 3, cidx % 3)
+            assert abs(np.exp(lp).sum() - 1) <= 1e-12
+            e = max(e, np.abs(np.exp(lp) - ex[cidx]).max())
+        errs[beta] = e
+    assert errs[0.05] <= 1e-9 and 1e-6 < errs[1.0] < 0.2
