@@ -229,6 +229,24 @@ int tn_kernel_check(tn_handle*, int32_t op, int64_t m, int32_t n, int32_t k, con
  *   TN_CHECK_ORTH: orthonormalisation of a random [m x n] block (k unused). */
 int tn_kernel_bench(tn_handle*, int32_t op, int64_t m, int32_t n, int64_t k, int32_t iters, double* ms_per_call);
 
+/* ---- f4: local dimensional reduction by loopy belief propagation (Sec. IV, Eqs. (11)-(13), Fig. 9).
+ * tn_lbp: `iterations` rounds of [all cluster -> edge messages, Eq. (11); all edge -> cluster messages, Eq. (12)] from
+ *   uniform messages, then the normalisers of Eq. (13); needs tn_set_beta; results stay on the
+ *   handle until the next tn_set_beta (reading S26).
+ * tn_lbp_message: the message arriving at cell (y, x) over leg 0 left, 1 right, 2 up, 3 down, 4 din, 5 dout: *n values
+ *   (<= 256, the range of the leg's projector), normalised to sum 1 (constant 1 where there is no neighbour).
+ * tn_lbp_marginals: log of the normalised LBP marginal p(x_n), Eq. (13), at n given states of cell (y, x)
+ *   (HOST uint32: bit sub*n_s + pos = that spin, as in the cluster map).
+ * tn_lbp_select: the K most probable states of cell (y, x) according to LBP ("we select the desired number
+ *   of most probable states in each cluster"): *n_out = min(K, d) states, p descending, ties by ascending state.
+ * The selection is reported; the contraction of this library keeps the full (factorised) cells. */
+int tn_lbp(tn_handle*, int32_t iterations);
+int tn_lbp_message(tn_handle*, int32_t y, int32_t x, int32_t leg, int32_t* n, double* nu /* HOST [256] */);
+int tn_lbp_marginals(tn_handle*, int32_t y, int32_t x, int64_t n, const uint32_t* cell_states /* HOST [n] */,
+                     double* logp /* HOST [n] */);
+int tn_lbp_select(tn_handle*, int32_t y, int32_t x, int32_t K, int32_t* n_out, uint32_t* cell_states /* HOST [K] */,
+                  double* logp /* HOST [K] */);
+
 /* tn_gemm_t_static: ALLOCATION-FREE variant of the Theta-core^T x skinny apply (a2, Fig. 7), for callers
  * that cannot call cudaMalloc (CUDA graph capture, tight serving loops):  C [k x n] = A [m x k]^T . B [m x n],  all three
  * DEVICE pointers, row-major with leading dimensions lda >= k, ldb >= n, ldc >= n (lda, ldb even; A, B 16-byte aligned),

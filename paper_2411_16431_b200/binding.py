@@ -11,7 +11,8 @@ _LIB_PATH = os.path.join(_HERE, "libtn_b200.so")
 
 EXPORTED_SYMBOLS = ["tn_create", "tn_set_stream", "tn_set_allocator", "tn_set_option", "tn_set_beta", "tn_contract",
                     "tn_log_z", "tn_row_lognorm", "tn_mps_shape", "tn_mps_tensor", "tn_branch_and_bound",
-                    "tn_get_stats", "tn_droplets", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_gemm_t_static", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
+                    "tn_get_stats", "tn_droplets", "tn_energy", "tn_kernel_check", "tn_kernel_bench", "tn_gemm_t_static",
+                    "tn_lbp", "tn_lbp_message", "tn_lbp_marginals", "tn_lbp_select", "tn_fp64_peak", "tn_last_error", "tn_destroy"]
 OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE = 1, 2, 3, 4, 5, 6, 7, 8, 9
 OPT_MERGE_CAP = 10
 OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 12, 13, 14, 15
@@ -69,6 +70,11 @@ def lib():
         L.tn_energy.argtypes = [C.c_void_p, C.c_int32, p_i8, p_f64]
         L.tn_droplets.argtypes = [C.c_void_p, C.c_int32, p_i32, p_f64, p_i8]
         L.tn_fp64_peak.argtypes = [p_f64]
+        p_u32 = C.POINTER(C.c_uint32)
+        L.tn_lbp.argtypes = [C.c_void_p, C.c_int32]
+        L.tn_lbp_message.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, p_i32, p_f64]
+        L.tn_lbp_marginals.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, p_u32, p_f64]
+        L.tn_lbp_select.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, p_i32, p_u32, p_f64]
         L.tn_gemm_t_static.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p,
                                        C.c_int64, C.c_void_p, C.c_int64]
         L.tn_kernel_bench.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, C.c_int64, C.c_int32, p_f64]
@@ -214,6 +220,32 @@ def tn_kernel_bench(handle, op, m, n, k, iters=10) -> float:
     return v.value
 
 
+def tn_lbp(handle, iterations):
+    _check(lib().tn_lbp(handle, int(iterations)))
+
+
+def tn_lbp_message(handle, y, x, leg):
+    n = C.c_int32()
+    out = np.empty(256, dtype=np.float64)
+    _check(lib().tn_lbp_message(handle, int(y), int(x), int(leg), C.byref(n), _ptr(out, C.c_double)))
+    return out[:n.value].copy()
+
+
+def tn_lbp_marginals(handle, y, x, cell_states):
+    st = np.ascontiguousarray(cell_states, dtype=np.uint32)
+    out = np.empty(st.size, dtype=np.float64)
+    _check(lib().tn_lbp_marginals(handle, int(y), int(x), int(st.size), _ptr(st, C.c_uint32), _ptr(out, C.c_double)))
+    return out
+
+
+def tn_lbp_select(handle, y, x, K):
+    st = np.empty(K, dtype=np.uint32)
+    lp = np.empty(K, dtype=np.float64)
+    n = C.c_int32()
+    _check(lib().tn_lbp_select(handle, int(y), int(x), int(K), C.byref(n), _ptr(st, C.c_uint32), _ptr(lp, C.c_double)))
+    return st[:n.value].copy(), lp[:n.value].copy()
+
+
 def tn_gemm_t_static(cuda_stream, m, n, k, dA, lda, dB, ldb, dC, ldc):
     """C [k x n] = A [m x k]^T . B [m x n] on DEVICE pointers (ints), allocation-free (include/tn.h); asynchronous."""
     _check(lib().tn_gemm_t_static(C.c_void_p(cuda_stream), int(m), int(n), int(k), C.c_void_p(dA), int(lda),
@@ -283,6 +315,18 @@ class TensorNetwork:
 
     def branch_and_bound(self, M):
         return tn_branch_and_bound(self.handle, M, self.n_spins)
+
+    def lbp(self, iterations):
+        tn_lbp(self.handle, iterations)
+
+    def lbp_message(self, y, x, leg):
+        return tn_lbp_message(self.handle, y, x, leg)
+
+    def lbp_marginals(self, y, x, cell_states):
+        return tn_lbp_marginals(self.handle, y, x, cell_states)
+
+    def lbp_select(self, y, x, K):
+        return tn_lbp_select(self.handle, y, x, K)
 
     def droplets(self, rank):
         return tn_droplets(self.handle, rank, self.n_spins)

@@ -13,7 +13,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtn_b200.so")
-SOURCES = ["api.cu", "kernels.cu", "tables.cu", "contract.cu", "search.cu", "probe.cu", "orth.cu", "tsgemm.cu"]
+SOURCES = ["api.cu", "kernels.cu", "tables.cu", "contract.cu", "search.cu", "probe.cu", "orth.cu", "tsgemm.cu", "lbp.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

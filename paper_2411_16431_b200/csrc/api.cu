@@ -288,6 +288,7 @@ int tn_set_beta(tn_handle* h, double beta) {
   if (!std::isfinite(beta) || beta < 0.0) tn_throw(TN_ERR_ARG, "beta must be finite and >= 0");
   DeviceGuard dg(h);
   mps_free(h);
+  h->have_lbp = false;
   memset(&h->st, 0, sizeof(h->st));
   if (h->d_cnt) TN_CUDA(cudaMemsetAsync(h->d_cnt, 0, 2 * sizeof(unsigned long long), h->stream));
   tables_set_beta(h, beta);
@@ -447,6 +448,58 @@ int tn_kernel_bench(tn_handle* h, int32_t op, int64_t m, int32_t n, int64_t k, i
   TN_API_END
 }
 
+int tn_lbp(tn_handle* h, int32_t iterations) {
+  TN_API_BEGIN
+  if (!h) tn_throw(TN_ERR_ARG, "handle is NULL");
+  if (!h->have_beta) tn_throw(TN_ERR_STATE, "tn_lbp before tn_set_beta");
+  if (iterations < 0 || iterations > 100000) tn_throw(TN_ERR_ARG, "iterations must be in 0..100000");
+  DeviceGuard dg(h);
+  lbp_run(h, iterations);
+  TN_API_END
+}
+
+int tn_lbp_message(tn_handle* h, int32_t y, int32_t x, int32_t leg, int32_t* n, double* nu) {
+  TN_API_BEGIN
+  if (!h || !n || !nu) tn_throw(TN_ERR_ARG, "NULL argument");
+  DeviceGuard dg(h);
+  lbp_message(h, y, x, leg, n, nu);
+  TN_API_END
+}
+
+int tn_lbp_marginals(tn_handle* h, int32_t y, int32_t x, int64_t n, const uint32_t* cell_states, double* logp) {
+  TN_API_BEGIN
+  if (!h || n < 0 || (n > 0 && (!cell_states || !logp))) tn_throw(TN_ERR_ARG, "bad argument");
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
+  try {
+    lbp_marginals(h, y, x, n, cell_states, logp);
+  } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
+    trim_free_list(h);
+    throw;
+  }
+  trim_free_list(h);
+  TN_API_END
+}
+
+int tn_lbp_select(tn_handle* h, int32_t y, int32_t x, int32_t K, int32_t* n_out, uint32_t* cell_states, double* logp) {
+  TN_API_BEGIN
+  if (!h || !n_out || !cell_states || !logp) tn_throw(TN_ERR_ARG, "NULL argument");
+  DeviceGuard dg(h);
+  const unsigned long long mark = h->serial;
+  try {
+    lbp_select(h, y, x, K, n_out, cell_states, logp);
+  } catch (...) {
+    cudaStreamSynchronize(h->stream);
+    h->release_since(mark);
+    trim_free_list(h);
+    throw;
+  }
+  trim_free_list(h);
+  TN_API_END
+}
+
 int tn_gemm_t_static(void* cuda_stream, int64_t m, int32_t n, int64_t k, const double* dA, int64_t lda, const double* dB,
                      int64_t ldb, double* dC, int64_t ldc) {
   TN_API_BEGIN
@@ -477,6 +530,7 @@ void tn_destroy(tn_handle* h) {
     DeviceGuard dg(h);
     cudaStreamSynchronize(h->stream);
     mps_free(h);
+    lbp_free(h);
     tables_destroy(h);
     for (void* p : {(void*)h->d_eu, (void*)h->d_ev, (void*)h->d_J, (void*)h->d_h, (void*)h->d_cell_of,
                     (void*)h->d_bit_of, (void*)h->d_cnt})

@@ -84,6 +84,8 @@ struct tn_handle {
   int D = 0, sweeps = 0;
   // options
   int merge = 0;            // TN_OPT_MERGE: merge candidates by boundary before the bound (Fig. 3(d))
+  double *lbp_nu = nullptr, *lbp_mu = nullptr;   // f4: LBP messages [cell][6][256] / [cell][7][256] (lbp.cu)
+  bool have_lbp = false;
   int droplets = 0, droplet_min_hamming = 1, droplet_max_count = 8;   // TN_OPT_DROPLETS ... (Fig. 4)
   double droplet_max_dE = 1.0;
   std::vector<int> drop_cnt;          // results of the last tn_branch_and_bound: droplets per returned state,
@@ -170,6 +172,12 @@ void energy_run(tn_handle* h, int n, const int8_t* states, double* energies);
 // ---- tsgemm.cu: allocation-free Theta-core^T x skinny apply on device pointers (static device scratch)
 void gemm_t_static_run(void* stream, i64 m, int n, i64 k, const double* A, i64 lda, const double* B, i64 ldb, double* C,
                        i64 ldc);
+// ---- lbp.cu (f4: loopy belief propagation, Sec. IV)
+void lbp_run(tn_handle* h, int iterations);
+void lbp_free(tn_handle* h);
+void lbp_message(tn_handle* h, int y, int x, int leg, int* n, double* out);
+void lbp_marginals(tn_handle* h, int y, int x, i64 n, const unsigned* states, double* logp);
+void lbp_select(tn_handle* h, int y, int x, int K, int* n_out, unsigned* states, double* logp);
 // ---- orth.cu
 void kernel_check_run(tn_handle* h, int op, i64 m, int n, int k, const double* A, const double* B, double* C);
 void kernel_bench_run(tn_handle* h, int op, i64 m, int n, i64 k, int iters, double* ms_per_call);
