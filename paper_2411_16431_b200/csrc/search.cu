@@ -267,7 +267,9 @@ __global__ void k_beam_scale(const double* logp, const double* Z, int nb, double
     __syncthreads();
   }
   mx = sh[0];
-  for (int i = threadIdx.x; i < nb; i += blockDim.x) scale[i] = Z[i] > 0.0 ? exp(logp[i] - mx) / Z[i] : 0.0;
+  // beam members more than 700 nats below the best keep a positive (clamped) scale: their children stay selectable when
+  // fewer than M better candidates exist (the exact log-scores decide the final order, k_sel_score)
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) scale[i] = Z[i] > 0.0 ? exp(fmax(logp[i] - mx, -700.0)) / Z[i] : 0.0;
   if (threadIdx.x == 0) scale[nb] = mx;   // key r = v fcd scale_m  <=>  score = log r + mx
 }
 

@@ -559,3 +559,31 @@ def test_square_lattice_workload_of_appendix_b():
     king's lattice of the same appendix (both diagonals) is outside the accepted geometry."""
     inst = instances.lattice(16, 16, 1, 1, p_keep=1.0, seed=1, h="zero")
     compare(inst, 4.0, 16, 1, 256, 1e-6)
+
+
+@pytest.mark.parametrize("sampled", [False, True])
+def test_exact_ties_beyond_the_candidate_list_follow_the_s8_order(sampled):
+    """J = 0, h = 0 on cells of 2^16 states: every candidate of every cell ties exactly, far more of them than the
+    candidate list holds.  The whole tie group is then collected and sorted, so the kept prefixes are the
+    FIRST ones in the S8 order (parent rank, then cell state) -- bit for bit the oracle's list -- and the run is
+    reproducible; select_tie_overflow counts the cells that took this route."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(2, 2, 2, 8, p_keep=0.0, seed=1, h="zero")
+    m, R, ln, ref = run_oracle(inst, 1.0, 0, 0, 8)
+    outs = []
+    for rep in range(2):
+        with _tn(inst) as t:
+            if sampled:                                   # the sampled-prefilter route (taken at the BASELINE sizes)
+                t.set_option(tnb.OPT_SELECT_DIRECT_MAX, 0)
+            t.set_beta(1.0)
+            t.contract(0, 0)
+            lz = t.log_z()
+            states, E, logp, pd = t.branch_and_bound(8)
+            st = t.stats()
+        outs.append((states.copy(), logp.copy(), pd))
+        assert abs(lz - inst.n_spins * np.log(2.0)) <= 1e-9 * lz
+        assert st["select_tie_overflow"] > 0 and st["select_tie_dropped"] == 0
+        assert np.array_equal(states, ref["states"])
+        assert np.allclose(logp, ref["logp"], rtol=1e-12, atol=0) and np.allclose(logp, -inst.n_spins * np.log(2.0))
+        assert abs(pd - ref["log_pd"]) <= 1e-9 * abs(pd)
+    assert np.array_equal(outs[0][0], outs[1][0]) and outs[0][2] == outs[1][2]
