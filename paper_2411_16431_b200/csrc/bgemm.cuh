@@ -108,12 +108,14 @@ __global__ void __launch_bounds__(256, 2) k_bgemm(int batches, int bg, int M, in
 //   BR: const double* operator()(int batch, int k) -> pointer to the N contiguous doubles of row k of B (16-byte aligned)
 //   WARPS: 8 (128 rows per CTA) or 4 (64 rows): the narrow CTA halves the shared-memory footprint, so that the K = 64,
 //   N = 64 instantiation (configs[3]) fits two independent CTAs per SM instead of one (barriers decoupled)
-template <int KP, int NT, int WARPS, class AR, class BR, class EP>
+//   NBUF: B buffers.  With 3 the fetch of batch i+1 lands in a buffer last read two batches ago, so the barrier between
+//   the multiply and the epilogue is not needed and the warps of a CTA drift out of phase (stores overlap DMMAs).
+template <int KP, int NT, int WARPS, int NBUF, class AR, class BR, class EP>
 __global__ void __launch_bounds__(32 * WARPS) k_bgemm_pipe(int batches, int bg, int M, int N, int K, AR ar, BR br, EP ep) {
   constexpr int BM = 16 * WARPS, NTH = 32 * WARPS, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
   extern __shared__ __align__(16) double bg_smem[];
   double* sA = bg_smem;
-  double* sB = bg_smem + BM * LDA;            // two buffers of KP * LDB
+  double* sB = bg_smem + BM * LDA;            // NBUF buffers of KP * LDB
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int m0 = blockIdx.y * BM;
   const int b0 = blockIdx.x * bg, b1 = min(batches, b0 + bg);
@@ -138,9 +140,9 @@ __global__ void __launch_bounds__(32 * WARPS) k_bgemm_pipe(int batches, int bg, 
     for (int k = lane; k < KP; k += 32) sA[r * LDA + k] = (src && k < K) ? __ldg(src + k) : 0.0;
   }
   for (int batch = b0; batch < b1; batch++) {
-    const int buf = (batch - b0) & 1;
+    const int buf = (batch - b0) % NBUF;
     if (batch + 1 < b1) {
-      fetch(batch + 1, buf ^ 1);
+      fetch(batch + 1, (buf + 1) % NBUF);
       asm volatile("cp.async.wait_group 1;");
     } else {
       asm volatile("cp.async.wait_group 0;");
@@ -168,7 +170,7 @@ __global__ void __launch_bounds__(32 * WARPS) k_bgemm_pipe(int batches, int bg, 
         dmma884(acc[1][j][0], acc[1][j][1], fa1, fb);
       }
     }
-    __syncthreads();      // everyone is done with sb before the fetch of batch + 2 overwrites it
+    if (NBUF < 3) __syncthreads();   // everyone is done with sb before the fetch of batch + 2 overwrites it
     if (row0 < M) {
 #pragma unroll
       for (int j = 0; j < NT; j++) {
@@ -192,12 +194,14 @@ template <int KP, int NT, class AR, class BR, class EP>
 void launch_bgemm_pipe_knt(tn_handle* h, int batches, int M, int N, int K, const AR& ar, const BR& br, const EP& ep) {
   constexpr int WARPS = (KP * NT >= 64 * 8) ? 4 : 8;     // the largest tile takes the narrow CTA (two per SM)
   constexpr int BM = 16 * WARPS, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
-  constexpr int smem = (int)sizeof(double) * (BM * LDA + 2 * KP * LDB);
-  TN_SMEM_OPT_IN(h, (k_bgemm_pipe<KP, NT, WARPS, AR, BR, EP>), smem);
+  constexpr int smem3 = (int)sizeof(double) * (BM * LDA + 3 * KP * LDB);
+  constexpr int NBUF = smem3 <= 75 * 1024 ? 3 : 2;       // a third buffer only where three CTAs per SM still fit
+  constexpr int smem = (int)sizeof(double) * (BM * LDA + NBUF * KP * LDB);
+  TN_SMEM_OPT_IN(h, (k_bgemm_pipe<KP, NT, WARPS, NBUF, AR, BR, EP>), smem);
   const int mt = (M + BM - 1) / BM;
   const int bg = (int)std::max<i64>(1, std::min<i64>(16, (i64)batches * mt / (8 * (i64)h->sms)));
   dim3 grid((unsigned)((batches + bg - 1) / bg), (unsigned)mt);
-  k_bgemm_pipe<KP, NT, WARPS, AR, BR, EP><<<grid, 32 * WARPS, smem, h->stream>>>(batches, bg, M, N, K, ar, br, ep);
+  k_bgemm_pipe<KP, NT, WARPS, NBUF, AR, BR, EP><<<grid, 32 * WARPS, smem, h->stream>>>(batches, bg, M, N, K, ar, br, ep);
   h->st.kernel_launches++;
   cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) tn_throw(TN_ERR_CUDA, "k_bgemm_pipe launch failed: %s", cudaGetErrorString(e));
