@@ -102,6 +102,8 @@ enum {
                                        boundaries of a cell fit TN_OPT_MERGE_CAP); 0 forces threshold + sort everywhere   */
   TN_OPT_SVD_DIRECT = 21,           /* 1 (default) / 0: where Theta is tiny (n <= 128, n m + n^2 <= 24000 entries) form it explicitly
                                        and take its SVD by one-sided Jacobi in one kernel instead of iterating            */
+  TN_OPT_COND_PIPE = 22,            /* 1 (default) / 0: search conditionals through the pipelined kernel k_cond (0: the generic
+                                       batched kernel, kept as the reference route for the kernel-level comparison)        */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */

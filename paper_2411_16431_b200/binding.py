@@ -19,6 +19,7 @@ OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP = 11, 
 OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT = 16, 17, 18, 19
 OPT_MERGE_SEGMENTED = 20
 OPT_SVD_DIRECT = 21
+OPT_COND_PIPE = 22
 
 
 class TnError(RuntimeError):

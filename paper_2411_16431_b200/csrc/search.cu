@@ -106,6 +106,152 @@ struct EpPV {   // stores V and, fused, collects Z_m = sum max(v, 0) fc[m][cl] a
     if (n) atomicAdd(nneg, (unsigned long long)n);
   }
 };
+// ---- conditionals, pipelined (round 2): V[m][(b,cl)][a] = w(b,cl) X[a_hi][b] sum_k LG[m][(Pd b, Po cl)][k] RMc[m][k][a]
+// One CTA = (beam element m, 128 rows (b,cl)); its A tile (gathered rows of LG) stays in shared memory while the column
+// tiles of the dense operand RMc[m] (32 columns each) stream through a cp.async double buffer, so loads of tile t+1,
+// DMMAs of tile t and the weighted stores of tile t overlap; the X factors of a tile are requested before the multiply.
+// Z_m = sum max(v, 0) fc[m][cl] and the count of negative / NaN entries come out of the epilogue as in EpPV.
+struct CondArgs {
+  const double* LG; const int *Pd, *Po; int nCl, n_o, npp, Dr;          // A rows
+  const double* RMc; int nA;                                             // B: [m][Dr][nA]
+  double* V; const double *X, *vS, *Yc, *fc; const int *vrow, *slot;     // epilogue
+  double* zpart; unsigned long long* nneg;
+  int nB, tshift, ntile, Mg; i64 per_m;
+};
+template <int KP>
+__global__ void __launch_bounds__(256) k_cond(CondArgs a) {
+  constexpr int BM = 128, NT = 4, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
+  extern __shared__ __align__(16) double cond_smem[];
+  double* sA = cond_smem;
+  double* sB = cond_smem + BM * LDA;            // two buffers of KP * LDB
+  __shared__ double s_rz[8];
+  __shared__ unsigned s_rn[8];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int m = blockIdx.x, m0 = blockIdx.y * BM, K = a.Dr, N = a.nA;
+  const double* Bm = a.RMc + (i64)m * K * N;
+  auto fetch = [&](int n0, int buf) {
+    double* dst = sB + buf * (KP * LDB);
+    constexpr int G = BN / 2;
+    for (int idx = tid; idx < KP * G; idx += 256) {
+      const int k = idx / G, g2 = 2 * (idx % G);
+      const int rem = k < K ? N - (n0 + g2) : 0;
+      const int bytes = rem >= 2 ? 16 : rem == 1 ? 8 : 0;
+      const double* src = bytes ? Bm + (i64)k * N + n0 + g2 : Bm;
+      unsigned sa = (unsigned)__cvta_generic_to_shared(dst + k * LDB + g2);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(src), "r"(bytes));
+    }
+    asm volatile("cp.async.commit_group;");
+  };
+  fetch(0, 0);
+  for (int r = warp; r < BM; r += 8) {
+    const int gi = m0 + r;
+    const double* src = gi < a.Mg ? a.LG + ((i64)m * a.npp + a.Pd[gi / a.nCl] * a.n_o + a.Po[gi % a.nCl]) * K : nullptr;
+#pragma unroll
+    for (int k = lane; k < KP; k += 32) sA[r * LDA + k] = (src && k < K) ? __ldg(src + k) : 0.0;
+  }
+  // row descriptors of this thread's two rows
+  const int row0 = m0 + 16 * warp + (lane >> 2), row1 = row0 + 8;
+  const int sl = a.slot[m];
+  double w[2], f[2], z[2] = {0.0, 0.0};
+  const double* xr[2];
+  double* vp[2];
+  unsigned neg = 0;
+#pragma unroll
+  for (int i = 0; i < 2; i++) {
+    const int row = i ? row1 : row0, rr = row < a.Mg ? row : 0, b = rr / a.nCl, cl = rr % a.nCl;
+    w[i] = a.vS[(i64)a.vrow[sl] * a.nB + b] * a.Yc[b * a.nCl + cl];
+    f[i] = a.fc[(i64)m * a.nCl + cl];
+    xr[i] = a.X + b;
+    vp[i] = a.V + (i64)m * a.per_m + (i64)rr * N;
+  }
+  const int ntn = (N + BN - 1) / BN;
+  for (int t = 0; t < ntn; t++) {
+    const int buf = t & 1, n0 = t * BN;
+    if (t + 1 < ntn) {
+      fetch(n0 + BN, buf ^ 1);
+      asm volatile("cp.async.wait_group 1;");
+    } else {
+      asm volatile("cp.async.wait_group 0;");
+    }
+    __syncthreads();
+    // X factors of this tile (columns a, a+1 share a_hi: tshift >= 1), requested before the multiply
+    double xv[2][NT];
+#pragma unroll
+    for (int j = 0; j < NT; j++) {
+      const int col = n0 + 8 * j + 2 * (lane & 3), cc = col < N ? col : 0;
+      xv[0][j] = __ldg(xr[0] + (i64)(cc >> a.tshift) * a.nB);
+      xv[1][j] = __ldg(xr[1] + (i64)(cc >> a.tshift) * a.nB);
+    }
+    const double* sb = sB + buf * (KP * LDB);
+    double acc[2][NT][2];
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+      for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+#pragma unroll
+    for (int kk = 0; kk < KP; kk += 4) {
+      const double fa0 = sA[(16 * warp + (lane >> 2)) * LDA + kk + (lane & 3)];
+      const double fa1 = sA[(16 * warp + 8 + (lane >> 2)) * LDA + kk + (lane & 3)];
+      const double* brow = sb + (kk + (lane & 3)) * LDB + (lane >> 2);
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const double fb = brow[8 * j];
+        dmma884(acc[0][j][0], acc[0][j][1], fa0, fb);
+        dmma884(acc[1][j][0], acc[1][j][1], fa1, fb);
+      }
+    }
+    __syncthreads();      // everyone is done with sb before the fetch of tile t + 2 overwrites it
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+      if ((i ? row1 : row0) >= a.Mg) continue;
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const int col = n0 + 8 * j + 2 * (lane & 3);
+        if (col >= N) continue;
+        const double s = w[i] * xv[i][j];
+        const double o0 = acc[i][j][0] * s, o1 = acc[i][j][1] * s;
+        *reinterpret_cast<double2*>(vp[i] + col) = make_double2(o0, o1);     // N even, col even
+        z[i] += fmax(o0, 0.0) + fmax(o1, 0.0);
+        neg += (o0 >= 0.0 ? 0u : 1u) + (o1 >= 0.0 ? 0u : 1u);               // negatives and NaNs (reading S7)
+      }
+    }
+  }
+  // ordered CTA reduction -> one partial per (m, row tile)
+  double tz = z[0] * f[0] + z[1] * f[1];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    tz += __shfl_xor_sync(0xffffffffu, tz, o);
+    neg += __shfl_xor_sync(0xffffffffu, neg, o);
+  }
+  if (lane == 0) { s_rz[warp] = tz; s_rn[warp] = neg; }
+  __syncthreads();
+  if (tid == 0) {
+    double zz = 0.0;
+    unsigned nn = 0;
+    for (int q = 0; q < 8; q++) { zz += s_rz[q]; nn += s_rn[q]; }
+    a.zpart[(i64)m * a.ntile + blockIdx.y] = zz;
+    if (nn) atomicAdd(a.nneg, (unsigned long long)nn);
+  }
+}
+template <int KP>
+static void launch_cond_k(tn_handle* h, int nb, const CondArgs& a) {
+  constexpr int LDA = smem_ld(KP), LDB = smem_ld(32);
+  constexpr int smem = (int)sizeof(double) * (128 * LDA + 2 * KP * LDB);
+  TN_SMEM_OPT_IN(h, k_cond<KP>, smem);
+  k_cond<KP><<<dim3((unsigned)nb, (unsigned)a.ntile), 256, smem, h->stream>>>(a);
+  TN_LAUNCH_CHECK(h);
+}
+// returns false when the shape does not fit (odd nA, X not shared by column pairs, bond > 64, too many row tiles)
+static bool launch_cond(tn_handle* h, int nb, const CondArgs& a) {
+  if (a.Dr < 1 || a.Dr > 64 || (a.nA & 1) || a.tshift < 1 || a.ntile > 65535 || (((uintptr_t)a.RMc) & 15) || (((uintptr_t)a.V) & 15))
+    return false;
+  if (a.Dr <= 16) launch_cond_k<16>(h, nb, a);
+  else if (a.Dr <= 32) launch_cond_k<32>(h, nb, a);
+  else if (a.Dr <= 48) launch_cond_k<48>(h, nb, a);
+  else launch_cond_k<64>(h, nb, a);
+  return true;
+}
+
 struct LdHA {   // A(i=(b',b''), kk=(b,cl)) = G[(Pd b * n_o + Po cl)][i]
   const double* G; const int *Pd, *Po; int nCl, n_o; i64 DD;
   __device__ __forceinline__ double operator()(int, int i, int kk) const {
@@ -1238,7 +1384,12 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         DBuf<double> zpart(h, (size_t)nb * std::max(ntile, 64));
         EpPV ep{V.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
                 c.nA, c.nB, c.nCl, c.tshift, ntile, per_m};
-        if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
+        CondArgs ca{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr, RMc.p, c.nA, V.p, c.X, c.BvS, c.Yc, fc.p,
+                    vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p, c.nB, c.tshift, ntile, Mg, per_m};
+        if (h->cond_pipe && launch_cond(h, nb, ca)) {
+          k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
+          TN_LAUNCH_CHECK(h);
+        } else if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
           // Z and the negative count came out of the GEMM epilogue: no extra pass over V
           k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
           TN_LAUNCH_CHECK(h);

@@ -86,3 +86,26 @@ def test_skinny_gemm_n_and_t(tn, m, n, k):
     Ct = _check(tn, tnb.CHECK_GEMM_T, A, Bt)
     reft = A.T @ Bt
     assert np.abs(Ct - reft).max() <= 1e-13 * m * max(1.0, np.abs(reft).max())
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,D", [(3, 3, 3, 4, 0.9, 4, 6), (3, 3, 2, 8, 0.97, 3, 12), (4, 4, 2, 4, 0.95, 2, 5)])
+def test_pipelined_conditional_kernel_against_the_generic_route(Ly, Lx, S, ns, p, seed, D):
+    """k_cond (cp.async-pipelined conditional GEMM, TN_OPT_COND_PIPE = 1, the default) against the generic batched kernel
+    (TN_OPT_COND_PIPE = 0) on the same boundary MPS: identical states, log-probabilities to rounding (the per-beam
+    normaliser is summed in another tile order), identical count of clamped negative conditionals; odd bonds (D = 5)
+    and ragged projectors included."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    out = []
+    for pipe in (1, 0):
+        with tnb.TensorNetwork(inst) as t:
+            t.set_option(tnb.OPT_COND_PIPE, pipe)
+            t.set_beta(1.2)
+            t.contract(D, 1)
+            lz = t.log_z()
+            states, E, logp, pd = t.branch_and_bound(64)
+            out.append((lz, states, logp, pd, t.stats()["negative_u"]))
+    assert abs(out[0][0] - out[1][0]) <= 1e-13 * abs(out[0][0])
+    assert np.array_equal(out[0][1], out[1][1])
+    assert np.allclose(out[0][2], out[1][2], rtol=1e-12, atol=0) and abs(out[0][3] - out[1][3]) <= 1e-12 * abs(out[0][3])
+    assert out[0][4] == out[1][4]
