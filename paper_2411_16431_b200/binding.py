@@ -20,6 +20,7 @@ OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT
 OPT_MERGE_SEGMENTED = 20
 OPT_SVD_DIRECT = 21
 OPT_COND_PIPE = 22
+OPT_TS_WIDE_ROWS = 23
 
 
 class TnError(RuntimeError):

@@ -26,12 +26,15 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 // TRANS = false: CTA owns rows [m0, m0+BM) of A / C, reduction index = columns of A.
 // TRANS = true : CTA owns columns [m0, m0+BM) of A (= rows of C), reduction index = rows of A.
-// In both cases "i" is the output row (BM per CTA, 16 per warp) and "kk" the reduction index.
-template <int NT, int WARPS, bool TRANS>
+// In both cases "i" is the output row (BM per CTA, 8 RPW per warp) and "kk" the reduction index.
+// RPW = 8-row fragments per warp: 2 (16 rows) by default; 3 (24 rows per warp, 192 per CTA) for narrow column counts,
+// where the multiply is limited by the shared-memory fragment loads per DMMA (measured: 74 % of the DMMA peak at 48
+// columns against 86 % at 80): 3 NT DMMAs per 3 + NT fragment loads instead of 2 NT per 2 + NT, still two CTAs per SM.
+template <int NT, int WARPS, bool TRANS, int RPW = 2>
 __global__ void __launch_bounds__(WARPS * 32, (NT <= 10 || WARPS < 8) ? 2 : 1)
 k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i64 ldb, double* __restrict__ C, i64 ldc,
          i64 Mout, int Nfull, i64 Kred, i64 kper, double* __restrict__ ws, int nz, i64 sBz, i64 sCz) {
-  constexpr int BM = 16 * WARPS, NTH = 32 * WARPS, NP = 8 * NT;
+  constexpr int BM = 8 * RPW * WARPS, NTH = 32 * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK);   // doubles
   constexpr int LDB = smem_ld(NP);
   constexpr int A_ELEMS = TRANS ? TS_BK * LDA : BM * LDA;
@@ -89,9 +92,9 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
     }
   };
 
-  double acc[2][NT][2];
+  double acc[RPW][NT][2];
 #pragma unroll
-  for (int i = 0; i < 2; i++)
+  for (int i = 0; i < RPW; i++)
 #pragma unroll
     for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
@@ -109,17 +112,17 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
     const double* b = sB + (kt % TS_STAGES) * B_ELEMS;
 #pragma unroll
     for (int kk = 0; kk < TS_BK; kk += 4) {
-      double fa[2];
+      double fa[RPW];
 #pragma unroll
-      for (int i = 0; i < 2; i++)
-        fa[i] = TRANS ? a[(kk + (lane & 3)) * LDA + 16 * warp + 8 * i + (lane >> 2)]
-                      : a[(16 * warp + 8 * i + (lane >> 2)) * LDA + kk + (lane & 3)];
+      for (int i = 0; i < RPW; i++)
+        fa[i] = TRANS ? a[(kk + (lane & 3)) * LDA + 8 * RPW * warp + 8 * i + (lane >> 2)]
+                      : a[(8 * RPW * warp + 8 * i + (lane >> 2)) * LDA + kk + (lane & 3)];
       const double* brow = b + (kk + (lane & 3)) * LDB + (lane >> 2);
 #pragma unroll
       for (int j = 0; j < NT; j++) {
         const double fb = brow[8 * j];
-        dmma884(acc[0][j][0], acc[0][j][1], fa[0], fb);
-        dmma884(acc[1][j][0], acc[1][j][1], fa[1], fb);
+#pragma unroll
+        for (int i = 0; i < RPW; i++) dmma884(acc[i][j][0], acc[i][j][1], fa[i], fb);
       }
     }
   }
@@ -128,8 +131,8 @@ k_tsgemm(const double* __restrict__ A, i64 lda, const double* __restrict__ B, i6
   double* out = (nsplit > 1 ? ws + ((size_t)bz * nsplit + split) * Mout * Nfull : C + (i64)bz * sCz) + n_off;
   const i64 ldo = nsplit > 1 ? Nfull : ldc;
 #pragma unroll
-  for (int i = 0; i < 2; i++) {
-    const i64 row = m0 + 16 * warp + 8 * i + (lane >> 2);
+  for (int i = 0; i < RPW; i++) {
+    const i64 row = m0 + 8 * RPW * warp + 8 * i + (lane >> 2);
     if (row < Mout) {
 #pragma unroll
       for (int j = 0; j < NT; j++) {
@@ -154,20 +157,20 @@ __global__ void k_ts_reduce(const double* __restrict__ ws, int nsplit, i64 M, in
 
 struct TsBatch { int n = 1; i64 sB = 0, sC = 0; };   // independent products sharing A: B_z = B + z sB, C_z = C + z sC
 
-template <int NT, int WARPS, bool TRANS>
+template <int NT, int WARPS, bool TRANS, int RPW = 2>
 void launch_ts(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
                i64 Kred, int nsplit, const TsBatch& tsb) {
-  constexpr int BM = 16 * WARPS, NP = 8 * NT;
+  constexpr int BM = 8 * RPW * WARPS, NP = 8 * NT;
   constexpr int LDA = TRANS ? smem_ld(BM) : smem_ld(TS_BK), LDB = smem_ld(NP);
   constexpr size_t smem = sizeof(double) * TS_STAGES * ((TRANS ? TS_BK * LDA : BM * LDA) + TS_BK * LDB);
-  TN_SMEM_OPT_IN(h, (k_tsgemm<NT, WARPS, TRANS>), smem);
+  TN_SMEM_OPT_IN(h, (k_tsgemm<NT, WARPS, TRANS, RPW>), smem);
   i64 kper = ((Kred + nsplit - 1) / nsplit + TS_BK - 1) / TS_BK * TS_BK;
   nsplit = (int)((Kred + kper - 1) / kper);
   const int nbz = tsb.n, nz = (N + NP - 1) / NP;
   double* ws = nsplit > 1 ? h->dalloc<double>((size_t)nbz * nsplit * Mout * N) : nullptr;
   dim3 grid((unsigned)((Mout + BM - 1) / BM), (unsigned)nsplit, (unsigned)(nz * nbz));
-  k_tsgemm<NT, WARPS, TRANS><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws, nz,
-                                                                     tsb.sB, tsb.sC);
+  k_tsgemm<NT, WARPS, TRANS, RPW><<<grid, WARPS * 32, smem, h->stream>>>(A, lda, B, ldb, C, ldc, Mout, N, Kred, kper, ws, nz,
+                                                                          tsb.sB, tsb.sC);
   TN_LAUNCH_CHECK(h);
   if (nsplit > 1) {
     k_ts_reduce<<<dim3(cdiv(Mout * N, 256), nbz), 256, 0, h->stream>>>(ws, nsplit, Mout, N, C, ldc, tsb.sC);
@@ -183,9 +186,15 @@ template <int NT, bool TRANS>
 void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, i64 Mout, int N,
                 i64 Kred, const TsBatch& tsb) {
   int warps = Mout > 64 ? 8 : Mout > 32 ? 4 : 2;
-  const i64 tiles = (Mout + 16 * warps - 1) / (16 * warps) * ((N + 8 * NT - 1) / (8 * NT)) * tsb.n;
+  // 24 rows per warp for 40..48 columns once the output has enough rows to fill the GPU with the 192-row tiles
+  // (measured on B200: 74 -> 80 % of the DMMA peak at 48 columns; neutral at 40, worse at 24, so only NT = 5, 6)
+  constexpr bool kWide = NT >= 5 && NT <= 6;
+  const bool enough = !TRANS && Mout >= (i64)192 * 2 * h->sms;   // (the T variant loses more to its split quantisation: 75 -> 71 %)
+  const int rpw = (kWide && warps == 8 && h->ts_rpw3 && enough) ? 3 : 2;
+  const int bm = 8 * rpw * warps;
+  const i64 tiles = (Mout + bm - 1) / bm * ((N + 8 * NT - 1) / (8 * NT)) * tsb.n;
   const int slots = h->sms * ((NT <= 10 || warps < 8) ? 2 : 1);
-  const double t_k = 2.0 * 16 * warps * (8 * NT) * slots / 37e12;      // seconds per reduction index per CTA
+  const double t_k = 2.0 * bm * (8 * NT) * slots / 37e12;              // seconds per reduction index per CTA
   const double t_ws = (double)Mout * N * 16.0 / 6e12 + 2e-7;           // seconds per extra split (write + read)
   int best = 1;
   double best_t = 1e30;
@@ -194,6 +203,9 @@ void pick_warps(tn_handle* h, const double* A, i64 lda, const double* B, i64 ldb
     const i64 waves = (tiles * sp + slots - 1) / slots;
     const double t = waves * ((double)((Kred + sp - 1) / sp) + 96.0) * t_k + (sp > 1 ? sp * t_ws + 6e-6 : 0.0);
     if (t < best_t) { best_t = t; best = sp; }
+  }
+  if constexpr (kWide) {
+    if (rpw == 3) { launch_ts<NT, 8, TRANS, 3>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb); return; }
   }
   if (warps == 8) launch_ts<NT, 8, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);
   else if (warps == 4) launch_ts<NT, 4, TRANS>(h, A, lda, B, ldb, C, ldc, Mout, N, Kred, best, tsb);

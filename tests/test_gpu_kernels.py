@@ -70,7 +70,8 @@ def test_orth_columns_zero_columns_stay_zero(tn):
 
 
 GEMM = [(1, 1, 1), (5, 3, 7), (128, 16, 128), (129, 17, 65), (1000, 32, 515), (4096, 80, 300), (333, 96, 2049),
-        (70000, 24, 64), (50, 130, 40)]
+        (70000, 24, 64), (50, 130, 40),
+        (60001, 48, 130), (310, 40, 60002), (57000, 30, 18)]      # 24-row warp tiles (outputs with >= 192 * 2 * SMs rows)
 
 
 @pytest.mark.parametrize("m,n,k", GEMM)
