@@ -21,6 +21,7 @@ OPT_MERGE_SEGMENTED = 20
 OPT_SVD_DIRECT = 21
 OPT_COND_PIPE = 22
 OPT_TS_WIDE_ROWS = 23
+OPT_RBLOCK_FACT = 24
 
 
 class TnError(RuntimeError):

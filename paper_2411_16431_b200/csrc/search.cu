@@ -282,6 +282,89 @@ __global__ void k_coef(const double* X, const double* vS, const double* Yc, cons
   const int b = kk / nCl, cl = kk % nCl, m = j / nT, tt = j % nT;
   out[t] = X[tt * nB + b] * vS[(i64)vrow[m] * nB + b] * Yc[b * nCl + cl] * fc[(i64)m * nCl + cl];
 }
+// ---- right blocks, factorised (round 2).  coef_m[(b,cl); t] = X[t][b] vS_m[b] Yc[b][cl] fc_m[cl] is a product of a factor
+// in (t, b) and a factor in (b, cl), so
+//   H_m[i; t] = sum_b X[t][b] vS_m[b] ( sum_cl Gy[(b,cl)][i] fc_m[cl] ),   Gy[(b,cl)][i] = Yc[b][cl] G[(Pd b, Po cl)][i]
+// costs 2 DD n_b (n_cl + n_T) FLOP per beam element instead of the 2 DD n_b n_cl n_T of the joint GEMM (8 x fewer for
+// 16 x 16): plain FMA work on operands that stay in shared memory / L2, no intermediate in HBM.
+// One CTA = 64 values of i = (b', b'') x 8 beam elements; thread = (i, 2 beam elements); b runs in chunks of 4 staged in
+// shared memory.
+__global__ void k_gather_Gy(const double* G, const double* Yc, const int* Pd, const int* Po, int nCl, int n_o, i64 DD, int Kg,
+                            double* out) {
+  i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (i64)Kg * DD) return;
+  const int kk = (int)(t / DD);
+  const i64 i = t % DD;
+  out[t] = Yc[kk] * G[(i64)(Pd[kk / nCl] * n_o + Po[kk % nCl]) * DD + i];
+}
+template <int NTT>   // NTT = number of a_hi values (n_T <= 16), compile-time bound of the accumulators
+__global__ void __launch_bounds__(256, 2) k_rblock_h(const double* __restrict__ Gy, const double* __restrict__ X,
+                                                  const double* __restrict__ vS, const double* __restrict__ fc,
+                                                  const int* __restrict__ vrow, int nb, int nB, int nCl, int nT, i64 DD,
+                                                  double* __restrict__ H) {
+  constexpr int BI = 64, BMM = 8, BB = 4;           // i values, beam elements, b values per stage (32 KB of G per stage)
+  __shared__ double sG[BB][16][BI];                 // [b][cl][i]
+  __shared__ double sX[BB][NTT];                    // X[t][b] of the stage
+  __shared__ double sF[BMM][16];                    // fc[m][cl]
+  __shared__ double sV[BMM][BB];                    // vS[vrow m][b] of the stage
+  const int tid = threadIdx.x, ti = tid & (BI - 1), tm = tid >> 6;        // 4 groups of 64 threads, 2 beam elements each
+  const i64 i0 = (i64)blockIdx.x * BI;
+  const int m0 = blockIdx.y * BMM;
+  for (int e = tid; e < BMM * 16; e += 256) {
+    const int mm = e / 16, cl = e % 16, m = m0 + mm;
+    sF[mm][cl] = (m < nb && cl < nCl) ? fc[(i64)m * nCl + cl] : 0.0;
+  }
+  double acc[2][NTT];
+#pragma unroll
+  for (int q = 0; q < 2; q++)
+#pragma unroll
+    for (int t = 0; t < NTT; t++) acc[q][t] = 0.0;
+  for (int b0 = 0; b0 < nB; b0 += BB) {
+    __syncthreads();
+    for (int e = tid; e < BB * nCl * BI; e += 256) {
+      const int ii = e % BI, cl = (e / BI) % nCl, bb = e / (BI * nCl);
+      const i64 gi = i0 + ii;
+      sG[bb][cl][ii] = (b0 + bb < nB && gi < DD) ? Gy[((i64)(b0 + bb) * nCl + cl) * DD + gi] : 0.0;
+    }
+    for (int e = tid; e < BB * NTT; e += 256) {
+      const int t = e % NTT, bb = e / NTT;
+      sX[bb][t] = (t < nT && b0 + bb < nB) ? X[(i64)t * nB + b0 + bb] : 0.0;
+    }
+    if (tid < BMM * BB) {
+      const int mm = tid / BB, bb = tid % BB, m = m0 + mm;
+      sV[mm][bb] = (m < nb && b0 + bb < nB) ? vS[(i64)vrow[m] * nB + b0 + bb] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int bb = 0; bb < BB; bb++) {
+      double w0 = 0.0, w1 = 0.0;
+      for (int cl = 0; cl < nCl; cl++) {
+        const double g = sG[bb][cl][ti];
+        w0 += g * sF[2 * tm][cl];
+        w1 += g * sF[2 * tm + 1][cl];
+      }
+      w0 *= sV[2 * tm][bb];
+      w1 *= sV[2 * tm + 1][bb];
+#pragma unroll
+      for (int t = 0; t < NTT; t++) {
+        const double xv = sX[bb][t];
+        acc[0][t] += xv * w0;
+        acc[1][t] += xv * w1;
+      }
+    }
+  }
+  const i64 gi = i0 + ti;
+  if (gi < DD)
+#pragma unroll
+    for (int q = 0; q < 2; q++) {
+      const int m = m0 + 2 * tm + q;
+      if (m < nb)
+#pragma unroll
+        for (int t = 0; t < NTT; t++)
+          if (t < nT) H[((i64)m * nT + t) * DD + gi] = acc[q][t];
+    }
+}
+
 struct StH { double* H; i64 DD; __device__ __forceinline__ void operator()(int, int, int i, int j, double v) const { H[(i64)j * DD + i] = v; } };
 
 // ---- small kernels -------------------------------------------------------------------------------
@@ -1313,11 +1396,24 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       TN_LAUNCH_CHECK(h);
       {   // H[(m,t)][(b',b'')] = sum_{(b,cl)} coef[(b,cl)][(m,t)] G[(Pd b, Po cl)][(b',b'')]
         const int Mg = (int)DD, Ng = nb * c.nT, Kg = c.nB * c.nCl;
-        h->st.flop_search += 2.0 * Mg * (double)Ng * Kg;
-        h->st.flop_search_rblocks += 2.0 * Mg * (double)Ng * Kg + 2.0 * nb * (double)Dl * c.nA * Dr +
-                                     2.0 * nb * (double)Dl * c.bh_rows * c.nA;
         bool done = false;
-        if ((DD & 1) == 0 && (Ng & 1) == 0) {
+        const bool fact = h->rblock_fact && c.nT <= 16 && c.nCl <= 16;
+        const double fl = fact ? 2.0 * Mg * (double)nb * c.nB * (c.nCl + c.nT) : 2.0 * Mg * (double)Ng * Kg;
+        h->st.flop_search += fl;
+        h->st.flop_search_rblocks += fl + 2.0 * nb * (double)Dl * c.nA * Dr + 2.0 * nb * (double)Dl * c.bh_rows * c.nA;
+        if (fact) {
+          DBuf<double> Gy(h, (size_t)Kg * DD);
+          k_gather_Gy<<<cdiv((i64)Kg * DD, 256), 256, 0, h->stream>>>(rt[x].G, c.Yc, c.Pd, c.Po, c.nCl, c.n_o, DD, Kg, Gy.p);
+          TN_LAUNCH_CHECK(h);
+          dim3 grid((unsigned)cdiv(DD, 64), (unsigned)cdiv(nb, 8));
+          if (c.nT <= 4)
+            k_rblock_h<4><<<grid, 256, 0, h->stream>>>(Gy.p, c.X, c.BvS, fcx.p, vrow.p + (size_t)x * nb, nb, c.nB, c.nCl, c.nT, DD, H.p);
+          else
+            k_rblock_h<16><<<grid, 256, 0, h->stream>>>(Gy.p, c.X, c.BvS, fcx.p, vrow.p + (size_t)x * nb, nb, c.nB, c.nCl, c.nT, DD, H.p);
+          TN_LAUNCH_CHECK(h);
+          done = true;
+        }
+        if (!done && (DD & 1) == 0 && (Ng & 1) == 0) {
           // both operands materialised row-major in the reduction index, then the streaming GEMM (tsgemm.cu)
           DBuf<double> Gg(h, (size_t)Kg * DD), cf(h, (size_t)Kg * Ng);
           k_gather_G<<<cdiv((i64)Kg * DD, 256), 256, 0, h->stream>>>(rt[x].G, c.Pd, c.Po, c.nCl, c.n_o, DD, Kg, Gg.p);
