@@ -620,25 +620,38 @@ void theta_core(tn_handle* h, const CellDev& c, const double* A, int dx, int dy,
 // ============================================================================================
 // mediating-tensor pieces
 // ============================================================================================
-__global__ void k_med_apply_bd(const double* T1, const double* Bd, double* Theta, int al, int n_o, int n_r,
-                               int n_i, int n_q, int g) {
+// one thread per (al, r, o, g): the n_i inputs are read ONCE into registers and all n_q outputs written from them
+// (n_i, n_q <= 16; Bd in shared memory) -- the first version re-read every input n_q times through L2
+__global__ void __launch_bounds__(256) k_med_apply_bd(const double* __restrict__ T1, const double* __restrict__ Bd,
+                                                      double* __restrict__ Theta, int al, int n_o, int n_r, int n_i, int n_q,
+                                                      int g) {
+  __shared__ double sBd[256];
+  for (int e = threadIdx.x; e < n_q * n_i; e += blockDim.x) sBd[e] = Bd[e];
+  __syncthreads();
   i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-  i64 total = (i64)al * n_r * n_o * n_q * g;
+  i64 total = (i64)al * n_r * n_o * g;
   if (t >= total) return;
   int ig = (int)(t % g);
   i64 u = t / g;
-  int q = (int)(u % n_q); u /= n_q;
   int o = (int)(u % n_o); u /= n_o;
   int r = (int)(u % n_r);
   int a = (int)(u / n_r);
   const double* src = T1 + ((((i64)a * n_o + o) * n_r + r) * n_i) * g + ig;
-  double acc = 0.0;
-  for (int i = 0; i < n_i; i++) acc += Bd[q * n_i + i] * src[(i64)i * g];
-  Theta[t] = acc;
+  double v[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) v[i] = i < n_i ? src[(i64)i * g] : 0.0;
+  double* dst = Theta + ((((i64)a * n_r + r) * n_o + o) * n_q) * g + ig;
+  for (int q = 0; q < n_q; q++) {
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc += (i < n_i ? sBd[q * n_i + i] : 0.0) * v[i];
+    dst[(i64)q * g] = acc;
+  }
 }
 void med_apply_bd(tn_handle* h, const double* T1, const double* Bd, double* Theta, int al, int n_o, int n_r,
                   int n_i, int n_q, int g) {
-  i64 total = (i64)al * n_r * n_o * n_q * g;
+  if (n_i > 16 || n_q > 16) tn_throw(TN_ERR_ARG, "mediating position: diagonal leg of %d x %d states (at most 16 x 16)", n_q, n_i);
+  i64 total = (i64)al * n_r * n_o * g;
   k_med_apply_bd<<<cdiv(total, 256), 256, 0, h->stream>>>(T1, Bd, Theta, al, n_o, n_r, n_i, n_q, g);
   TN_LAUNCH_CHECK(h);
 }
