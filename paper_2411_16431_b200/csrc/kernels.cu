@@ -403,24 +403,42 @@ __device__ __forceinline__ int pdep8(int v, int mask) {
 }
 
 // Yk[o][(a,cl)][s] = sum_ch wC[cl][ch] * Y[o][Pl[a]*n_i + Pi[ch]][s]
-__global__ void k_map_L_med(CellDev c, const double* Y, double* Yk, int outer, int s) {
+// one thread per (o, a, s): the n_i inputs are read once into registers and all n_cl outputs written from them
+// (W1[cl][i] = sum_{ch: Pi ch = i} wC[cl][ch] in shared memory); n_i, n_cl <= 16
+__global__ void __launch_bounds__(256) k_map_L_med(CellDev c, const double* __restrict__ Y, double* __restrict__ Yk, int outer,
+                                                   int s) {
+  __shared__ double W1[256];
+  for (int e = threadIdx.x; e < c.nCl * c.n_i; e += blockDim.x) {
+    const int cl = e / c.n_i, i = e % c.n_i;
+    double w = 0.0;
+    for (int ch = 0; ch < c.nCh; ch++)
+      if (c.Pi[ch] == i) w += c.wC[cl * c.nCh + ch];
+    W1[e] = w;
+  }
+  __syncthreads();
   i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-  i64 total = (i64)outer * c.nK * s;
+  i64 total = (i64)outer * c.nA * s;
   if (t >= total) return;
   int is = (int)(t % s);
-  int k = (int)((t / s) % c.nK);
-  int o = (int)(t / ((i64)s * c.nK));
-  int a = k / c.nCl, cl = k % c.nCl;
+  int a = (int)((t / s) % c.nA);
+  int o = (int)(t / ((i64)s * c.nA));
   const double* base = Y + ((i64)o * (c.n_l * c.n_i) + (i64)c.Pl[a] * c.n_i) * s + is;
-  double acc = 0.0;
-  for (int ch = 0; ch < c.nCh; ch++) acc += c.wC[cl * c.nCh + ch] * base[(i64)c.Pi[ch] * s];
-  Yk[t] = acc;
+  double v[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) v[i] = i < c.n_i ? base[(i64)i * s] : 0.0;
+  double* dst = Yk + ((i64)o * c.nK + (i64)a * c.nCl) * s + is;
+  for (int cl = 0; cl < c.nCl; cl++) {
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc += (i < c.n_i ? W1[cl * c.n_i + i] : 0.0) * v[i];
+    dst[(i64)cl * s] = acc;
+  }
 }
 // Y[o][(l,i)][s] = sum_{a: Pl a = l} sum_cl sum_{ch: Pi ch = i} wC[cl][ch] Yk[o][(a,cl)][s]
-// W2[i][cl] = sum_{ch: Pi ch = i} wC[cl][ch] is built once per CTA in shared memory (n_i * nCl <= 256 entries), so
-// the inner loop is one FMA per (a, cl) with loads that are coalesced over s.
-__global__ void __launch_bounds__(256) k_map_LT_med(CellDev c, const double* Yk, double* Y, int outer, int s, int nbits,
-                                                    int half) {
+// one thread per (o, l, s): every Yk entry is read once, the n_i outputs accumulate in registers
+// (W2[i][cl] = sum_{ch: Pi ch = i} wC[cl][ch] in shared memory)
+__global__ void __launch_bounds__(256) k_map_LT_med(CellDev c, const double* __restrict__ Yk, double* __restrict__ Y, int outer,
+                                                    int s, int nbits, int half) {
   __shared__ double W2[256];
   const int fc_mask = (~c.m_din) & (c.nCh - 1), nfc = c.nCh / c.n_i;
   for (int e = threadIdx.x; e < c.n_i * c.nCl; e += blockDim.x) {
@@ -432,24 +450,30 @@ __global__ void __launch_bounds__(256) k_map_LT_med(CellDev c, const double* Yk,
   }
   __syncthreads();
   i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-  int wl = c.n_l * c.n_i;
-  i64 total = (i64)outer * wl * s;
+  i64 total = (i64)outer * c.n_l * s;
   if (t >= total) return;
   int is = (int)(t % s);
-  int li = (int)((t / s) % wl);
-  int o = (int)(t / ((i64)s * wl));
-  int l = li / c.n_i, i = li % c.n_i;
+  int l = (int)((t / s) % c.n_l);
+  int o = (int)(t / ((i64)s * c.n_l));
   int fa_mask = (~c.m_left) & (c.nA - 1);
   int nfa = c.nA / c.n_l;
   int a0 = pdep8(l, c.m_left);
-  const double* w2 = W2 + i * c.nCl;
-  double acc = 0.0;
+  double acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = 0.0;
   for (int fa = 0; fa < nfa; fa++) {
     const int a = a0 | pdep8(fa, fa_mask);
     const double* src = Yk + ((i64)o * c.nK + (i64)a * c.nCl) * s + is;
-    for (int cl = 0; cl < c.nCl; cl++) acc += w2[cl] * src[(i64)cl * s];
+    for (int cl = 0; cl < c.nCl; cl++) {
+      const double v = src[(i64)cl * s];
+#pragma unroll
+      for (int i = 0; i < 16; i++) acc[i] += (i < c.n_i ? W2[i * c.nCl + cl] : 0.0) * v;
+    }
   }
-  Y[t] = acc;
+  double* dst = Y + ((i64)o * (c.n_l * c.n_i) + (i64)l * c.n_i) * s + is;
+#pragma unroll
+  for (int i = 0; i < 16; i++)
+    if (i < c.n_i) dst[(i64)i * s] = acc[i];
 }
 // Yk[o][(a,cl)][s] = Y[o][Pr[a]*n_o + Po[cl]][s]
 __global__ void k_map_R(CellDev c, const double* Y, double* Yk, int outer, int s) {
@@ -497,7 +521,7 @@ void map_L(tn_handle* h, const CellDev& c, bool fold, const double* Y, double* Y
     g.nsplit = 1;
     gemm_general(h, g);
   } else {
-    i64 total = (i64)outer * c.nK * s;
+    i64 total = (i64)outer * c.nA * s;
     k_map_L_med<<<cdiv(total, 256), 256, 0, h->stream>>>(c, Y, Yk, outer, s);
     TN_LAUNCH_CHECK(h);
   }
@@ -513,7 +537,7 @@ void map_LT(tn_handle* h, const CellDev& c, bool fold, const double* Yk, double*
     g.nsplit = 1;
     gemm_general(h, g);
   } else {
-    i64 total = (i64)outer * c.n_l * c.n_i * s;
+    i64 total = (i64)outer * c.n_l * s;
     k_map_LT_med<<<cdiv(total, 256), 256, 0, h->stream>>>(c, Yk, Y, outer, s, 0, 0);
     TN_LAUNCH_CHECK(h);
   }
