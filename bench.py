@@ -341,7 +341,7 @@ STAGES = [  # (stats ms key, label, kernel, flop key, bytes key, bound)
      "flop_search_rblocks", None, "alu"),
     ("ms_search_cond", "search_cond", "k_cond<KP> (conditionals: A tile resident, dense operand through a cp.async double buffer; Z fused in the epilogue)",
      "flop_search_cond", "bytes_search_cond", "tensor"),
-    ("ms_search_select", "search_select", "k_sel_hist (sample) + k_sel_prefilter + k_csel_* + bitonic (top-M)", None,
+    ("ms_search_select", "search_select", "k_sel_hist_rows (bound from the row maxima of V) + k_sel_prefilter (reads only rows that reach it) + k_csel_* + bitonic (top-M)", None,
      "bytes_search_select", "hbm"),
     ("ms_tables", "tables", "k_tables", None, None, "hbm"),
 ]

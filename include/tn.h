@@ -107,6 +107,8 @@ enum {
   TN_OPT_TS_WIDE_ROWS = 23,         /* 1 (default) / 0: 24-row warp tiles in the streaming GEMM for 24..48 columns (tuning switch) */
   TN_OPT_RBLOCK_FACT = 24,          /* 1 (default) / 0: right blocks through the factorised contraction (sum over c_lo, then over b)
                                        instead of the joint GEMM over (b, c_lo) x (beam, a_hi) (0: reference route)            */
+  TN_OPT_SELECT_ROWS = 25,          /* 1 (default) / 0: top-M bound from the row maxima of V written by the conditional kernel and a
+                                       prefilter that reads only the rows that reach it (0: hashed 1/64 sample + full pass over V)  */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */

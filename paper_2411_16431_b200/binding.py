@@ -22,6 +22,7 @@ OPT_SVD_DIRECT = 21
 OPT_COND_PIPE = 22
 OPT_TS_WIDE_ROWS = 23
 OPT_RBLOCK_FACT = 24
+OPT_SELECT_ROWS = 25
 
 
 class TnError(RuntimeError):

@@ -117,9 +117,10 @@ struct CondArgs {
   double* V; const double *X, *vS, *Yc, *fc; const int *vrow, *slot;     // epilogue
   double* zpart; unsigned long long* nneg;
   int nB, tshift, ntile, Mg; i64 per_m;
+  double* rowmax;    // [m][Mg]: largest entry of every row of V (0 if none is positive); the selection reads it first
 };
 template <int KP>
-__global__ void __launch_bounds__(256) k_cond(CondArgs a) {
+__global__ void __launch_bounds__(256, 3) k_cond(CondArgs a) {
   constexpr int BM = 128, NT = 4, BN = 8 * NT, LDA = smem_ld(KP), LDB = smem_ld(BN);
   extern __shared__ __align__(16) double cond_smem[];
   double* sA = cond_smem;
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(256) k_cond(CondArgs a) {
   // row descriptors of this thread's two rows
   const int row0 = m0 + 16 * warp + (lane >> 2), row1 = row0 + 8;
   const int sl = a.slot[m];
-  double w[2], f[2], z[2] = {0.0, 0.0};
+  double w[2], f[2], z[2] = {0.0, 0.0}, vmx[2] = {0.0, 0.0};
   const double* xr[2];
   double* vp[2];
   unsigned neg = 0;
@@ -212,8 +213,19 @@ __global__ void __launch_bounds__(256) k_cond(CondArgs a) {
         const double o0 = acc[i][j][0] * s, o1 = acc[i][j][1] * s;
         *reinterpret_cast<double2*>(vp[i] + col) = make_double2(o0, o1);     // N even, col even
         z[i] += fmax(o0, 0.0) + fmax(o1, 0.0);
+        vmx[i] = fmax(vmx[i], fmax(o0, o1));                                 // (fmax ignores NaNs)
         neg += (o0 >= 0.0 ? 0u : 1u) + (o1 >= 0.0 ? 0u : 1u);               // negatives and NaNs (reading S7)
       }
+    }
+  }
+  if (a.rowmax) {   // the four lanes that share a row
+#pragma unroll
+    for (int i = 0; i < 2; i++) {
+      double v = vmx[i];
+      v = fmax(v, __shfl_xor_sync(0xffffffffu, v, 1));
+      v = fmax(v, __shfl_xor_sync(0xffffffffu, v, 2));
+      const int row = i ? row1 : row0;
+      if ((lane & 3) == 0 && row < a.Mg) a.rowmax[(i64)m * a.Mg + row] = v;
     }
   }
   // ordered CTA reduction -> one partial per (m, row tile)
@@ -629,6 +641,28 @@ __global__ void k_sel_collect(SelArgs a, const SelState* st, Raw* out, unsigned*
     }
   }
 }
+// Histogram of one radix digit of the keys of the ROW MAXIMA (one candidate per row (m, b, c_lo): the row's largest entry
+// with its best c_hi).  A subset of the candidates, so its (M+1)-th largest key is a lower bound of the true (M+1)-th
+// largest -- the prefilter threshold -- from 8 bytes per row (written by k_cond) instead of a scattered sample of V.
+__global__ void k_sel_hist_rows(const double* rowmax, const double* scale, const double* fmx, int nb, int Mg, int nCl,
+                                const SelState* st, int shift, int nbits, int first, unsigned* hist) {
+  __shared__ unsigned sh[4096];
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sh[i] = 0;
+  __syncthreads();
+  const unsigned long long prefix = st->prefix;
+  const i64 total = (i64)nb * Mg;
+  for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+    const int m = (int)(t / Mg), cl = (int)(t % Mg) % nCl;
+    const double r = rowmax[t] * scale[m] * fmx[(i64)m * nCl + cl];
+    if (!(r > 0.0)) continue;
+    const unsigned long long key = (unsigned long long)__double_as_longlong(r);
+    if (!first && (key >> (shift + nbits)) != prefix) continue;
+    atomicAdd(&sh[(key >> shift) & ((1u << nbits) - 1)], 1u);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x)
+    if (sh[i]) atomicAdd(&hist[i], sh[i]);
+}
 // fmx[m][cl] = max_ch fcd(m, cl, ch): upper bound used to reject whole (m,i,a) entries with one compare
 __global__ void k_sel_fmax(SelArgs a, double* fmx, int* chbest = nullptr) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -646,7 +680,7 @@ __global__ void k_sel_fmax(SelArgs a, double* fmx, int* chbest = nullptr) {
 // Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).  Grid (chunk, m),
 // 16-byte loads, shifts instead of divisions (nA, nCl powers of two); survivors are rare.
 __global__ void __launch_bounds__(256) k_sel_prefilter(SelArgs a, int lgA, const SelState* st, const double* fmx, double* keys,
-                                                       Raw* out, unsigned* count, unsigned cap) {
+                                                       Raw* out, unsigned* count, unsigned cap, const double* rowmax = nullptr) {
   double thr = __longlong_as_double((long long)st->thresh);
   thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
   const int m = blockIdx.y, nchunk = gridDim.x;
@@ -655,9 +689,11 @@ __global__ void __launch_bounds__(256) k_sel_prefilter(SelArgs a, int lgA, const
   const double2* v2 = reinterpret_cast<const double2*>(a.V + (i64)m * a.per_m);
   const double sc = a.scale[m];
   const double* fm = fmx + (i64)m * a.nCl;
+  const double* rmx = rowmax ? rowmax + (i64)m * (a.per_m >> lgA) : nullptr;
   for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
-    const double2 x = v2[q];
     const int i = (int)((2 * q) >> lgA), cl = i & (a.nCl - 1);
+    if (rmx && !(rmx[i] * sc * fm[cl] >= thr)) continue;      // nothing in this row reaches the bound: V is not read
+    const double2 x = v2[q];
     const double bound = fmax(x.x, x.y) * sc * fm[cl];
     if (!(bound >= thr) || !(bound > 0.0)) continue;
 #pragma unroll
@@ -1451,6 +1487,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       const i64 per_m = (i64)c.nB * c.nCl * c.nA;
       Tic t_c(h, &h->st.ms_search_cond);
       DBuf<double> LG(h, (size_t)nb * npp * Dr), V(h, (size_t)nb * per_m);
+      DBuf<double> rowmax(h, (size_t)nb * c.nB * c.nCl);   // largest entry of every row of V (written by k_cond)
+      bool have_rowmax = false;
       k_hrow<<<cdiv(nb, 256), 256, 0, h->stream>>>(st_cur, ncell, nb, cellidx, x, ns, h->d_cells, hrow.p);
       TN_LAUNCH_CHECK(h);
       k_fc<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(c, drow.p + (size_t)x * nb_row, sl_cur, nb, fc.p);
@@ -1481,8 +1519,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         EpPV ep{V.p, c.X, c.BvS, c.Yc, fc.p, vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p,
                 c.nA, c.nB, c.nCl, c.tshift, ntile, per_m};
         CondArgs ca{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr, RMc.p, c.nA, V.p, c.X, c.BvS, c.Yc, fc.p,
-                    vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p, c.nB, c.tshift, ntile, Mg, per_m};
+                    vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p, c.nB, c.tshift, ntile, Mg, per_m,
+                    h->select_rows ? rowmax.p : nullptr};
         if (h->cond_pipe && launch_cond(h, nb, ca)) {
+          have_rowmax = h->select_rows != 0;
           k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
           TN_LAUNCH_CHECK(h);
         } else if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
@@ -1702,23 +1742,34 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       if (cand_sorted) {
         // nothing: the merged route produced the sorted candidate list
       } else if (!direct) {
-        // (1) lower bound of the (M+1)-th largest key from a hashed 1/64 sample of V (two radix digits)
+        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
+        TN_LAUNCH_CHECK(h);
+        // (1) lower bound of the (M+1)-th largest key from a SUBSET of the candidates (two radix digits): the row maxima
+        //     that k_cond wrote (one candidate per row of V), else a hashed 1/64 sample of V
         for (int pass = 0; pass < 2; pass++) {
-          k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
+          if (have_rowmax) {
+            const int Mg = c.nB * c.nCl;
+            k_sel_hist_rows<<<(unsigned)std::min<i64>((i64)h->sms * 8, ((i64)nb * Mg + 255) / 256), 256, 0, h->stream>>>(
+                rowmax.p, scale.p, fmx.p, nb, Mg, c.nCl, sel.p, shifts[pass], nbitsv[pass], pass == 0, hist.p);
+          } else {
+            k_sel_hist<<<gsel, 256, 0, h->stream>>>(sa, sel.p, shifts[pass], nbitsv[pass], pass == 0, 6, hist.p);
+          }
           TN_LAUNCH_CHECK(h);
           k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, 0ull);
           TN_LAUNCH_CHECK(h);
         }
-        // (2) one pass over V: everything at or above the bound goes to the compact list
-        k_sel_fmax<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(sa, fmx.p);
-        TN_LAUNCH_CHECK(h);
+        // (2) one pass over V (only the rows whose maximum reaches the bound are read when the row maxima are there):
+        //     everything at or above the bound goes to the compact list
         TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
         {
           int lgA = 0;
           while ((1 << lgA) < c.nA) lgA++;
           const int nchunk = (int)std::max<i64>(1, std::min<i64>(64, per_m / 8192));
-          k_sel_prefilter<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap);
-          h->st.bytes_search_select += 8.0 * nb * (double)per_m * (1.0 + 2.0 / 64.0);
+          k_sel_prefilter<<<dim3(nchunk, nb), 256, 0, h->stream>>>(sa, lgA, sel.p, fmx.p, ckeys.p, craw.p, count.p, ccap,
+                                                                   have_rowmax ? rowmax.p : nullptr);
+          // algorithmic bytes: with the row maxima 8 B per row (three times) instead of one read of V + the sample
+          h->st.bytes_search_select += have_rowmax ? 3.0 * 8.0 * nb * (double)c.nB * c.nCl
+                                                   : 8.0 * nb * (double)per_m * (1.0 + 2.0 / 64.0);
         }
         TN_LAUNCH_CHECK(h);
         const unsigned n1 = d2h(h, count.p);

@@ -132,3 +132,23 @@ def test_factorised_right_blocks_against_the_joint_gemm(Ly, Lx, S, ns, p, seed, 
     assert abs(out[0][0] - out[1][0]) <= 1e-12 * abs(out[0][0])
     assert np.array_equal(out[0][1], out[1][1])
     assert np.allclose(out[0][2], out[1][2], rtol=1e-11, atol=0) and abs(out[0][3] - out[1][3]) <= 1e-11 * abs(out[0][3])
+
+
+@pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,D,M", [(3, 3, 3, 4, 0.9, 4, 6, 64), (3, 4, 2, 8, 0.97, 3, 12, 256),
+                                                 (3, 4, 2, 4, 0.95, 2, 5, 7)])
+def test_row_maxima_selection_bound_gives_the_same_lists(Ly, Lx, S, ns, p, seed, D, M):
+    """The top-M bound from the row maxima of V (written by k_cond) + the row-skipping prefilter (TN_OPT_SELECT_ROWS = 1,
+    the default) against the hashed 1/64 sample + full pass over V (0): any subset of the candidates gives a valid lower
+    bound, so the selected lists must be IDENTICAL (bitwise), not merely close.  The sampled route is forced."""
+    import paper_2411_16431_b200 as tnb
+    inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
+    out = []
+    for rows in (1, 0):
+        with tnb.TensorNetwork(inst) as t:
+            t.set_option(tnb.OPT_SELECT_ROWS, rows)
+            t.set_option(tnb.OPT_SELECT_DIRECT_MAX, 0)
+            t.set_beta(1.2)
+            t.contract(D, 1)
+            states, E, logp, pd = t.branch_and_bound(M)
+            out.append((states, logp, pd))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]) and out[0][2] == out[1][2]
