@@ -64,6 +64,8 @@ def parse_args():
     ap.add_argument("--schedule", default="zipper-then-sweeps", choices=["zipper-then-sweeps", "interleaved"],
                     help="TN_OPT_SCHEDULE: variant (ii) of PAPER.md:179 (default) or a sweep after every zipper step")
     ap.add_argument("--oversample", type=int, default=None, help="TN_OPT_OVERSAMPLE (extra block columns of the SVD)")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="tn_set_option by numeric key (tuning switches of include/tn.h), e.g. --opt 26=0")
     ap.add_argument("--two-step", action="store_true", help="TN_OPT_TWO_STEP: zipper and passes at 2 D, then cut to D")
     ap.add_argument("--no-headline-fast", action="store_true",
                     help="skip the second one-step record of configs[3], taken in the paper's own mode (seeded randomized "
@@ -625,6 +627,9 @@ def set_contract_options(tnb, t, args, svd_mode=None):
         t.set_option(tnb.OPT_TWO_STEP, 1)
     if args.oversample is not None:
         t.set_option(tnb.OPT_OVERSAMPLE, args.oversample)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        t.set_option(int(k), float(v))
 
 
 def headline_record(tnb, instances, args, step, timed, fp64_peak, peaks, peak_src, local, svd_mode=None):

@@ -109,6 +109,9 @@ enum {
                                        instead of the joint GEMM over (b, c_lo) x (beam, a_hi) (0: reference route)            */
   TN_OPT_SELECT_ROWS = 25,          /* 1 (default) / 0: top-M bound from the row maxima of V written by the conditional kernel and a
                                        prefilter that reads only the rows that reach it (0: hashed 1/64 sample + full pass over V)  */
+  TN_OPT_LAZY_V = 26,               /* 1 (default) / 0: the conditional kernel does not write V; once the selection bound is known
+                                       the rows that reach it are recomputed and written (no merge / droplets; needs
+                                       TN_OPT_SELECT_ROWS and the pipelined conditional kernel) */
   TN_OPT_SELECT_DIRECT_MAX = 6 /* top-M selection: candidate counts up to this run the radix passes straight on
                              all candidates; above it a hashed 1/64 sample gives a lower bound of the (M+1)-th
                              key first and one prefilter pass compacts the survivors (default 2^22)  */

@@ -10,7 +10,7 @@ from .binding import (TnError, TensorNetwork, lib, tn_branch_and_bound, tn_contr
                       tn_row_lognorm, tn_set_allocator, tn_set_beta, tn_set_option, tn_set_stream, TnStats,
                       EXPORTED_SYMBOLS, OPT_GAP_GUARD, OPT_SVD_TOL, OPT_SVD_MAXIT, OPT_OVERSAMPLE, OPT_EXACT_CAP, OPT_SELECT_DIRECT_MAX, OPT_SVD_CHEB, OPT_SVD_LOCK, OPT_MERGE, OPT_MERGE_CAP,
                       OPT_SCHEDULE, OPT_SWEEP_RANGE, OPT_SVD_MODE, OPT_RSVD_ITERS, OPT_TWO_STEP,
-                      OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT, OPT_MERGE_SEGMENTED, OPT_SVD_DIRECT, OPT_COND_PIPE, OPT_TS_WIDE_ROWS, OPT_RBLOCK_FACT, OPT_SELECT_ROWS, tn_droplets, tn_gemm_t_static,
+                      OPT_DROPLETS, OPT_DROPLET_MAX_DE, OPT_DROPLET_MIN_HAMMING, OPT_DROPLET_MAX_COUNT, OPT_MERGE_SEGMENTED, OPT_SVD_DIRECT, OPT_COND_PIPE, OPT_TS_WIDE_ROWS, OPT_RBLOCK_FACT, OPT_SELECT_ROWS, OPT_LAZY_V, tn_droplets, tn_gemm_t_static,
                       tn_lbp, tn_lbp_message, tn_lbp_marginals, tn_lbp_select)
 
 __all__ = [n for n in dir() if not n.startswith("_")]

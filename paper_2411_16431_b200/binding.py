@@ -23,6 +23,7 @@ OPT_COND_PIPE = 22
 OPT_TS_WIDE_ROWS = 23
 OPT_RBLOCK_FACT = 24
 OPT_SELECT_ROWS = 25
+OPT_LAZY_V = 26
 
 
 class TnError(RuntimeError):

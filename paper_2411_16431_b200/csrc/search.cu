@@ -118,6 +118,8 @@ struct CondArgs {
   double* zpart; unsigned long long* nneg;
   int nB, tshift, ntile, Mg; i64 per_m;
   double* rowmax;    // [m][Mg]: largest entry of every row of V (0 if none is positive); the selection reads it first
+  int store;         // 0: V is NOT written (lazy mode: k_cond_rows writes the rows that reach the selection bound later)
+  int tally;         // 0: Z partials and the negative count are not written (second run of the same cell)
 };
 template <int KP>
 __global__ void __launch_bounds__(256, 3) k_cond(CondArgs a) {
@@ -211,7 +213,7 @@ __global__ void __launch_bounds__(256, 3) k_cond(CondArgs a) {
         if (col >= N) continue;
         const double s = w[i] * xv[i][j];
         const double o0 = acc[i][j][0] * s, o1 = acc[i][j][1] * s;
-        *reinterpret_cast<double2*>(vp[i] + col) = make_double2(o0, o1);     // N even, col even
+        if (a.store) *reinterpret_cast<double2*>(vp[i] + col) = make_double2(o0, o1);     // N even, col even
         z[i] += fmax(o0, 0.0) + fmax(o1, 0.0);
         vmx[i] = fmax(vmx[i], fmax(o0, o1));                                 // (fmax ignores NaNs)
         neg += (o0 >= 0.0 ? 0u : 1u) + (o1 >= 0.0 ? 0u : 1u);               // negatives and NaNs (reading S7)
@@ -228,6 +230,7 @@ __global__ void __launch_bounds__(256, 3) k_cond(CondArgs a) {
       if ((lane & 3) == 0 && row < a.Mg) a.rowmax[(i64)m * a.Mg + row] = v;
     }
   }
+  if (!a.tally) return;
   // ordered CTA reduction -> one partial per (m, row tile)
   double tz = z[0] * f[0] + z[1] * f[1];
 #pragma unroll
@@ -677,6 +680,78 @@ __global__ void k_sel_fmax(SelArgs a, double* fmx, int* chbest = nullptr) {
   fmx[t] = mx;
   if (chbest) chbest[t] = best;
 }
+// ---- lazy V (round 2, TN_OPT_LAZY_V): k_cond ran with store = 0 (row maxima, Z and the negative count only: no 8 B per
+// entry to HBM); once the selection bound is known, this kernel recomputes the rows whose maximum reaches it and writes
+// them to their places in V, where the prefilter (same row test) and k_sel_score read them.  Same DMMA sequence per
+// entry as k_cond (k ascending in steps of 4 from a zero accumulator, then one multiply by the same weight), so the
+// recomputed entries equal the ones the row maxima came from.  Grid (row chunks of 1024, m); a warp takes 8 listed rows.
+template <int KP>
+__global__ void __launch_bounds__(256) k_cond_rows(CondArgs a, const SelState* st, const double* scale, const double* fmx) {
+  constexpr int NT = 4, BN = 8 * NT;
+  __shared__ int s_list[1024];
+  __shared__ int s_cnt;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int m = blockIdx.y, r0 = blockIdx.x * 1024, K = a.Dr, N = a.nA;
+  if (tid == 0) s_cnt = 0;
+  __syncthreads();
+  double thr = __longlong_as_double((long long)st->thresh);
+  thr = st->takeall ? 0.0 : thr * (1.0 - 1e-12);
+  const double sc = scale[m];
+  for (int r = r0 + tid; r < min(r0 + 1024, a.Mg); r += 256) {
+    const int cl = r % a.nCl;
+    if (a.rowmax[(i64)m * a.Mg + r] * sc * fmx[(i64)m * a.nCl + cl] >= thr) s_list[atomicAdd(&s_cnt, 1)] = r;   // the prefilter's test
+  }
+  __syncthreads();
+  const int cnt = s_cnt;
+  const double* Bm = a.RMc + (i64)m * K * N;
+  const int sl = a.slot[m];
+  for (int g = warp; g * 8 < cnt; g += 8) {
+    const int li = g * 8 + (lane >> 2);
+    const bool live = li < cnt;
+    const int row = live ? s_list[li] : 0, b = row / a.nCl, cl = row % a.nCl;
+    const double* src = a.LG + ((i64)m * a.npp + a.Pd[b] * a.n_o + a.Po[cl]) * K;
+    double fa[KP / 4];
+#pragma unroll
+    for (int q = 0; q < KP / 4; q++) {
+      const int k = 4 * q + (lane & 3);
+      fa[q] = (live && k < K) ? __ldg(src + k) : 0.0;
+    }
+    const double w = a.vS[(i64)a.vrow[sl] * a.nB + b] * a.Yc[b * a.nCl + cl];
+    const double* xr = a.X + b;
+    double* vp = a.V + (i64)m * a.per_m + (i64)row * N;
+    for (int n0 = 0; n0 < N; n0 += BN) {
+      double acc[NT][2];
+#pragma unroll
+      for (int j = 0; j < NT; j++) acc[j][0] = acc[j][1] = 0.0;
+#pragma unroll
+      for (int q = 0; q < KP / 4; q++) {
+        const int k = 4 * q + (lane & 3);
+#pragma unroll
+        for (int j = 0; j < NT; j++) {
+          const int col = n0 + 8 * j + (lane >> 2);
+          const double fb = (k < K && col < N) ? __ldg(Bm + (i64)k * N + col) : 0.0;
+          dmma884(acc[j][0], acc[j][1], fa[q], fb);
+        }
+      }
+      if (!live) continue;
+#pragma unroll
+      for (int j = 0; j < NT; j++) {
+        const int col = n0 + 8 * j + 2 * (lane & 3);
+        if (col >= N) continue;
+        const double s = w * __ldg(xr + (i64)(col >> a.tshift) * a.nB);
+        *reinterpret_cast<double2*>(vp + col) = make_double2(acc[j][0] * s, acc[j][1] * s);
+      }
+    }
+  }
+}
+static void launch_cond_rows(tn_handle* h, int nb, const CondArgs& a, const SelState* st, const double* scale, const double* fmx) {
+  const dim3 grid((unsigned)((a.Mg + 1023) / 1024), (unsigned)nb);
+  if (a.Dr <= 16) k_cond_rows<16><<<grid, 256, 0, h->stream>>>(a, st, scale, fmx);
+  else if (a.Dr <= 32) k_cond_rows<32><<<grid, 256, 0, h->stream>>>(a, st, scale, fmx);
+  else if (a.Dr <= 48) k_cond_rows<48><<<grid, 256, 0, h->stream>>>(a, st, scale, fmx);
+  else k_cond_rows<64><<<grid, 256, 0, h->stream>>>(a, st, scale, fmx);
+  TN_LAUNCH_CHECK(h);
+}
 // Prefilter pass over all of V: candidates with key >= thr go to the compact list (keys + Raw).  Grid (chunk, m),
 // 16-byte loads, shifts instead of divisions (nA, nCl powers of two); survivors are rare.
 __global__ void __launch_bounds__(256) k_sel_prefilter(SelArgs a, int lgA, const SelState* st, const double* fmx, double* keys,
@@ -689,10 +764,44 @@ __global__ void __launch_bounds__(256) k_sel_prefilter(SelArgs a, int lgA, const
   const double2* v2 = reinterpret_cast<const double2*>(a.V + (i64)m * a.per_m);
   const double sc = a.scale[m];
   const double* fm = fmx + (i64)m * a.nCl;
-  const double* rmx = rowmax ? rowmax + (i64)m * (a.per_m >> lgA) : nullptr;
+  if (rowmax) {
+    // one test per ROW (a lane per row, 32 rows per warp step); the warp then walks the rows that passed together, so
+    // the cost is the 8 B per row of the maxima plus the few rows that reach the bound
+    const double* rmx = rowmax + (i64)m * (a.per_m >> lgA);
+    const int nrows = (int)(a.per_m >> lgA), rpc = (nrows + nchunk - 1) / nchunk;
+    const int r0 = blockIdx.x * rpc, r1 = min(nrows, r0 + rpc);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, half = a.nA >> 1;
+    for (int base = r0 + 32 * warp; base < r1; base += 256) {
+      const int ri = base + lane;
+      unsigned mask = __ballot_sync(0xffffffffu, ri < r1 && rmx[ri] * sc * fm[ri & (a.nCl - 1)] >= thr);
+      while (mask) {
+        const int i = base + __ffs(mask) - 1, cl = i & (a.nCl - 1);
+        mask &= mask - 1;
+        for (int qq = lane; qq < half; qq += 32) {
+          const double2 x = v2[(i64)i * half + qq];
+          const double bound = fmax(x.x, x.y) * sc * fm[cl];
+          if (!(bound >= thr) || !(bound > 0.0)) continue;
+#pragma unroll
+          for (int e = 0; e < 2; e++) {
+            const double v = e ? x.y : x.x;
+            if (!(v > 0.0)) continue;
+            const double vs = v * sc;
+            const int aa = 2 * qq + e;
+            for (int ch = 0; ch < a.nCh; ch++) {
+              double r = vs * sel_fcd(a, m, cl, ch);
+              if (r > 0.0 && r >= thr) {
+                unsigned idx = atomicAdd(count, 1u);
+                if (idx < cap) { keys[idx] = r; out[idx] = Raw{m, i, aa, ch}; }
+              }
+            }
+          }
+        }
+      }
+    }
+    return;
+  }
   for (i64 q = c0 + threadIdx.x; q < c1; q += 256) {
     const int i = (int)((2 * q) >> lgA), cl = i & (a.nCl - 1);
-    if (rmx && !(rmx[i] * sc * fm[cl] >= thr)) continue;      // nothing in this row reaches the bound: V is not read
     const double2 x = v2[q];
     const double bound = fmax(x.x, x.y) * sc * fm[cl];
     if (!(bound >= thr) || !(bound > 0.0)) continue;
@@ -1489,6 +1598,9 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
       DBuf<double> LG(h, (size_t)nb * npp * Dr), V(h, (size_t)nb * per_m);
       DBuf<double> rowmax(h, (size_t)nb * c.nB * c.nCl);   // largest entry of every row of V (written by k_cond)
       bool have_rowmax = false;
+      bool lazy_v = false;                                 // V not written by k_cond: k_cond_rows fills the rows the selection reads
+      CondArgs ca_rows{};                                  // the conditional kernel's arguments, kept for that second kernel
+      std::unique_ptr<DBuf<double>> RMc_keep;              // its dense operand stays alive until then
       k_hrow<<<cdiv(nb, 256), 256, 0, h->stream>>>(st_cur, ncell, nb, cellidx, x, ns, h->d_cells, hrow.p);
       TN_LAUNCH_CHECK(h);
       k_fc<<<cdiv((i64)nb * c.nCl, 256), 256, 0, h->stream>>>(c, drow.p + (size_t)x * nb_row, sl_cur, nb, fc.p);
@@ -1509,7 +1621,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         h->st.flop_search += 2.0 * nb * (double)Mg * Ng * Dr;
         h->st.flop_search_cond += 2.0 * nb * (double)Mg * Ng * Dr;
         h->st.bytes_search_cond += 8.0 * nb * (double)per_m;
-        DBuf<double> RMc(h, (size_t)nb * Dr * c.nA);
+        RMc_keep.reset(new DBuf<double>(h, (size_t)nb * Dr * c.nA));
+        DBuf<double>& RMc = *RMc_keep;
         k_rmc<<<cdiv((i64)nb * Dr * c.nA, 256), 256, 0, h->stream>>>(rt[x].RM, sl_cur, c.Pr, c.BhS, c.wA, hrow.p, nb, Dr, c.n_r, c.nA, RMc.p);
         TN_LAUNCH_CHECK(h);
         ArPV ar{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
@@ -1520,16 +1633,23 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
                 c.nA, c.nB, c.nCl, c.tshift, ntile, per_m};
         CondArgs ca{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr, RMc.p, c.nA, V.p, c.X, c.BvS, c.Yc, fc.p,
                     vrow.p + (size_t)x * nb_row, sl_cur, zpart.p, nneg.p, c.nB, c.tshift, ntile, Mg, per_m,
-                    h->select_rows ? rowmax.p : nullptr};
+                    h->select_rows ? rowmax.p : nullptr, 1, 1};
+        // lazy V: only on the route that reads V through the row test (no merge, no droplets, not the direct passes)
+        lazy_v = h->lazy_v && h->select_rows && !h->merge && !h->droplets &&
+                 (i64)nb * per_m * c.nCh > (i64)h->select_direct_max;
+        ca.store = lazy_v ? 0 : 1;
         if (h->cond_pipe && launch_cond(h, nb, ca)) {
           have_rowmax = h->select_rows != 0;
+          ca_rows = ca;
+          if (lazy_v) h->st.bytes_search_cond += 8.0 * nb * ((double)npp * Dr + (double)Dr * c.nA + Mg) - 8.0 * nb * (double)per_m;
           k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
           TN_LAUNCH_CHECK(h);
-        } else if (launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep)) {
+        } else if ((lazy_v = false, launch_bgemm<false>(h, nb, Mg, Ng, Dr, ar, be, ep))) {
           // Z and the negative count came out of the GEMM epilogue: no extra pass over V
           k_beam_Z_final<<<cdiv(nb, 128), 128, 0, h->stream>>>(zpart.p, nb, ntile, Z.p);
           TN_LAUNCH_CHECK(h);
         } else {
+          lazy_v = false;
           LdPA a{LG.p, c.Pd, c.Po, c.nCl, c.n_o, npp, Dr};
           StPV e{V.p, c.BhS, c.wA, c.X, c.BvS, c.Yc, hrow.p, vrow.p + (size_t)x * nb_row, sl_cur, c.nA, c.nB, c.nCl, c.tshift, per_m};
           dim3 grid(nb, cdiv(Mg, 64), cdiv(Ng, 64));
@@ -1758,6 +1878,8 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           k_sel_resolve<<<1, 1024, 0, h->stream>>>(sel.p, hist.p, shifts[pass], nbitsv[pass], pass == 0, 0ull);
           TN_LAUNCH_CHECK(h);
         }
+        // lazy V: the rows that reach the bound are computed now (the others are never written, never read)
+        if (lazy_v) launch_cond_rows(h, nb, ca_rows, sel.p, scale.p, fmx.p);
         // (2) one pass over V (only the rows whose maximum reaches the bound are read when the row maxima are there):
         //     everything at or above the bound goes to the compact list
         TN_CUDA(cudaMemsetAsync(count.p, 0, sizeof(unsigned), h->stream));
@@ -1775,6 +1897,12 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
         const unsigned n1 = d2h(h, count.p);
         if (n1 > ccap) {
           direct = true;                              // massive ties at the bound: fall back to the direct passes
+          if (lazy_v) {                               // ... which read all of V: write it now (no second tally of Z)
+            ca_rows.store = 1;
+            ca_rows.tally = 0;
+            if (!launch_cond(h, nb, ca_rows)) tn_throw(TN_ERR_CUDA, "cell (%d,%d): lazy V could not be completed", y, x);
+            lazy_v = false;
+          }
         } else if (n1 <= cap) {
           ncand = n1;
           TN_CUDA(cudaMemcpyAsync(raw.p, craw.p, sizeof(Raw) * n1, cudaMemcpyDeviceToDevice, h->stream));

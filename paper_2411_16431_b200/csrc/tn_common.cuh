@@ -94,6 +94,7 @@ struct tn_handle {
   int drop_K = 0;
   int merge_segmented = 1;
   int ts_rpw3 = 1;          // TN_OPT_TS_WIDE_ROWS: 24-row warp tiles in k_tsgemm for 24..48 columns
+  int lazy_v = 1;           // TN_OPT_LAZY_V: V is not written by k_cond; k_cond_rows writes the rows the selection reads
   int select_rows = 1;      // TN_OPT_SELECT_ROWS: selection bound and prefilter through the row maxima of V
   int rblock_fact = 1;      // TN_OPT_RBLOCK_FACT: factorised right-block contraction (k_rblock_h)
   int cond_pipe = 1;        // TN_OPT_COND_PIPE: pipelined conditional GEMM (k_cond) where the shape fits

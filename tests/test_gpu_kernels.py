@@ -139,16 +139,21 @@ def test_factorised_right_blocks_against_the_joint_gemm(Ly, Lx, S, ns, p, seed, 
 def test_row_maxima_selection_bound_gives_the_same_lists(Ly, Lx, S, ns, p, seed, D, M):
     """The top-M bound from the row maxima of V (written by k_cond) + the row-skipping prefilter (TN_OPT_SELECT_ROWS = 1,
     the default) against the hashed 1/64 sample + full pass over V (0): any subset of the candidates gives a valid lower
-    bound, so the selected lists must be IDENTICAL (bitwise), not merely close.  The sampled route is forced."""
+    bound, so the selected lists must be IDENTICAL (bitwise), not merely close.  The sampled route is forced.
+    Lazy V (TN_OPT_LAZY_V = 1, the default: k_cond writes no V, k_cond_rows recomputes the rows that reach the bound) is
+    compared the same way: the recomputed entries are the ones the row maxima came from, so again bitwise."""
     import paper_2411_16431_b200 as tnb
     inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
     out = []
-    for rows in (1, 0):
+    for rows, lazy in ((1, 1), (1, 0), (0, 0)):
         with tnb.TensorNetwork(inst) as t:
             t.set_option(tnb.OPT_SELECT_ROWS, rows)
+            t.set_option(tnb.OPT_LAZY_V, lazy)
             t.set_option(tnb.OPT_SELECT_DIRECT_MAX, 0)
             t.set_beta(1.2)
             t.contract(D, 1)
             states, E, logp, pd = t.branch_and_bound(M)
-            out.append((states, logp, pd))
-    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]) and out[0][2] == out[1][2]
+            out.append((states, logp, pd, t.stats()["negative_u"]))
+    for o in out[1:]:
+        assert np.array_equal(out[0][0], o[0]) and np.array_equal(out[0][1], o[1]) and out[0][2] == o[2]
+        assert out[0][3] == o[3]
