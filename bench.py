@@ -339,8 +339,8 @@ STAGES = [  # (stats ms key, label, kernel, flop key, bytes key, bound)
      None, "tensor"),
     ("ms_orth_svd", "orth_svd", "k_orth_coop (Cholesky-QR rounds, one cooperative launch) + k_jacobi_rows (Rayleigh-Ritz)",
      "flop_orth_svd", None, "alu"),
-    ("ms_search_rblocks", "search_rblocks", "k_gather_Gy + k_rblock_h (right blocks, factorised: c_lo first, then b; plain FMA) + k_rs + k_tsgemm (Bh)",
-     "flop_search_rblocks", None, "alu"),
+    ("ms_search_rblocks", "search_rblocks", "k_gather_Gy + k_rblock_mma (right blocks, factorised: c_lo first, then b; two DMMA products per stage) + k_rs + k_tsgemm (Bh)",
+     "flop_search_rblocks", None, "tensor"),
     ("ms_search_cond", "search_cond", "k_cond<KP> (conditionals: A tile resident, dense operand through a cp.async double buffer; Z fused in the epilogue)",
      "flop_search_cond", "bytes_search_cond", "tensor"),
     ("ms_search_select", "search_select", "k_sel_hist_rows (bound from the row maxima of V) + k_sel_prefilter (reads only rows that reach it) + k_csel_* + bitonic (top-M)", None,

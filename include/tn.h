@@ -105,8 +105,9 @@ enum {
   TN_OPT_COND_PIPE = 22,            /* 1 (default) / 0: search conditionals through the pipelined kernel k_cond (0: the generic
                                        batched kernel, kept as the reference route for the kernel-level comparison)        */
   TN_OPT_TS_WIDE_ROWS = 23,         /* 1 (default) / 0: 24-row warp tiles in the streaming GEMM for 24..48 columns (tuning switch) */
-  TN_OPT_RBLOCK_FACT = 24,          /* 1 (default) / 0: right blocks through the factorised contraction (sum over c_lo, then over b)
-                                       instead of the joint GEMM over (b, c_lo) x (beam, a_hi) (0: reference route)            */
+  TN_OPT_RBLOCK_FACT = 24,          /* 1 (default) / 2 / 0: right blocks through the factorised contraction (sum over c_lo, then over b;
+                                       1: on the FP64 tensor cores, 2: the plain-FMA kernel) instead of the joint GEMM over
+                                       (b, c_lo) x (beam, a_hi) (0: reference route)                                            */
   TN_OPT_SELECT_ROWS = 25,          /* 1 (default) / 0: top-M bound from the row maxima of V written by the conditional kernel and a
                                        prefilter that reads only the rows that reach it (0: hashed 1/64 sample + full pass over V)  */
   TN_OPT_LAZY_V = 26,               /* 1 (default) / 0: the conditional kernel does not write V; once the selection bound is known

@@ -272,7 +272,7 @@ int tn_set_option(tn_handle* h, int32_t key, double v) {
     case TN_OPT_TS_WIDE_ROWS: h->ts_rpw3 = v != 0.0; break;
     case TN_OPT_SELECT_ROWS: h->select_rows = v != 0.0; break;
     case TN_OPT_LAZY_V: h->lazy_v = v != 0.0; break;
-    case TN_OPT_RBLOCK_FACT: h->rblock_fact = v != 0.0; break;
+    case TN_OPT_RBLOCK_FACT: h->rblock_fact = v == 2.0 ? 2 : v != 0.0; break;
     case TN_OPT_COND_PIPE: h->cond_pipe = v != 0.0; break;
     case TN_OPT_SVD_DIRECT: h->svd_direct = v != 0.0; break;
     case TN_OPT_MERGE_SEGMENTED: h->merge_segmented = v != 0.0; break;

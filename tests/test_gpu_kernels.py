@@ -115,13 +115,13 @@ def test_pipelined_conditional_kernel_against_the_generic_route(Ly, Lx, S, ns, p
 @pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,D", [(3, 3, 3, 4, 0.9, 4, 6), (3, 4, 2, 8, 0.97, 3, 12), (3, 4, 2, 4, 0.95, 2, 5),
                                                (3, 3, 3, 2, 0.85, 7, 4)])
 def test_factorised_right_blocks_against_the_joint_gemm(Ly, Lx, S, ns, p, seed, D):
-    """k_rblock_h (right blocks summed over c_lo first, then over b: TN_OPT_RBLOCK_FACT = 1, the default) against the
-    joint GEMM over (b, c_lo) x (beam, a_hi) (TN_OPT_RBLOCK_FACT = 0) on the same boundary MPS: identical states,
-    log-probabilities and log Z to rounding (another summation order)."""
+    """k_rblock_mma / k_rblock_h (right blocks summed over c_lo first, then over b: TN_OPT_RBLOCK_FACT = 1, the default, on
+    the tensor cores; 2: the plain-FMA kernel) against the joint GEMM over (b, c_lo) x (beam, a_hi) (TN_OPT_RBLOCK_FACT = 0)
+    on the same boundary MPS: identical states, log-probabilities and log Z to rounding (another summation order)."""
     import paper_2411_16431_b200 as tnb
     inst = instances.lattice(Ly, Lx, S, ns, p_keep=p, seed=seed)
     out = []
-    for fact in (1, 0):
+    for fact in (1, 2, 0):
         with tnb.TensorNetwork(inst) as t:
             t.set_option(tnb.OPT_RBLOCK_FACT, fact)
             t.set_beta(1.2)
@@ -129,9 +129,10 @@ def test_factorised_right_blocks_against_the_joint_gemm(Ly, Lx, S, ns, p, seed, 
             lz = t.log_z()
             states, E, logp, pd = t.branch_and_bound(64)
             out.append((lz, states, logp, pd))
-    assert abs(out[0][0] - out[1][0]) <= 1e-12 * abs(out[0][0])
-    assert np.array_equal(out[0][1], out[1][1])
-    assert np.allclose(out[0][2], out[1][2], rtol=1e-11, atol=0) and abs(out[0][3] - out[1][3]) <= 1e-11 * abs(out[0][3])
+    for o in out[1:]:
+        assert abs(out[0][0] - o[0]) <= 1e-12 * abs(out[0][0])
+        assert np.array_equal(out[0][1], o[1])
+        assert np.allclose(out[0][2], o[2], rtol=1e-11, atol=0) and abs(out[0][3] - o[3]) <= 1e-11 * abs(out[0][3])
 
 
 @pytest.mark.parametrize("Ly,Lx,S,ns,p,seed,D,M", [(3, 3, 3, 4, 0.9, 4, 6, 64), (3, 4, 2, 8, 0.97, 3, 12, 256),
