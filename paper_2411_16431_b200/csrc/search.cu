@@ -313,8 +313,9 @@ __global__ void k_gather_Gy(const double* G, const double* Yc, const int* Pd, co
   out[t] = Yc[kk] * G[(i64)(Pd[kk / nCl] * n_o + Po[kk % nCl]) * DD + i];
 }
 // The same factorised contraction on the FP64 tensor cores (round 2, the default; the plain-FMA kernel below stays as
-// TN_OPT_RBLOCK_FACT = 2 for the kernel-level comparison).  Per stage of BB = 8 values of b a CTA (64 values of i, 8 beam
-// elements) runs two small DMMA products with the intermediate in shared memory:
+// TN_OPT_RBLOCK_FACT = 2 for the kernel-level comparison).  Per stage of BB = 4 values of b a CTA (64 values of i, 8 beam
+// elements) runs two small DMMA products with the intermediate in shared memory; the G tile of the next stage arrives
+// through a cp.async double buffer meanwhile:
 //   phase 1  W_b[i][m] = sum_cl G[b][cl][i] fc[m][cl]          (A = G_b^T from shared memory, B = fc fragments in registers;
 //            the per-beam factor vS_m[b] is applied to the accumulator fragment on its way to shared memory)
 //   phase 2  H_m[i][t] += sum_b W[m][b][i] X[t][b]              (warp = beam element m; one k-step of 4 values of b per DMMA)
@@ -324,16 +325,29 @@ __global__ void __launch_bounds__(256, 2) k_rblock_mma(const double* __restrict_
                                                     const double* __restrict__ vS, const double* __restrict__ fc,
                                                     const int* __restrict__ vrow, int nb, int nB, int nCl, int nT, i64 DD,
                                                     double* __restrict__ H) {
-  constexpr int BI = 64, BMM = 8, BB = 8, LDI = BI + 4, LDM = BB * LDI + 2, LDX = 8 * NTB + 4;
+  constexpr int BI = 64, BMM = 8, BB = 4, LDI = BI + 4, LDM = BB * LDI + 2, LDX = 8 * NTB + 4;
   extern __shared__ __align__(16) double rb_smem[];
-  double* sG = rb_smem;                       // [BB][16][LDI]   G[b][cl][i]
-  double* sW = sG + BB * 16 * LDI;            // [BMM][LDM]      W[m][b][i]  (row b at b * LDI)
-  double* sX = sW + BMM * LDM;                // [BB][LDX]       X[t][b] of the stage
-  double* sV = sX + BB * LDX;                 // [BMM][BB]       vS[vrow m][b] of the stage
+  double* sG = rb_smem;                       // 2 x [BB][16][LDI]   G[b][cl][i], cp.async double buffer
+  double* sW = sG + 2 * BB * 16 * LDI;        // [BMM][LDM]          W[m][b][i]  (row b at b * LDI)
+  double* sX = sW + BMM * LDM;                // 2 x [BB][LDX]       X[t][b] of the stage
+  double* sV = sX + 2 * BB * LDX;             // 2 x [BMM][BB]       vS[vrow m][b] of the stage
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, q = lane & 3;
   const i64 i0 = (i64)blockIdx.x * BI;
   const int m0 = blockIdx.y * BMM;
   const int ks = (nCl + 3) >> 2, ncl4 = 4 * ks;        // k-steps of phase 1 (rows cl >= nCl are zero-filled)
+  // G tile of a stage: 16-byte cp.async (DD even, i0 a multiple of 64: a pair of i values is inside or outside together)
+  auto fetch = [&](int b0, int buf) {
+    double* dst = sG + buf * (BB * 16 * LDI);
+    for (int e = tid; e < BB * ncl4 * (BI / 2); e += 256) {
+      const int i2 = 2 * (e % (BI / 2)), cl = (e / (BI / 2)) % ncl4, bb = e / ((BI / 2) * ncl4);
+      const bool in = cl < nCl && b0 + bb < nB && i0 + i2 < DD;
+      const double* src = in ? Gy + ((i64)(b0 + bb) * nCl + cl) * DD + i0 + i2 : Gy;
+      unsigned sa = (unsigned)__cvta_generic_to_shared(dst + (bb * 16 + cl) * LDI + i2);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(src), "r"(in ? 16 : 0));
+    }
+    asm volatile("cp.async.commit_group;");
+  };
+  fetch(0, 0);
   double ff[4];                                        // B fragments of phase 1: fc[m0 + g][4 s + q]
 #pragma unroll
   for (int s4 = 0; s4 < 4; s4++) {
@@ -345,46 +359,48 @@ __global__ void __launch_bounds__(256, 2) k_rblock_mma(const double* __restrict_
   for (int ib = 0; ib < 8; ib++)
 #pragma unroll
     for (int tb = 0; tb < NTB; tb++) acc[ib][tb][0] = acc[ib][tb][1] = 0.0;
-  for (int b0 = 0; b0 < nB; b0 += BB) {
-    __syncthreads();
-    for (int e = tid; e < BB * ncl4 * BI; e += 256) {
-      const int ii = e % BI, cl = (e / BI) % ncl4, bb = e / (BI * ncl4);
-      const i64 gi = i0 + ii;
-      sG[(bb * 16 + cl) * LDI + ii] = (cl < nCl && b0 + bb < nB && gi < DD) ? Gy[((i64)(b0 + bb) * nCl + cl) * DD + gi] : 0.0;
+  int buf = 0;
+  for (int b0 = 0; b0 < nB; b0 += BB, buf ^= 1) {
+    // (sG[buf ^ 1] was last read in phase 1 of the previous stage, before that stage's second barrier)
+    if (b0 + BB < nB) {
+      fetch(b0 + BB, buf ^ 1);
+      asm volatile("cp.async.wait_group 1;");
+    } else {
+      asm volatile("cp.async.wait_group 0;");
     }
+    double* sXb = sX + buf * (BB * LDX);
+    double* sVb = sV + buf * (BMM * BB);
     for (int e = tid; e < BB * 8 * NTB; e += 256) {
       const int t = e % (8 * NTB), bb = e / (8 * NTB);
-      sX[bb * LDX + t] = (t < nT && b0 + bb < nB) ? X[(i64)t * nB + b0 + bb] : 0.0;
+      sXb[bb * LDX + t] = (t < nT && b0 + bb < nB) ? X[(i64)t * nB + b0 + bb] : 0.0;
     }
     if (tid < BMM * BB) {
       const int mm = tid / BB, bb = tid % BB, m = m0 + mm;
-      sV[mm * BB + bb] = (m < nb && b0 + bb < nB) ? vS[(i64)vrow[m] * nB + b0 + bb] : 0.0;
+      sVb[mm * BB + bb] = (m < nb && b0 + bb < nB) ? vS[(i64)vrow[m] * nB + b0 + bb] : 0.0;
     }
     __syncthreads();
+    const double* sGb = sG + buf * (BB * 16 * LDI);
     // phase 1: warp = block of 8 values of i, all BB values of b
-#pragma unroll 2
+#pragma unroll
     for (int bb = 0; bb < BB; bb++) {
       double c0 = 0.0, c1 = 0.0;
 #pragma unroll
       for (int s4 = 0; s4 < 4; s4++)
-        if (s4 < ks) dmma884(c0, c1, sG[(bb * 16 + 4 * s4 + q) * LDI + warp * 8 + g], ff[s4]);
+        if (s4 < ks) dmma884(c0, c1, sGb[(bb * 16 + 4 * s4 + q) * LDI + warp * 8 + g], ff[s4]);
       // accumulator fragment: row i = 8 warp + g, columns m = 2 q, 2 q + 1
-      sW[(2 * q) * LDM + bb * LDI + warp * 8 + g] = c0 * sV[(2 * q) * BB + bb];
-      sW[(2 * q + 1) * LDM + bb * LDI + warp * 8 + g] = c1 * sV[(2 * q + 1) * BB + bb];
+      sW[(2 * q) * LDM + bb * LDI + warp * 8 + g] = c0 * sVb[(2 * q) * BB + bb];
+      sW[(2 * q + 1) * LDM + bb * LDI + warp * 8 + g] = c1 * sVb[(2 * q + 1) * BB + bb];
     }
     __syncthreads();
-    // phase 2: warp = beam element
+    // phase 2: warp = beam element, one k-step (the BB = 4 values of b)
+    double fx[NTB];
 #pragma unroll
-    for (int k4 = 0; k4 < BB / 4; k4++) {
-      double fx[NTB];
+    for (int tb = 0; tb < NTB; tb++) fx[tb] = sXb[q * LDX + tb * 8 + g];
 #pragma unroll
-      for (int tb = 0; tb < NTB; tb++) fx[tb] = sX[(4 * k4 + q) * LDX + tb * 8 + g];
+    for (int ib = 0; ib < 8; ib++) {
+      const double fa = sW[warp * LDM + q * LDI + ib * 8 + g];
 #pragma unroll
-      for (int ib = 0; ib < 8; ib++) {
-        const double fa = sW[warp * LDM + (4 * k4 + q) * LDI + ib * 8 + g];
-#pragma unroll
-        for (int tb = 0; tb < NTB; tb++) dmma884(acc[ib][tb][0], acc[ib][tb][1], fa, fx[tb]);
-      }
+      for (int tb = 0; tb < NTB; tb++) dmma884(acc[ib][tb][0], acc[ib][tb][1], fa, fx[tb]);
     }
   }
   const int m = m0 + warp;
@@ -405,8 +421,8 @@ __global__ void __launch_bounds__(256, 2) k_rblock_mma(const double* __restrict_
 template <int NTB>
 static void launch_rblock_mma(tn_handle* h, dim3 grid, const double* Gy, const double* X, const double* vS, const double* fc,
                               const int* vrow, int nb, int nB, int nCl, int nT, i64 DD, double* H) {
-  constexpr int BI = 64, BMM = 8, BB = 8, LDI = BI + 4, LDM = BB * LDI + 2, LDX = 8 * NTB + 4;
-  constexpr int smem = (int)sizeof(double) * (BB * 16 * LDI + BMM * LDM + BB * LDX + BMM * BB);
+  constexpr int BI = 64, BMM = 8, BB = 4, LDI = BI + 4, LDM = BB * LDI + 2, LDX = 8 * NTB + 4;
+  constexpr int smem = (int)sizeof(double) * (2 * BB * 16 * LDI + BMM * LDM + 2 * BB * LDX + 2 * BMM * BB);
   TN_SMEM_OPT_IN(h, k_rblock_mma<NTB>, smem);
   k_rblock_mma<NTB><<<grid, 256, smem, h->stream>>>(Gy, X, vS, fc, vrow, nb, nB, nCl, nT, DD, H);
   TN_LAUNCH_CHECK(h);
@@ -1650,9 +1666,10 @@ void run(tn_handle* h, int M, bool logz_only, int* n_out, int8_t* states_out, do
           k_gather_Gy<<<cdiv((i64)Kg * DD, 256), 256, 0, h->stream>>>(rt[x].G, c.Yc, c.Pd, c.Po, c.nCl, c.n_o, DD, Kg, Gy.p);
           TN_LAUNCH_CHECK(h);
           dim3 grid((unsigned)cdiv(DD, 64), (unsigned)cdiv(nb, 8));
-          if (h->rblock_fact != 2 && c.nT <= 8)
+          const bool mma = h->rblock_fact != 2 && (DD & 1) == 0;     // 16-byte cp.async rows
+          if (mma && c.nT <= 8)
             launch_rblock_mma<1>(h, grid, Gy.p, c.X, c.BvS, fcx.p, vrow.p + (size_t)x * nb, nb, c.nB, c.nCl, c.nT, DD, H.p);
-          else if (h->rblock_fact != 2)
+          else if (mma)
             launch_rblock_mma<2>(h, grid, Gy.p, c.X, c.BvS, fcx.p, vrow.p + (size_t)x * nb, nb, c.nB, c.nCl, c.nT, DD, H.p);
           else if (c.nT <= 4)
             k_rblock_h<4><<<grid, 256, 0, h->stream>>>(Gy.p, c.X, c.BvS, fcx.p, vrow.p + (size_t)x * nb, nb, c.nB, c.nCl, c.nT, DD, H.p);
